@@ -1,0 +1,178 @@
+/*
+ * stroke_expand.h -- C-ABI of the B200 (sm_100a) stroke-expansion library.
+ *
+ * What the library computes: "GPU-friendly Stroke Expansion" (arxiv 2405.00127, PAPER.md): every
+ * input path segment (line / quadratic / cubic Bezier, fp32) of a stroked path is expanded, fully in
+ * parallel, into the records of a strongly-correct outline: the two parallel curves
+ * at +-half-width flattened to lines (section 4) or circular arcs (section 5)
+ * through an Euler-spiral intermediate (section 7, Alg. 2), evolute patches where curvature
+ * exceeds 1/half-width (section 6), joins and caps (Alg. 1).
+ *
+ * Pipeline behind these calls: (a) tag-stream scan  (b) per-segment count
+ * (c) allocation scan  (d) write.  All of it runs in hand-written CUDA kernels; there is no CPU path.
+ *
+ * Conventions
+ *  - Every function returns an sx_status (0 = OK, < 0 = error).  No exception crosses the boundary.
+ *  - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  The caller owns every buffer it
+ *    passes; the library never frees caller memory.  The context owns its scratch buffers.
+ *  - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls are
+ *    asynchronous on that stream unless stated otherwise.
+ *  - One sx_ctx serves one stream at a time (it holds the scratch of the call in flight).
+ */
+#ifndef STROKE_EXPAND_H
+#define STROKE_EXPAND_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ------------------------------------------------------------------ status codes */
+typedef int32_t sx_status;
+enum {
+    SX_OK = 0,
+    SX_E_INVALID_ARG = -1, /* null pointer, size out of range, mode/tolerance/affine invalid           */
+    SX_E_BAD_STREAM = -2,  /* malformed tag stream, detected on the device (see sx_count)              */
+    SX_E_CAPACITY = -3,    /* output buffer smaller than the record count                              */
+    SX_E_CUDA = -4,        /* a CUDA runtime call failed; sx_strerror gives cudaGetErrorString text    */
+    SX_E_STATE = -5        /* sx_write without a preceding successful sx_count                         */
+};
+
+/* ------------------------------------------------------------------ input encoding (PAPER.md 8.2, L460-489)
+ * Tag stream: one byte per input segment (Table 1):
+ *   bits 0-1  coordinate count: 1 line, 2 quadratic, 3 cubic (0 is invalid)
+ *   bit 2     subpath end: set on the last segment of a subpath
+ *   bit 3     must be 0 (16-bit coordinates are not supported; fp32 only)
+ *   bit 4     path end: set on the last segment of a path (implies subpath end)
+ *   bits 5,6  ignored (one transform per call; the style is indexed by path)
+ *   bit 7     closed subpath; meaningful on a subpath-end tag (reading R-8: the paper
+ *             leaves bit 7 unused and does not say how open/closed reaches the shader).  The caller
+ *             supplies the closing segment, as the paper's encoder does (L483); there is no
+ *             stroke-cap-marker segment: the scan gives every segment its subpath's first segment.
+ * Point stream (L464, L470, L483): float2.  Segment i reads points pt_off[i] .. pt_off[i]+count_i
+ *   (its first point is the previous segment's last) and pt_off[i+1] = pt_off[i] + count_i +
+ *   subpath_end_i.  A subpath of k segments owns 1 + sum(count) points.
+ * Style: one per path.  half-width = width/2 * sqrt|det(affine)| (R-14).  width <= 0 or non-finite:
+ *   the path emits no records (not an error). */
+typedef struct {
+    float width;
+    float miter_limit; /* SVG definition: miter used while 1/sin(beta/2) <= miter_limit              */
+    uint8_t join;      /* SX_JOIN_*                                                                   */
+    uint8_t cap;       /* SX_CAP_*                                                                    */
+    uint16_t _pad;
+    uint32_t _rsv;
+} sx_style; /* 16 bytes */
+
+enum { SX_JOIN_MITER = 0, SX_JOIN_ROUND = 1, SX_JOIN_BEVEL = 2 };
+enum { SX_CAP_BUTT = 0, SX_CAP_SQUARE = 1, SX_CAP_ROUND = 2 };
+enum { SX_MODE_LINE = 0, SX_MODE_ARC = 1 };
+
+/* ------------------------------------------------------------------ output records
+ * Records are grouped by input segment, in segment order (hence by path); path_offsets[p] is the
+ * index of path p's first record and path_offsets[n_paths] the total (this replaces the paper's
+ * per-record 32-bit path id, L452-458).  Within a segment the order is canonical:
+ * for every Euler-spiral piece in increasing t: [-h side, forward][+h side, mirrored]; then the
+ * join [-h side][+h side], or on the last segment of an open subpath [end cap][start cap].
+ * All outlines are positively oriented (winding numbers >= 0, L197). */
+typedef struct { float x0, y0, x1, y1; } sx_line; /* SX_MODE_LINE: 16 bytes, one 16-byte store */
+
+typedef struct {
+    float x0, y0, x1, y1;
+    float angle;   /* signed turning from start tangent to end tangent, CCW positive; 0 = straight.
+                      (The paper stores curvature, L452: kappa = 2 sin(angle/2) / |p1 - p0|.)        */
+    uint32_t seg;  /* source segment index                                                         */
+    uint32_t kind; /* SX_KIND_* | SX_KIND_PLUS                                                     */
+    uint32_t _pad;
+} sx_arc; /* SX_MODE_ARC: 32 bytes, two 16-byte stores */
+
+enum {
+    SX_KIND_OFFSET = 0,     /* parallel curve, regular range                                          */
+    SX_KIND_OFFSET_REV = 1, /* parallel curve over a super-critical range, reversed (L191, L403)      */
+    SX_KIND_EVOLUTE = 2,    /* evolute, output twice (L197)                                           */
+    SX_KIND_CONNECTOR = 3,  /* offset <-> evolute connecting line, output twice (L197)                */
+    SX_KIND_JOIN_OUTER = 4,
+    SX_KIND_JOIN_INNER = 5, /* through the vertex (strong correctness, L35)                           */
+    SX_KIND_CAP = 6,
+    SX_KIND_PLUS = 8        /* flag: record belongs to the +h side                                    */
+};
+
+/* ------------------------------------------------------------------ context */
+typedef struct sx_ctx sx_ctx;
+
+/* Create a context on CUDA device `device` (host-synchronous).  Fails with SX_E_CUDA when no usable
+ * device exists: there is no CPU fallback. */
+sx_status sx_create(sx_ctx** out, int32_t device);
+/* Free the context and its scratch (host-synchronous). */
+sx_status sx_destroy(sx_ctx* ctx);
+
+/* ------------------------------------------------------------------ phase 1: scan + count + scan
+ * Runs kernels (a) tag-stream scan, (b) per-segment count (Alg. 1/2 without the
+ * writes) and (c) the allocation scan.
+ *   d_tags[n_tags], d_points_xy[2*n_points], d_styles[n_paths]   device, read-only
+ *   h_affine[6]   HOST, row-major a b c d e f:  x' = a x + c y + e,  y' = b x + d y + f (L462);
+ *                 must be finite and non-singular
+ *   tolerance     > 0, device px (L37).  Internally split 0.1 / 0.8 between the cubic->Euler-spiral
+ *                 fit and the flattening (R-13)
+ *   d_path_offsets[n_paths+1]  device, written: first record index of every path, then the total
+ *   h_total       HOST, optional.  When non-NULL the call synchronises the stream, checks the
+ *                 device-side stream validation and writes the record count; SX_E_BAD_STREAM is
+ *                 returned here (coordinate count 0, bit 3 set, last tag without path end,
+ *                 sum(count+end) != n_points, path-end count != n_paths).  When NULL the call stays
+ *                 asynchronous and a bad stream yields zero records; sx_write reports the error.
+ * n_tags, n_points < 2^32.  n_tags == 0 is valid only with n_paths == 0 (total = 0).
+ * The input pointers must stay valid until the matching sx_write has completed. */
+sx_status sx_count(sx_ctx* ctx, const uint8_t* d_tags, uint64_t n_tags, const float* d_points_xy, uint64_t n_points,
+                   const sx_style* d_styles, uint64_t n_paths, const float* h_affine, float tolerance, int32_t mode,
+                   uint64_t* d_path_offsets, uint64_t* h_total, void* cuda_stream);
+
+/* ------------------------------------------------------------------ phase 2: write
+ * Kernel (d): writes the records of the preceding sx_count into d_out_records (sx_line[] or sx_arc[]
+ * by mode, 16-byte aligned) of capacity cap_records.  SX_E_CAPACITY if the capacity is known to be
+ * too small (the total is known on the host only when sx_count was given h_total; otherwise the
+ * kernel itself refuses to write past the capacity and the error is reported by sx_last_error after
+ * a stream sync). */
+sx_status sx_write(sx_ctx* ctx, void* d_out_records, uint64_t cap_records, void* cuda_stream);
+
+/* ------------------------------------------------------------------ one-shot, device buffers
+ * sx_count + allocate + sx_write.  `alloc` is called once (host side, after the count is known) and
+ * must return a device pointer of at least `bytes` bytes, 16-byte aligned, valid on `cuda_stream`
+ * (e.g. the torch caching allocator); NULL means allocation failure (SX_E_CAPACITY).  The result
+ * buffer belongs to the caller.  Synchronises the stream once (to read the 8-byte total). */
+typedef void* (*sx_alloc_fn)(uint64_t bytes, void* user);
+sx_status stroke_expand(sx_ctx* ctx, const uint8_t* d_tags, uint64_t n_tags, const float* d_points_xy, uint64_t n_points,
+                        const sx_style* d_styles, uint64_t n_paths, const float* h_affine, float tolerance, int32_t mode,
+                        sx_alloc_fn alloc, void* user, void** d_out_records, uint64_t* h_n_records,
+                        uint64_t* d_path_offsets, void* cuda_stream);
+
+/* ------------------------------------------------------------------ one-shot, HOST buffers (end to end)
+ * Same computation with every buffer on the host (pinned memory gives asynchronous copies): copies
+ * the streams to the device, runs the four kernels, copies records and path offsets back.
+ * h_out_records has room for cap_records records; *h_n_records receives the count even when
+ * SX_E_CAPACITY is returned (so the caller can retry).  Returns after the results are in host memory. */
+sx_status stroke_expand_host(sx_ctx* ctx, const uint8_t* h_tags, uint64_t n_tags, const float* h_points_xy, uint64_t n_points,
+                             const sx_style* h_styles, uint64_t n_paths, const float* h_affine, float tolerance, int32_t mode,
+                             void* h_out_records, uint64_t cap_records, uint64_t* h_n_records, uint64_t* h_path_offsets,
+                             void* cuda_stream);
+
+/* ------------------------------------------------------------------ introspection
+ * Device pointers into the context's scratch of the last sx_count (valid until the next call on the
+ * context): the tag-scan results and the per-segment record counts / offsets.  Any out pointer may
+ * be NULL.  Used by the parity tests and the bench report. */
+sx_status sx_segment_info(sx_ctx* ctx, const uint32_t** d_pt_off, const uint32_t** d_path_idx, const uint32_t** d_sp_first,
+                          const uint32_t** d_seg_count, const uint64_t** d_seg_offset);
+
+/* Device-side error state of the last call(s) on the context; synchronises `cuda_stream`. Returns
+ * SX_OK, SX_E_BAD_STREAM or SX_E_CAPACITY and clears the state. */
+sx_status sx_last_error(sx_ctx* ctx, void* cuda_stream);
+
+/* Number of kernel launches the library has issued on this context so far. */
+uint64_t sx_launch_count(const sx_ctx* ctx);
+
+/* Static text for a status code (for SX_E_CUDA: the last CUDA error string seen by this thread). */
+const char* sx_strerror(sx_status status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* STROKE_EXPAND_H */
