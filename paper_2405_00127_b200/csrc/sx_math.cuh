@@ -1,0 +1,240 @@
+// sx_math.cuh -- device functions of the stroke-expansion kernels (sm_100a).
+//
+// The curve mathematics of "GPU-friendly Stroke Expansion" (PAPER.md sections 2, 4-7, App. A) as used
+// by the count kernel (b) and the write kernel (d).  Citations are PAPER.md line numbers; "R-n" are
+// the readings listed in DESIGN.md section 3.
+//
+// Arithmetic discipline: this translation unit is compiled with -fmad=false, so
+// every a*b+c written with plain operators is two IEEE roundings and every fused multiply-add is an
+// explicit fmaf().  Everything that decides an integer (accept/split of Alg. 2, the Euler-spiral
+// parameters, subdivision counts, subdivision parameters t_i) uses plain operators in a fixed order,
+// identical in the count and the write kernel, so the two passes agree bit for bit.  Vertex
+// coordinates are evaluated in segment-local coordinates with explicit fmaf and the segment base
+// point is added last (fp32 ulp at 16384 px is 9.8e-4 px).
+#pragma once
+#include <stdint.h>
+#include <math.h>
+#include <string.h>
+
+#ifndef SX_DEV
+#define SX_DEV __device__ __forceinline__
+#endif
+
+namespace sx {
+
+// ---------------------------------------------------------------- constants (R-13)
+constexpr float kEpsQ2 = 1e-12f;             // (1e-6 px)^2: "near zero" derivative, L251
+constexpr float kDeltaT = 1e-4f;             // parameter perturbation relative to dt, L251
+constexpr float kDtMin = 1.0f / 65536.0f;    // deepest level of Alg. 2 (paper silent)
+constexpr float kNMax = 65535.0f;            // clamp of a single subdivision count
+constexpr float kC1 = 1.0976991822760038f;   // L155
+constexpr float kC2 = 0.9148117935952064f;
+constexpr float kC3 = 0.16145779359520596f;
+constexpr float kPi = 3.14159265358979323846f;
+constexpr float kQuarterPi = 0.78539816339744830962f;
+constexpr float kSqrt8Over3 = 0.94280904158206336587f;  // sqrt(8)/3, L149
+constexpr float kKnot0 = 0.70107076f;        // f_approx(0.8), f_approx(1.25), f_approx(2.1)
+constexpr float kKnot1 = 0.90324929f;
+constexpr float kKnot2 = 2.03885779f;
+
+enum : uint32_t { kOffset = 0, kOffsetRev = 1, kEvolute = 2, kConnector = 3, kJoinOuter = 4, kJoinInner = 5, kCap = 6, kPlus = 8 };
+enum : int { kJoinMiter = 0, kJoinRound = 1, kJoinBevel = 2, kCapButt = 0, kCapSquare = 1, kCapRound = 2, kModeLine = 0, kModeArc = 1 };
+
+// ---------------------------------------------------------------- float2 helpers (plain operators: no contraction)
+struct V2 { float x, y; };
+SX_DEV V2 v2(float x, float y) { V2 r; r.x = x; r.y = y; return r; }
+SX_DEV V2 operator-(V2 a, V2 b) { return v2(a.x - b.x, a.y - b.y); }
+SX_DEV float dot(V2 a, V2 b) { return a.x * b.x + a.y * b.y; }
+SX_DEV float cross(V2 a, V2 b) { return a.x * b.y - a.y * b.x; }
+SX_DEV float len2(V2 a) { return a.x * a.x + a.y * a.y; }
+SX_DEV V2 unit(V2 a) { float l = sqrtf(len2(a)); return v2(a.x / l, a.y / l); }
+
+#ifdef __CUDA_ARCH__
+SX_DEV float u2f(uint32_t u) { return __uint_as_float(u); }
+#else
+SX_DEV float u2f(uint32_t u) { float f; memcpy(&f, &u, 4); return f; }
+#endif
+
+SX_DEV int ctz32(uint32_t x) {
+#ifdef __CUDA_ARCH__
+    return __ffs((int)x) - 1;
+#else
+    return __builtin_ctz(x);
+#endif
+}
+
+// ---------------------------------------------------------------- per-call parameters (kernel argument, by value)
+struct Params {
+    const uint8_t* tags;
+    const float* pts;        // xy interleaved
+    const uint8_t* styles;   // sx_style[], 16 B each
+    const uint32_t* pt_off;  // from the tag scan
+    const uint32_t* path_idx;
+    const uint32_t* sp_first;
+    float A[6];              // affine (L462)
+    float scale;             // sqrt|det A| (R-14)
+    float tol_es, tol_fl;    // 0.1 / 0.8 of the tolerance (R-13)
+    int mode;
+    uint32_t n_tags;
+};
+
+// ---------------------------------------------------------------- segment in device space, local to P0
+struct Seg {
+    int kind;         // 1 line, 2 quad, 3 cubic
+    V2 P0, P3;        // global end points
+    V2 c1, c2, c3;    // control points relative to P0, after degree elevation (L349)
+    V2 ts, te;        // unit start / end tangents
+    bool degenerate;  // all control points coincide
+};
+
+// transform (R-14): x' = fma(a,x,fma(c,y,e)), y' = fma(b,x,fma(d,y,f))
+SX_DEV V2 xform(const float* A, float x, float y) {
+    return v2(fmaf(A[0], x, fmaf(A[2], y, A[4])), fmaf(A[1], x, fmaf(A[3], y, A[5])));
+}
+
+// first control-polygon leg that is not (near) zero, else (1,0) (R-5): the limit tangent of the curve
+SX_DEV V2 pick_tangent(V2 a, V2 b, V2 c, bool* degenerate) {
+    *degenerate = false;
+    if (len2(a) >= kEpsQ2) return unit(a);
+    if (len2(b) >= kEpsQ2) return unit(b);
+    if (len2(c) >= kEpsQ2) return unit(c);
+    *degenerate = true;
+    return v2(1.0f, 0.0f);
+}
+
+#ifdef __CUDA_ARCH__
+SX_DEV float2 ldg2(const float* p) { return __ldg(reinterpret_cast<const float2*>(p)); }
+#else
+SX_DEV V2 ldg2(const float* p) { return v2(p[0], p[1]); }
+#endif
+
+SX_DEV Seg load_segment(const Params& P, uint32_t i, uint32_t tag) {
+    Seg s;
+    int cnt = tag & 3;
+    const float* p = P.pts + 2 * (uint64_t)P.pt_off[i];
+    auto a0 = ldg2(p), a1 = ldg2(p + 2);
+    V2 q0 = xform(P.A, a0.x, a0.y), q1 = xform(P.A, a1.x, a1.y);
+    s.kind = cnt;
+    s.P0 = q0;
+    bool dg, dg2;
+    if (cnt == 1) {
+        s.P3 = q1;
+        V2 d = q1 - q0;
+        s.c3 = d;
+        s.c1 = v2(d.x / 3.0f, d.y / 3.0f);
+        s.c2 = v2(d.x * (2.0f / 3.0f), d.y * (2.0f / 3.0f));
+        s.ts = s.te = pick_tangent(d, d, d, &dg);
+    } else if (cnt == 2) {
+        auto a2 = ldg2(p + 4);
+        V2 q2 = xform(P.A, a2.x, a2.y);
+        s.P3 = q2;
+        V2 a = q1 - q0, b = q2 - q0;
+        s.c1 = v2(a.x * (2.0f / 3.0f), a.y * (2.0f / 3.0f));
+        s.c2 = v2(b.x + (a.x - b.x) * (2.0f / 3.0f), b.y + (a.y - b.y) * (2.0f / 3.0f));
+        s.c3 = b;
+        s.ts = pick_tangent(a, b, b, &dg);
+        s.te = pick_tangent(b - a, b, b, &dg2);
+    } else {
+        auto a2 = ldg2(p + 4), a3 = ldg2(p + 6);
+        V2 q2 = xform(P.A, a2.x, a2.y), q3 = xform(P.A, a3.x, a3.y);
+        s.P3 = q3;
+        s.c1 = q1 - q0;
+        s.c2 = q2 - q0;
+        s.c3 = q3 - q0;
+        s.ts = pick_tangent(s.c1, s.c2, s.c3, &dg);
+        s.te = pick_tangent(s.c3 - s.c2, s.c3 - s.c1, s.c3, &dg2);
+    }
+    s.degenerate = dg;
+    return s;
+}
+
+// start point and start tangent only (join partner / start cap owner)
+SX_DEV void load_segment_start(const Params& P, uint32_t j, V2* P0, V2* ts) {
+    Seg s = load_segment(P, j, P.tags[j]);
+    *P0 = s.P0;
+    *ts = s.ts;
+}
+
+// ---------------------------------------------------------------- cubic evaluation (Alg. 2), Bernstein form
+SX_DEV V2 cubic_pos(const Seg& s, float t) {
+    float mt = 1.0f - t;
+    float a = 3.0f * mt * mt * t, b = 3.0f * mt * t * t, c = t * t * t;
+    return v2(a * s.c1.x + b * s.c2.x + c * s.c3.x, a * s.c1.y + b * s.c2.y + c * s.c3.y);
+}
+SX_DEV V2 cubic_q(const Seg& s, float t) {  // C'(t)/3
+    float mt = 1.0f - t;
+    float a = mt * mt, b = 2.0f * mt * t, c = t * t;
+    V2 d0 = s.c1, d1 = s.c2 - s.c1, d2 = s.c3 - s.c2;
+    return v2(a * d0.x + b * d1.x + c * d2.x, a * d0.y + b * d1.y + c * d2.y);
+}
+// position, |q| and unit tangent at t with the near-zero-derivative rule of L251 (R-5)
+SX_DEV void eval_cubic(const Seg& s, float t, float dt, V2* pos, float* qmag, V2* u) {
+    V2 q = cubic_q(s, t);
+    float q2 = len2(q);
+    *qmag = sqrtf(q2);
+    if (t == 1.0f) { *pos = s.c3; *u = s.te; return; }
+    *pos = cubic_pos(s, t);
+    if (q2 >= kEpsQ2) { *u = v2(q.x / *qmag, q.y / *qmag); return; }
+    V2 qp = cubic_q(s, t - kDeltaT * dt);
+    *u = (len2(qp) > 0.0f) ? unit(qp) : v2(1.0f, 0.0f);
+}
+
+// ---------------------------------------------------------------- section 7.1: cubic -> Euler spiral error estimate
+// L215 unit-chord normalisation; L217 d-bar; L221 e1; L225 area; L227 e2; L229 e3; guards R-4.
+SX_DEV float fit_error(V2 u0, V2 u1, float q0mag, float q1mag, V2 ch, float dt, float* th0_out, float* th1_out, float* chord_out) {
+    float chord2 = len2(ch);
+    float chord = sqrtf(chord2);
+    *chord_out = chord;
+    if (chord2 < kEpsQ2) { *th0_out = 0.0f; *th1_out = 0.0f; return INFINITY; }
+    V2 uc = v2(ch.x / chord, ch.y / chord);
+    float s0 = cross(u0, uc), c0 = dot(u0, uc);
+    float s1 = cross(uc, u1), c1 = dot(uc, u1);
+    float th0 = atan2f(s0, c0), th1 = atan2f(s1, c1);
+    *th0_out = th0;
+    *th1_out = th1;
+    if (c0 < -0.5f || c1 < -0.5f) return 2.0f * chord;
+    float d0 = q0mag * dt / chord, d1 = q1mag * dt / chord;
+    float db0 = 2.0f / (3.0f * (1.0f + c0)), db1 = 2.0f / (3.0f * (1.0f + c1));
+    float s01 = s0 * c1 + c0 * s1;
+    float area = 0.15f * (2.0f * d0 * s0 + 2.0f * d1 * s1 - d0 * d1 * s01);
+    float areb = 0.15f * (2.0f * db0 * s0 + 2.0f * db1 * s1 - db0 * db1 * s01);
+    float ksum = fabsf(th0 + th1), kdif = fabsf(th0 - th1);
+    float k2 = ksum * ksum;
+    float e1 = 4.6255e-6f * k2 * k2 * ksum + 7.5e-3f * k2 * kdif;
+    float e2 = 1.55f * fabsf(area - areb);
+    float dd0 = db0 - d0, dd1 = db1 - d1;
+    float e3 = (0.005f * ksum + 0.07f * kdif) * sqrtf(dd0 * dd0 + dd1 * dd1);
+    return chord * (e1 + e2 + e3);
+}
+
+// ---------------------------------------------------------------- Appendix A: geometric Hermite interpolation
+// k = th0+th1, D = th1-th0 (L634); k1 (L636) and chord/arc ratio c (L641-651), terms in the paper's order.
+SX_DEV void ghi(float th0, float th1, float* k1_out, float* c_out) {
+    float k = th0 + th1, D = th1 - th0;
+    float k2 = k * k, k4 = k2 * k2, k6 = k4 * k2;
+    float D2 = D * D, D3 = D2 * D, D4 = D2 * D2, D5 = D4 * D, D6 = D4 * D2, D7 = D6 * D;
+    float k1 = 6.0f * D;
+    k1 -= D3 / 70.0f;
+    k1 -= D5 / 10780.0f;
+    k1 += D7 * 2.769178184818219e-7f;
+    k1 -= k2 * D / 10.0f;
+    k1 += k2 * D3 / 4200.0f;
+    k1 += k2 * D5 * 1.6959677820260655e-5f;
+    k1 -= k4 * D / 1400.0f;
+    k1 += k4 * D3 * 6.84915970574303e-5f;
+    k1 -= k6 * D * 7.936475029053326e-6f;
+    float c = 1.0f;
+    c -= D2 / 40.0f;
+    c += D4 * 0.00034226190482569864f;
+    c -= D6 * 1.9349474568904524e-6f;
+    c -= k2 / 24.0f;
+    c += k2 * D2 * 0.0024702380951963226f;
+    c -= k2 * D4 * 3.7297408997537985e-5f;
+    c += k4 / 1920.0f;
+    c -= k4 * D2 * 4.87350869747975e-5f;
+    c -= k6 * 3.1001936068463107e-6f;
+    *k1_out = k1;
+    *c_out = c;
+}
+
+}  // namespace sx

@@ -1,0 +1,273 @@
+// sx_segment.cuh -- one input segment end to end (Alg. 1 L306-343 per thread, Alg. 2 L351-438 inside).
+//
+// process_segment<EMIT=false> returns the number of records the segment produces (count kernel);
+// process_segment<EMIT=true> writes them in the canonical order (write kernel).  Both instantiate the
+// same plan functions, so the counts agree by construction.
+#pragma once
+#include "sx_piece.cuh"
+
+namespace sx {
+
+// ---------------------------------------------------------------- record sink
+struct Writer {
+    float4* out;     // sx_line[] (1 float4 per record) or sx_arc[] (2 float4 per record)
+    uint64_t base;   // index of the segment's first record
+    uint32_t seg;
+    int mode;
+    SX_DEV void put(uint32_t idx, V2 a, V2 b, float angle, uint32_t kind) const {
+        uint64_t r = base + idx;
+        if (mode == kModeLine) {
+            out[r] = make_float4(a.x, a.y, b.x, b.y);
+        } else {
+            out[2 * r] = make_float4(a.x, a.y, b.x, b.y);
+            out[2 * r + 1] = make_float4(angle, u2f(seg), u2f(kind), 0.0f);
+        }
+    }
+};
+
+// one side's record in forward-t order; the +h side is the mirror image of its forward list (reverse
+// order, end points swapped, angle negated)
+struct SideSink {
+    const Writer* w;
+    uint32_t first;  // index (within the segment) of the side's first record
+    uint32_t total;
+    bool mirror;
+    SX_DEV void put(uint32_t idx, V2 a, V2 b, float angle, uint32_t kind) const {
+        if (mirror) w->put(first + (total - 1u - idx), b, a, -angle, kind | kPlus);
+        else w->put(first + idx, a, b, angle, kind);
+    }
+};
+
+// ---------------------------------------------------------------- one side of one piece
+template <bool EMIT>
+SX_DEV uint32_t piece_side(Piece& p, float eta, bool mirror, const Params& P, const Writer* w, uint32_t first) {
+    SidePlan s = side_plan(p, eta, P.mode, P.tol_fl);
+    if (!EMIT) return (uint32_t)s.total;
+    SideSink k;
+    k.w = w; k.first = first; k.total = (uint32_t)s.total; k.mirror = mirror;
+    const bool arc = P.mode == kModeArc;
+    uint32_t idx = 0;
+    for (int r = 0; r < s.nr; r++) {
+        const OffPlan o = r == 0 ? s.off[0] : s.off[1];
+        const bool sup = r == 0 ? s.sup[0] : s.sup[1];
+        if (!sup) {
+            V2 prev = es_offset(p, o.ta, eta);
+            float tp = o.ta;
+            for (int i = 1; i <= o.n; i++) {
+                float t = i < o.n ? offset_t(p, o, eta, i) : o.tb;
+                V2 cur = es_offset(p, t, eta);
+                k.put(idx++, prev, cur, arc ? es_dphi(p, tp, t) : 0.0f, kOffset);
+                prev = cur; tp = t;
+            }
+        } else {
+            // evolute patch (section 6): the evolute meets the offset curve at the cusp
+            V2 Oa = es_offset(p, o.ta, eta), Ob = es_offset(p, o.tb, eta);
+            V2 Ea = s.cusp_a ? Oa : es_evolute(p, o.ta), Eb = s.cusp_b ? Ob : es_evolute(p, o.tb);
+            if (!s.cusp_a) { k.put(idx, Oa, Ea, 0.0f, kConnector); k.put(idx + 1, Oa, Ea, 0.0f, kConnector); idx += 2; }  // "output twice", L197
+            const int ne = s.evo.n;
+            V2 pe = Ea;
+            for (int i = 0; i < ne; i++) {
+                V2 b = (i == ne - 1) ? Eb : es_evolute(p, evolute_t(p, s.evo, i + 1));
+                k.put(idx + i, pe, b, 0.0f, kEvolute);
+                k.put(idx + ne + i, pe, b, 0.0f, kEvolute);
+                pe = b;
+            }
+            idx += 2 * ne;
+            V2 prev = Ob;  // reversed offset (L403, L191)
+            float tp = o.tb;
+            for (int i = o.n - 1; i >= 0; i--) {
+                float t = i > 0 ? offset_t(p, o, eta, i) : o.ta;
+                V2 cur = i > 0 ? es_offset(p, t, eta) : Oa;
+                k.put(idx++, prev, cur, arc ? es_dphi(p, tp, t) : 0.0f, kOffsetRev);
+                prev = cur; tp = t;
+            }
+            if (!s.cusp_b) { k.put(idx, Eb, Ob, 0.0f, kConnector); k.put(idx + 1, Eb, Ob, 0.0f, kConnector); idx += 2; }
+        }
+    }
+    return (uint32_t)s.total;
+}
+
+// ---------------------------------------------------------------- round joins / caps (L65-69 exact arc metric; R-10)
+SX_DEV int round_count(float phi, float h, int mode, float tol_fl) {
+    if (mode == kModeArc) return (phi <= 0.5f * kPi) ? 1 : 2;
+    float n_f = 1.0f;
+    if (tol_fl < h) n_f = ceilf(phi / (2.0f * acosf(1.0f - tol_fl / h)));
+    return count_clamp(n_f);
+}
+// centre V, from A = V + r sweeping CCW by phi to B, n records
+SX_DEV void emit_round(const Writer* w, uint32_t first, int n, V2 V, V2 r, V2 A, V2 B, float phi, uint32_t kind, bool arc) {
+    V2 prev = A;
+    float ang = arc ? phi / (float)n : 0.0f;
+    for (int i = 1; i <= n; i++) {
+        V2 cur = B;
+        if (i < n) {
+            float a = phi * (float)i / (float)n, sa, ca;
+            sincosf(a, &sa, &ca);
+            cur.x = V.x + fmaf(ca, r.x, -sa * r.y);
+            cur.y = V.y + fmaf(sa, r.x, ca * r.y);
+        }
+        w->put(first + (uint32_t)(i - 1), prev, cur, ang, kind);
+        prev = cur;
+    }
+}
+
+struct Style { float width, miter_limit; int join, cap; };
+
+// join between this segment (end point V, end tangent T0) and its partner (start point W, start
+// tangent T1) -- R-10.  -h side runs forward A->B, +h side backward B'->A'.
+template <bool EMIT>
+SX_DEV uint32_t emit_join(const Params& P, const Style& st, V2 V, V2 T0, V2 W, V2 T1, float h, const Writer* w, uint32_t first) {
+    float cr = cross(T0, T1), dt = dot(T0, T1);
+    bool outer_minus = (cr > 0.0f) || (cr == 0.0f && dt < 0.0f);
+    float phi = fabsf(atan2f(cr, dt));
+    float opd = 1.0f + dt;
+    bool miter_ok = (opd > 1e-6f) && (2.0f / opd <= st.miter_limit * st.miter_limit);
+    const bool arc = P.mode == kModeArc;
+    uint32_t idx = 0;
+#pragma unroll
+    for (int side = 0; side < 2; side++) {
+        bool outer = side == 0 ? outer_minus : !outer_minus;
+        uint32_t sb = side == 0 ? 0u : (uint32_t)kPlus;
+        V2 s0, s1;
+        if (EMIT) {
+            s0 = side == 0 ? offset_point(V, T0, -h) : offset_point(W, T1, h);
+            s1 = side == 0 ? offset_point(W, T1, -h) : offset_point(V, T0, h);
+        }
+        if (!outer) {  // inner join: through the vertex (strong correctness, L35)
+            if (EMIT) { w->put(first + idx, s0, V, 0.0f, kJoinInner | sb); w->put(first + idx + 1, V, s1, 0.0f, kJoinInner | sb); }
+            idx += 2;
+        } else if (st.join == kJoinRound) {
+            int n = round_count(phi, h, P.mode, P.tol_fl);
+            if (EMIT) {
+                V2 r = side == 0 ? v2(h * T0.y, -h * T0.x) : v2(fmaf(h, -T1.y, W.x - V.x), fmaf(h, T1.x, W.y - V.y));
+                emit_round(w, first + idx, n, V, r, s0, s1, phi, kJoinOuter | sb, arc);
+            }
+            idx += (uint32_t)n;
+        } else if (st.join == kJoinMiter && miter_ok) {
+            if (EMIT) {
+                float k = (side == 0 ? -h : h) / opd;  // tip = V -/+ h (N0+N1)/(1+dt)
+                V2 tip = v2(fmaf(k, -T0.y - T1.y, V.x), fmaf(k, T0.x + T1.x, V.y));
+                w->put(first + idx, s0, tip, 0.0f, kJoinOuter | sb);
+                w->put(first + idx + 1, tip, s1, 0.0f, kJoinOuter | sb);
+            }
+            idx += 2;
+        } else {
+            if (EMIT) w->put(first + idx, s0, s1, 0.0f, kJoinOuter | sb);
+            idx += 1;
+        }
+    }
+    return idx;
+}
+
+// cap at vertex V with outward direction T: from V - hN(T) counter-clockwise to V + hN(T) (R-11)
+template <bool EMIT>
+SX_DEV uint32_t emit_cap(const Params& P, const Style& st, V2 V, V2 T, float h, const Writer* w, uint32_t first) {
+    if (st.cap == kCapRound) {
+        int n = round_count(kPi, h, P.mode, P.tol_fl);
+        if (EMIT) emit_round(w, first, n, V, v2(h * T.y, -h * T.x), offset_point(V, T, -h), offset_point(V, T, h), kPi, kCap, P.mode == kModeArc);
+        return (uint32_t)n;
+    }
+    if (st.cap == kCapSquare) {
+        if (EMIT) {
+            V2 from = offset_point(V, T, -h), to = offset_point(V, T, h);
+            V2 c1 = v2(fmaf(h, T.y + T.x, V.x), fmaf(h, T.y - T.x, V.y));
+            V2 c2 = v2(fmaf(h, T.x - T.y, V.x), fmaf(h, T.x + T.y, V.y));
+            w->put(first, from, c1, 0.0f, kCap);
+            w->put(first + 1, c1, c2, 0.0f, kCap);
+            w->put(first + 2, c2, to, 0.0f, kCap);
+        }
+        return 3;
+    }
+    if (EMIT) w->put(first, offset_point(V, T, -h), offset_point(V, T, h), 0.0f, kCap);
+    return 1;
+}
+
+// ---------------------------------------------------------------- Alg. 2: cubic -> Euler spirals -> records
+// Iterative bisection with the two-word stack (t0_u, dt), pop by count-trailing-zeros (L444).  One pass
+// serves both sides: the fit does not depend on the offset.
+template <bool EMIT>
+SX_DEV uint32_t flatten_cubic(const Params& P, const Seg& s, float h, const Writer* w) {
+    uint32_t t0_u = 0, n = 0;
+    float dt = 1.0f;
+    V2 last_p = v2(0.0f, 0.0f), last_u = s.ts;
+    float last_qmag = sqrtf(len2(s.c1));
+    for (;;) {
+        float t0 = (float)t0_u * dt;
+        if (t0 == 1.0f) break;
+        float t1 = t0 + dt;
+        V2 next_p, next_u;
+        float next_qmag, th0, th1, chord;
+        eval_cubic(s, t1, dt, &next_p, &next_qmag, &next_u);
+        V2 ch = next_p - last_p;
+        float err = fit_error(last_u, next_u, last_qmag, next_qmag, ch, dt, &th0, &th1, &chord);
+        if (err <= P.tol_es || dt <= kDtMin) {
+            Piece p;
+            p.base = s.P0; p.P3 = s.P3;
+            p.la = last_p; p.lb = next_p;
+            p.ua = last_u; p.ub = next_u;
+            p.ch = ch;
+            p.at0 = (t0 == 0.0f); p.at1 = (t1 == 1.0f);
+            piece_params(p, th0, th1, chord);
+            uint32_t nm = piece_side<EMIT>(p, -h, false, P, w, n);  // -h side, forward
+            n += nm;
+            uint32_t np = piece_side<EMIT>(p, h, true, P, w, n);    // +h side, mirrored
+            n += np;
+            t0_u += 1;
+            int shift = ctz32(t0_u);
+            t0_u >>= shift;
+            dt *= (float)(1u << shift);
+            last_p = next_p; last_u = next_u; last_qmag = next_qmag;
+        } else {
+            t0_u *= 2;
+            dt *= 0.5f;
+        }
+    }
+    return n;
+}
+
+// ---------------------------------------------------------------- Alg. 1: the whole segment
+template <bool EMIT>
+SX_DEV uint32_t process_segment(const Params& P, uint32_t i, Writer* w) {
+    uint32_t tag = P.tags[i];
+    uint32_t path = P.path_idx[i];
+#ifdef __CUDA_ARCH__
+    uint4 raw = __ldg(reinterpret_cast<const uint4*>(P.styles) + path);
+#else
+    uint4 raw = reinterpret_cast<const uint4*>(P.styles)[path];
+#endif
+    Style st;
+    st.width = u2f(raw.x);
+    st.miter_limit = u2f(raw.y);
+    st.join = (int)(raw.z & 0xffu);
+    st.cap = (int)((raw.z >> 8) & 0xffu);
+    float h = 0.5f * st.width * P.scale;
+    if (!(h > 0.0f && h < INFINITY)) return 0;  // width <= 0 or non-finite: the path emits nothing
+    Seg s = load_segment(P, i, tag);
+    uint32_t n;
+    if (s.kind == 1 || s.degenerate) {
+        // straight fast path (R-1b): the two offset lines are exact
+        if (EMIT) {
+            w->put(0, offset_point(s.P0, s.ts, -h), offset_point(s.P3, s.te, -h), 0.0f, kOffset);
+            w->put(1, offset_point(s.P3, s.te, h), offset_point(s.P0, s.ts, h), 0.0f, kOffset | kPlus);
+        }
+        n = 2;
+    } else {
+        n = flatten_cubic<EMIT>(P, s, h, w);
+    }
+    bool sp_end = ((tag >> 2) | (tag >> 4)) & 1u;
+    bool closed = (tag >> 7) & 1u;
+    if (!sp_end || closed) {
+        uint32_t j = sp_end ? P.sp_first[i] : i + 1;
+        V2 W, T1;
+        load_segment_start(P, j, &W, &T1);
+        n += emit_join<EMIT>(P, st, s.P3, s.te, W, T1, h, w, n);
+    } else {
+        V2 F, Tf;
+        load_segment_start(P, P.sp_first[i], &F, &Tf);
+        n += emit_cap<EMIT>(P, st, s.P3, s.te, h, w, n);
+        n += emit_cap<EMIT>(P, st, F, v2(-Tf.x, -Tf.y), h, w, n);
+    }
+    return n;
+}
+
+}  // namespace sx
