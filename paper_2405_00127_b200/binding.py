@@ -1,0 +1,220 @@
+"""Thin Python binding of include/stroke_expand.h: same names, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libstroke_expand.so; torch is used for device memory
+and streams.  There is no CPU fallback: loading fails loudly when the library has not been built
+(`python -m paper_2405_00127_b200.build`), and sx_create fails when there is no CUDA device.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+SO_PATH = os.path.join(_HERE, "libstroke_expand.so")
+
+SX_OK, SX_E_INVALID_ARG, SX_E_BAD_STREAM, SX_E_CAPACITY, SX_E_CUDA, SX_E_STATE = 0, -1, -2, -3, -4, -5
+SX_MODE_LINE, SX_MODE_ARC = 0, 1
+RECORD_BYTES = {SX_MODE_LINE: 16, SX_MODE_ARC: 32}
+ARC_DTYPE = np.dtype([("x0", "<f4"), ("y0", "<f4"), ("x1", "<f4"), ("y1", "<f4"), ("angle", "<f4"), ("seg", "<u4"),
+                      ("kind", "<u4"), ("pad", "<u4")])
+
+EXPORTS = ["sx_create", "sx_destroy", "sx_count", "sx_write", "stroke_expand", "stroke_expand_host", "sx_segment_info",
+           "sx_last_error", "sx_launch_count", "sx_strerror"]
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
+_lib = None
+
+
+class StrokeExpandError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        super().__init__(f"{where}: {sx_strerror(status)} (status {status})")
+
+
+def lib():
+    """Load the C-ABI library (built in-tree by paper_2405_00127_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(SO_PATH):
+            raise ImportError(f"{SO_PATH} is missing: build it with `python -m paper_2405_00127_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(SO_PATH)
+        vp, u64, i32, f32 = C.c_void_p, C.c_uint64, C.c_int32, C.c_float
+        stream_args = [vp, u64, vp, u64, vp, u64, vp, f32, i32]  # tags, n, points, n, styles, n, affine, tol, mode
+        L.sx_create.argtypes = [C.POINTER(vp), i32]
+        L.sx_destroy.argtypes = [vp]
+        L.sx_count.argtypes = [vp] + stream_args + [vp, C.POINTER(u64), vp]
+        L.sx_write.argtypes = [vp, vp, u64, vp]
+        L.stroke_expand.argtypes = [vp] + stream_args + [ALLOC_FN, vp, C.POINTER(vp), C.POINTER(u64), vp, vp]
+        L.stroke_expand_host.argtypes = [vp] + stream_args + [vp, u64, C.POINTER(u64), vp, vp]
+        L.sx_segment_info.argtypes = [vp] + [C.POINTER(vp)] * 5
+        L.sx_last_error.argtypes = [vp, vp]
+        L.sx_launch_count.argtypes = [vp]
+        L.sx_launch_count.restype = u64
+        L.sx_strerror.argtypes = [i32]
+        L.sx_strerror.restype = C.c_char_p
+        for name in EXPORTS:
+            if name not in ("sx_launch_count", "sx_strerror"):
+                getattr(L, name).restype = i32
+        _lib = L
+    return _lib
+
+
+def sx_strerror(status):
+    return lib().sx_strerror(int(status)).decode()
+
+
+def _check(status, where):
+    if status != SX_OK:
+        raise StrokeExpandError(status, where)
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def _affine(affine):
+    a = np.ascontiguousarray(np.asarray(affine, dtype=np.float32).reshape(6))
+    return a, C.c_void_p(a.ctypes.data)
+
+
+def _dev_streams(tags, points, styles):
+    """tags u8[N], points f32[Npts,2], styles u8[P,16] (or any 16-byte rows) as contiguous CUDA tensors."""
+    assert tags.is_cuda and points.is_cuda and styles.is_cuda, "device tensors expected (use stroke_expand_host for host data)"
+    assert tags.dtype == torch.uint8 and points.dtype == torch.float32 and styles.dtype == torch.uint8
+    assert tags.is_contiguous() and points.is_contiguous() and styles.is_contiguous()
+    n_paths = styles.numel() // 16
+    return (C.c_void_p(tags.data_ptr()), tags.numel(), C.c_void_p(points.data_ptr()), points.numel() // 2,
+            C.c_void_p(styles.data_ptr()), n_paths)
+
+
+def sx_create(device=0):
+    h = C.c_void_p()
+    _check(lib().sx_create(C.byref(h), int(device)), "sx_create")
+    return h
+
+
+def sx_destroy(ctx):
+    _check(lib().sx_destroy(ctx), "sx_destroy")
+
+
+def sx_count(ctx, tags, points, styles, affine, tolerance, mode, path_offsets, want_total=True, stream=None):
+    """Phase 1.  path_offsets: int64/uint64 CUDA tensor [n_paths+1], written.  Returns the record count (or None
+    when want_total is False: the call then stays asynchronous)."""
+    args = _dev_streams(tags, points, styles)
+    a, ap = _affine(affine)
+    assert path_offsets.is_cuda and path_offsets.element_size() == 8 and path_offsets.numel() >= args[5] + 1
+    total = C.c_uint64(0)
+    st = lib().sx_count(ctx, *args, ap, float(tolerance), int(mode), C.c_void_p(path_offsets.data_ptr()),
+                        C.byref(total) if want_total else None, _stream_ptr(stream))
+    _check(st, "sx_count")
+    return int(total.value) if want_total else None
+
+
+def sx_write(ctx, out_records, cap_records, stream=None):
+    """Phase 2.  out_records: CUDA tensor with room for cap_records records (16 B line / 32 B arc)."""
+    assert out_records.is_cuda and out_records.is_contiguous()
+    _check(lib().sx_write(ctx, C.c_void_p(out_records.data_ptr()), int(cap_records), _stream_ptr(stream)), "sx_write")
+
+
+def stroke_expand(ctx, tags, points, styles, affine, tolerance, mode, stream=None):
+    """One shot on device tensors.  Returns (records, path_offsets): records is a float32 CUDA tensor [M,4]
+    (line mode) or [M,8] (arc mode: x0 y0 x1 y1 angle seg kind pad, the last three as raw bits);
+    path_offsets an int64 CUDA tensor [n_paths+1].  The output is allocated by the torch caching allocator
+    through the library's allocation callback."""
+    args = _dev_streams(tags, points, styles)
+    a, ap = _affine(affine)
+    dev = tags.device
+    path_offsets = torch.empty(args[5] + 1, dtype=torch.int64, device=dev)
+    holder = {}
+    width = 4 if mode == SX_MODE_LINE else 8
+
+    def _alloc(nbytes, _user):
+        t = torch.empty((nbytes // (4 * width), width), dtype=torch.float32, device=dev)
+        holder["t"] = t
+        return t.data_ptr()
+
+    cb = ALLOC_FN(_alloc)
+    out_ptr, n_rec = C.c_void_p(), C.c_uint64(0)
+    st = lib().stroke_expand(ctx, *args, ap, float(tolerance), int(mode), cb, None, C.byref(out_ptr), C.byref(n_rec),
+                             C.c_void_p(path_offsets.data_ptr()), _stream_ptr(stream))
+    _check(st, "stroke_expand")
+    rec = holder.get("t")
+    if rec is None:
+        rec = torch.empty((0, width), dtype=torch.float32, device=dev)
+    return rec, path_offsets
+
+
+def stroke_expand_host(ctx, tags, points, styles, affine, tolerance, mode, out_records, path_offsets, stream=None):
+    """One shot on HOST tensors (pin them for asynchronous copies).  out_records: host float32 tensor [cap,4] or
+    [cap,8]; path_offsets: host int64 tensor [n_paths+1].  Returns the record count; raises on SX_E_CAPACITY with
+    the needed count in the exception's .needed."""
+    for t in (tags, points, styles, out_records, path_offsets):
+        assert not t.is_cuda and t.is_contiguous()
+    assert tags.dtype == torch.uint8 and points.dtype == torch.float32 and styles.dtype == torch.uint8
+    a, ap = _affine(affine)
+    width = 4 if mode == SX_MODE_LINE else 8
+    cap = out_records.numel() // width
+    n_paths = styles.numel() // 16
+    assert path_offsets.element_size() == 8 and path_offsets.numel() >= n_paths + 1
+    n_rec = C.c_uint64(0)
+    st = lib().stroke_expand_host(ctx, C.c_void_p(tags.data_ptr()), tags.numel(), C.c_void_p(points.data_ptr()),
+                                  points.numel() // 2, C.c_void_p(styles.data_ptr()), n_paths, ap, float(tolerance), int(mode),
+                                  C.c_void_p(out_records.data_ptr()), cap, C.byref(n_rec), C.c_void_p(path_offsets.data_ptr()),
+                                  _stream_ptr(stream))
+    if st == SX_E_CAPACITY:
+        e = StrokeExpandError(st, "stroke_expand_host")
+        e.needed = int(n_rec.value)
+        raise e
+    _check(st, "stroke_expand_host")
+    return int(n_rec.value)
+
+
+def _view(ptr, n, dtype, device):
+    """Zero-copy torch view of ctx scratch memory (valid until the next call on the context)."""
+    if n == 0 or not ptr:
+        return torch.empty(0, dtype=dtype, device=device)
+    nbytes = n * torch.empty(0, dtype=dtype).element_size()
+
+    class _Mem:
+        __cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (int(ptr), True), "version": 3}
+
+    return torch.as_tensor(_Mem(), device=device).view(dtype)
+
+
+def sx_segment_info(ctx, n_tags, device="cuda:0"):
+    """Copies of the last sx_count's per-segment scan results: dict of CUDA tensors pt_off, path_idx, sp_first,
+    seg_count (int32 views of the u32 data) and seg_offset (int64)."""
+    ptrs = [C.c_void_p() for _ in range(5)]
+    _check(lib().sx_segment_info(ctx, *[C.byref(p) for p in ptrs]), "sx_segment_info")
+    names = ["pt_off", "path_idx", "sp_first", "seg_count", "seg_offset"]
+    out = {}
+    for name, p in zip(names, ptrs):
+        dt = torch.int64 if name == "seg_offset" else torch.int32
+        out[name] = _view(p.value, n_tags, dt, device).clone()
+    return out
+
+
+def sx_last_error(ctx, stream=None):
+    return int(lib().sx_last_error(ctx, _stream_ptr(stream)))
+
+
+def sx_launch_count(ctx):
+    return int(lib().sx_launch_count(ctx))
+
+
+def scene_to_torch(scene, device=None, pin=False):
+    """Marshal a scenes.Scene (numpy streams) into the tensors the calls above take."""
+    tags = torch.from_numpy(np.ascontiguousarray(scene["tags"]))
+    points = torch.from_numpy(np.ascontiguousarray(scene["points"], dtype=np.float32))
+    styles = torch.from_numpy(np.ascontiguousarray(scene["styles"]).view(np.uint8).reshape(-1, 16).copy())
+    if device is not None:
+        return tags.to(device), points.to(device), styles.to(device)
+    if pin:
+        return tags.pin_memory(), points.pin_memory(), styles.pin_memory()
+    return tags, points, styles

@@ -1,0 +1,322 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the CPU oracle on the same seeded inputs.
+
+The bar (BASELINE.json north_star): tag-scan results bit-exact; per-segment record counts identical on
+>= 99.9 % of input segments; end-point coordinates within 1e-3 px absolute wherever counts match; and the GPU
+output passes the same watertightness / winding / tolerance checks as the oracle's.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from oracle import checkers as ck
+from paper_2405_00127_b200 import scenes as S
+
+pytestmark = pytest.mark.gpu
+
+COUNT_PARITY = 0.999   # north_star
+COORD_TOL = 1e-3       # px, north_star
+ANGLE_TOL = 2e-5       # rad: fp32 evaluation of an angle of a few radians
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2405_00127_b200 import binding
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return binding
+
+
+@pytest.fixture(scope="module")
+def ctx(B):
+    c = B.sx_create(0)
+    yield c
+    B.sx_destroy(c)
+
+
+class GpuResult:
+    pass
+
+
+def gpu_run(B, ctx, sc, mode, host=False):
+    dev = "cuda:0"
+    if host:
+        tags, pts, sty = B.scene_to_torch(sc, pin=True)
+        cap = 1 << 16
+        while True:
+            out = torch.empty((cap, 4 if mode == 0 else 8), dtype=torch.float32).pin_memory()
+            poff = torch.empty(sc.n_paths + 1, dtype=torch.int64).pin_memory()
+            try:
+                m = B.stroke_expand_host(ctx, tags, pts, sty, sc.affine, sc.tolerance, mode, out, poff)
+                break
+            except B.StrokeExpandError as e:
+                assert e.status == B.SX_E_CAPACITY
+                cap = e.needed
+        rec = out[:m].numpy().copy()
+        poff = poff.numpy().copy()
+    else:
+        tags, pts, sty = B.scene_to_torch(sc, device=dev)
+        rec_t, poff_t = B.stroke_expand(ctx, tags, pts, sty, sc.affine, sc.tolerance, mode)
+        torch.cuda.synchronize()
+        rec = rec_t.cpu().numpy()
+        poff = poff_t.cpu().numpy()
+    assert B.sx_last_error(ctx) == 0
+    info = B.sx_segment_info(ctx, sc.n_segments)
+    g = GpuResult()
+    g.xy = np.ascontiguousarray(rec[:, :4])
+    if mode == 1:
+        g.angle = np.ascontiguousarray(rec[:, 4])
+        g.seg = np.ascontiguousarray(rec[:, 5]).view(np.uint32)
+        g.kind = np.ascontiguousarray(rec[:, 6]).view(np.uint32).astype(np.uint8)
+    else:
+        g.angle = np.zeros(len(rec), np.float32)
+    g.path_off = poff.astype(np.uint64)
+    g.seg_count = info["seg_count"].cpu().numpy().astype(np.uint32)
+    g.seg_off = info["seg_offset"].cpu().numpy().astype(np.int64)
+    g.pt_off = info["pt_off"].cpu().numpy().astype(np.uint32)
+    g.path_idx = info["path_idx"].cpu().numpy().astype(np.uint32)
+    g.sp_first = info["sp_first"].cpu().numpy().astype(np.uint32)
+    return g
+
+
+def compare(sc, mode, g, r, min_parity=COUNT_PARITY):
+    """Element-by-element comparison; returns the count-parity fraction."""
+    assert np.array_equal(g.pt_off, r.pt_off) and np.array_equal(g.path_idx, r.path_idx) and np.array_equal(g.sp_first, r.sp_first)
+    same = g.seg_count == r.seg_count
+    parity = float(same.mean()) if len(same) else 1.0
+    assert parity >= min_parity, parity
+    assert int(g.seg_count.sum()) == len(g.xy)
+    assert np.array_equal(g.seg_off, np.cumsum(g.seg_count.astype(np.int64)) - g.seg_count)
+    assert np.isfinite(g.xy).all()
+    segs = np.flatnonzero(same)
+    rep = r.seg_count[segs].astype(np.int64)
+    o_off = np.cumsum(r.seg_count.astype(np.int64)) - r.seg_count
+    within = np.arange(rep.sum()) - np.repeat(np.cumsum(rep) - rep, rep)
+    io = np.repeat(o_off[segs], rep) + within
+    ig = np.repeat(g.seg_off[segs], rep) + within
+    d = np.abs(g.xy[ig].astype(np.float64) - r.xy[io].astype(np.float64))
+    assert d.max(initial=0.0) <= COORD_TOL, d.max()
+    if mode == 1:
+        assert np.abs(g.angle[ig] - r.angle[io]).max(initial=0.0) <= ANGLE_TOL
+        assert np.array_equal(g.kind[ig], r.kind[io]) and np.array_equal(g.seg[ig], r.seg[io])
+    if parity == 1.0:
+        assert np.array_equal(g.path_off, r.path_off)
+    return parity
+
+
+def oracle_run(sc, mode):
+    return oracle.expand(sc.tags, sc.points, sc.styles, sc.affine, sc.tolerance, mode)
+
+
+# ---------------------------------------------------------------- element-by-element parity at oracle-sized inputs
+CASES = [("c1", None, 0), ("c2", None, 0), ("c2", None, 1), ("c3", 6000, 0), ("c4", 8000, 1), ("c5", 600, 0), ("c5", 600, 1)]
+
+
+@pytest.mark.parametrize("name,npaths,mode", CASES)
+def test_parity_with_oracle(B, ctx, name, npaths, mode):
+    sc = S.make(name, n_paths=npaths)
+    g = gpu_run(B, ctx, sc, mode)
+    r = oracle_run(sc, mode)
+    compare(sc, mode, g, r)
+    assert ck.watertight_violations(g.xy, g.path_off) == 0
+
+
+@pytest.mark.parametrize("name,npaths,mode", [("c1", 64, 0), ("c2", 300, 1)])
+def test_host_buffer_entry_point_matches_device_entry_point(B, ctx, name, npaths, mode):
+    sc = S.make(name, n_paths=npaths)
+    gd = gpu_run(B, ctx, sc, mode)
+    gh = gpu_run(B, ctx, sc, mode, host=True)
+    assert np.array_equal(gd.xy.view(np.uint32), gh.xy.view(np.uint32)) and np.array_equal(gd.path_off, gh.path_off)
+    assert np.array_equal(gd.angle.view(np.uint32), gh.angle.view(np.uint32))
+
+
+# ---------------------------------------------------------------- the same invariant checks the oracle passes
+@pytest.mark.parametrize("name,npaths,mode", [("c1", 64, 0), ("c2", 240, 0), ("c2", 240, 1), ("c3", 300, 0), ("c4", 200, 1), ("c5", 12, 0), ("c5", 12, 1)])
+def test_gpu_output_passes_the_invariants(B, ctx, name, npaths, mode):
+    from test_oracle_outline import _winding_band
+    sc = S.make(name, n_paths=npaths)
+    g = gpu_run(B, ctx, sc, mode)
+    assert ck.watertight_violations(g.xy, g.path_off) == 0
+    rng = np.random.default_rng(123)
+    paths = rng.choice(npaths, size=min(npaths, 10), replace=False)
+    st = _winding_band(sc, g, paths, rng, mode)
+    assert st["inside"] > 500 and st["outside"] > 500
+    assert st["neg"] == 0 and st["inside_fail"] == 0 and st["outside_fail"] == 0, st
+
+
+def test_gpu_offsets_track_the_true_parallel_curve(B, ctx):
+    """L37: offset vertices within the ES-fit budget of the true parallel curve of the source cubic."""
+    sc = S.make("c1", n_paths=16)
+    g = gpu_run(B, ctx, sc, 1)  # arc mode carries seg / kind per record
+    cubs = ck.segment_cubics(sc.tags, sc.points, sc.affine)
+    halfw = 0.5 * sc.styles["width"][g.path_idx]
+    tame = []
+    for sg in range(sc.n_segments):
+        cb, h = cubs[sg], float(halfw[sg])
+        t = np.linspace(0, 1, 1001)
+        d = ck.cubic_deriv(cb, t)
+        dd = 6 * ((1 - t)[:, None] * (cb[2] - 2 * cb[1] + cb[0]) + t[:, None] * (cb[3] - 2 * cb[2] + cb[1]))
+        kap = (d[:, 0] * dd[:, 1] - d[:, 1] * dd[:, 0]) / np.hypot(d[:, 0], d[:, 1]) ** 3
+        if np.abs(kap).max() * h < 2.0:
+            tame.append(sg)
+    vmax, mmax = ck.check_offsets(cubs, halfw, g.xy, g.kind, g.seg, angle=g.angle, segs=tame[:40])
+    assert vmax < 0.05 and mmax < 1.2 * sc.tolerance
+
+
+# ---------------------------------------------------------------- edge cases
+def test_empty_input(B, ctx):
+    dev = "cuda:0"
+    tags = torch.empty(0, dtype=torch.uint8, device=dev)
+    pts = torch.empty((0, 2), dtype=torch.float32, device=dev)
+    sty = torch.empty((0, 16), dtype=torch.uint8, device=dev)
+    rec, poff = B.stroke_expand(ctx, tags, pts, sty, S.IDENTITY, 0.25, 0)
+    assert rec.shape[0] == 0 and poff.cpu().tolist() == [0]
+
+
+def test_hand_built_rectangle(B, ctx):
+    sc = S.from_paths([dict(start=[10, 20], segs=[[[50, 20]]], width=4.0, cap=S.CAP_BUTT)])
+    g = gpu_run(B, ctx, sc, 0)
+    assert g.xy.tolist() == [[10, 18, 50, 18], [50, 22, 10, 22], [50, 18, 50, 22], [10, 22, 10, 18]]
+
+
+def test_zero_width_and_mixed_subpaths(B, ctx):
+    # path 0: two subpaths (open polyline + closed triangle); path 1: zero width (emits nothing); path 2: single quad
+    tags = np.array([1, 1 | 4, 1, 1, 1 | 4 | 16 | 128, 3 | 4 | 16, 2 | 4 | 16], dtype=np.uint8)
+    pts = np.array([[0, 0], [10, 0], [10, 10],  [20, 20], [30, 20], [25, 30], [20, 20],
+                    [0, 50], [10, 60], [20, 40], [30, 50],  [50, 50], [60, 70], [70, 50]], dtype=np.float32)
+    st = S.make_styles([2.0, 0.0, 3.0], [S.JOIN_MITER, S.JOIN_ROUND, S.JOIN_BEVEL], [S.CAP_SQUARE, S.CAP_ROUND, S.CAP_ROUND], 4.0)
+    sc = S.Scene(name="mixed", tags=tags, points=pts, styles=st, affine=S.IDENTITY.copy(), tolerance=0.25, modes=(0, 1))
+    for mode in (0, 1):
+        g = gpu_run(B, ctx, sc, mode)
+        r = oracle_run(sc, mode)
+        assert compare(sc, mode, g, r, 1.0) == 1.0
+        assert g.seg_count[5] == 0 and g.path_off[1] == g.path_off[2]
+        assert ck.watertight_violations(g.xy, g.path_off) == 0
+
+
+@pytest.mark.parametrize("n", [1, 15, 16, 17, 2047, 2048, 2049, 4095, 4096, 4097, 12289])
+def test_scan_tile_boundaries(B, ctx, n):
+    """Ragged tails and exact multiples of the scan tiles (4096 tags, 2048 counts): polylines of n line segments
+    split into subpaths / paths at irregular places."""
+    rng = np.random.default_rng(n)
+    tags = np.ones(n, dtype=np.uint8)
+    ends = rng.uniform(size=n) < 0.07
+    ends[-1] = True
+    pends = ends & (rng.uniform(size=n) < 0.5)
+    pends[-1] = True
+    tags[ends] |= 4
+    tags[pends] |= 16
+    tags[ends & (rng.uniform(size=n) < 0.5)] |= 128
+    npts = int(n + ends.sum())
+    pts = rng.uniform(0, 1000, (npts, 2)).astype(np.float32)
+    npaths = int(pends.sum())
+    st = S.make_styles(rng.uniform(1, 5, npaths), rng.integers(0, 3, npaths), rng.integers(0, 3, npaths), 4.0)
+    sc = S.Scene(name="tiles", tags=tags, points=pts, styles=st, affine=S.IDENTITY.copy(), tolerance=0.25, modes=(0,))
+    g = gpu_run(B, ctx, sc, 0)
+    r = oracle_run(sc, 0)
+    compare(sc, 0, g, r)
+
+
+@pytest.mark.parametrize("bad", ["zero_count", "bit3", "no_path_end", "pts", "paths"])
+def test_bad_streams_are_rejected(B, ctx, bad):
+    dev = "cuda:0"
+    tags = np.array([1, 3 | 4 | 16], dtype=np.uint8)
+    n_pts, n_paths = 5, 1
+    if bad == "zero_count":
+        tags[0] = 0
+    elif bad == "bit3":
+        tags[0] |= 8
+    elif bad == "no_path_end":
+        tags[1] = 3 | 4
+    elif bad == "pts":
+        n_pts = 6
+    else:
+        n_paths = 2
+    t = torch.from_numpy(tags).to(dev)
+    p = torch.zeros((n_pts, 2), dtype=torch.float32, device=dev)
+    s = torch.from_numpy(S.make_styles([1.0] * n_paths, 0, 0, 4.0).view(np.uint8).reshape(-1, 16).copy()).to(dev)
+    with pytest.raises(B.StrokeExpandError) as e:
+        B.stroke_expand(ctx, t, p, s, S.IDENTITY, 0.25, 0)
+    assert e.value.status == B.SX_E_BAD_STREAM
+    B.sx_last_error(ctx)
+
+
+def test_invalid_arguments_and_capacity(B, ctx):
+    sc = S.make("c1", n_paths=4)
+    tags, pts, sty = B.scene_to_torch(sc, device="cuda:0")
+    poff = torch.empty(sc.n_paths + 1, dtype=torch.int64, device="cuda:0")
+    for kw in (dict(tolerance=0.0), dict(mode=7), dict(affine=[1, 0, 2, 0, 0, 0]), dict(affine=[np.nan, 0, 0, 1, 0, 0])):
+        a = dict(affine=sc.affine, tolerance=0.25, mode=0)
+        a.update(kw)
+        with pytest.raises(B.StrokeExpandError) as e:
+            B.sx_count(ctx, tags, pts, sty, a["affine"], a["tolerance"], a["mode"], poff)
+        assert e.value.status == B.SX_E_INVALID_ARG
+    out = torch.empty((8, 4), dtype=torch.float32, device="cuda:0")
+    with pytest.raises(B.StrokeExpandError) as e:
+        B.sx_write(ctx, out, 8)
+    assert e.value.status == B.SX_E_STATE
+    total = B.sx_count(ctx, tags, pts, sty, sc.affine, 0.25, 0, poff)
+    assert total > 8
+    with pytest.raises(B.StrokeExpandError) as e:
+        B.sx_write(ctx, out, 8)
+    assert e.value.status == B.SX_E_CAPACITY
+    # asynchronous count (no host total): the kernel itself refuses to write past the capacity
+    B.sx_count(ctx, tags, pts, sty, sc.affine, 0.25, 0, poff, want_total=False)
+    guard = torch.full((16, 4), 7.0, dtype=torch.float32, device="cuda:0")
+    B.sx_write(ctx, guard, 8)
+    assert B.sx_last_error(ctx) == B.SX_E_CAPACITY
+    assert (guard[8:] == 7.0).all()
+
+
+# ---------------------------------------------------------------- full-size configs, in the launch configuration bench.py times
+def _sampled_full_size(B, ctx, name, mode, n_sample, seed):
+    sc = S.make(name)
+    dev = "cuda:0"
+    tags, pts, sty = B.scene_to_torch(sc, device=dev)
+    poff = torch.empty(sc.n_paths + 1, dtype=torch.int64, device=dev)
+    total = B.sx_count(ctx, tags, pts, sty, sc.affine, sc.tolerance, mode, poff)
+    width = 4 if mode == 0 else 8
+    out = torch.empty((total, width), dtype=torch.float32, device=dev)
+    B.sx_write(ctx, out, total)
+    torch.cuda.synchronize()
+    assert B.sx_last_error(ctx) == 0
+    info = B.sx_segment_info(ctx, sc.n_segments)
+    poff_h = poff.cpu().numpy()
+    assert poff_h[0] == 0 and poff_h[-1] == total and (np.diff(poff_h) >= 0).all()
+    cnt = info["seg_count"]
+    assert int(cnt.to(torch.int64).sum()) == total
+    rng = np.random.default_rng(seed)
+    paths = np.sort(rng.choice(sc.n_paths, size=n_sample, replace=False))
+    sub, tsel = S.subset_paths(sc, paths)
+    r = oracle_run(sub, mode)
+    g_cnt = cnt[torch.from_numpy(tsel).to(dev)].cpu().numpy().astype(np.uint32)
+    same = g_cnt == r.seg_count
+    assert same.mean() >= COUNT_PARITY
+    # records of the sampled paths, path by path
+    worst = 0.0
+    for k, p in enumerate(paths):
+        a, b = int(poff_h[p]), int(poff_h[p + 1])
+        oa, ob = int(r.path_off[k]), int(r.path_off[k + 1])
+        segs = np.flatnonzero(r.path_idx == k)
+        if not same[segs].all():
+            continue
+        assert b - a == ob - oa
+        got = out[a:b].cpu().numpy()
+        worst = max(worst, float(np.abs(got[:, :4].astype(np.float64) - r.xy[oa:ob].astype(np.float64)).max(initial=0.0)))
+        assert ck.watertight_violations(got[:, :4], np.array([0, b - a])) == 0
+        if mode == 1:
+            assert np.abs(got[:, 4] - r.angle[oa:ob]).max(initial=0.0) <= ANGLE_TOL
+    assert worst <= COORD_TOL, worst
+    del out
+
+
+def test_full_size_c3_sampled(B, ctx):
+    _sampled_full_size(B, ctx, "c3", 0, 400, 7)
+
+
+def test_full_size_c4_sampled(B, ctx):
+    _sampled_full_size(B, ctx, "c4", 1, 400, 8)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_full_size_c5_sampled(B, ctx, mode):
+    _sampled_full_size(B, ctx, "c5", mode, 60, 9 + mode)
