@@ -63,7 +63,7 @@ class ClockSampler(threading.Thread):
                 for k, bit in names.items():
                     if r & bit:
                         self.reasons.add(k)
-                time.sleep(0.02)
+                time.sleep(0.002)
         except Exception as e:  # no NVML: report that, never fake numbers
             self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
 

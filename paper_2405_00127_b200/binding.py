@@ -182,7 +182,7 @@ def _view(ptr, n, dtype, device):
     nbytes = n * torch.empty(0, dtype=dtype).element_size()
 
     class _Mem:
-        __cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (int(ptr), True), "version": 3}
+        __cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (int(ptr), False), "version": 3}
 
     return torch.as_tensor(_Mem(), device=device).view(dtype)
 
