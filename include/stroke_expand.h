@@ -166,6 +166,13 @@ sx_status sx_segment_info(sx_ctx* ctx, const uint32_t** d_pt_off, const uint32_t
  * SX_OK, SX_E_BAD_STREAM or SX_E_CAPACITY and clears the state. */
 sx_status sx_last_error(sx_ctx* ctx, void* cuda_stream);
 
+/* Memory knob for the piece cache: sx_count stores every accepted Euler-spiral piece
+ * (80 bytes) so that sx_write need not repeat the cubic -> spiral fit.  The cache grows on demand; this call
+ * caps it at max_pieces descriptors (0 = no cap, the default).  A call whose pieces do not fit is still
+ * computed correctly, by the slower thread-per-segment writer.  Host-synchronous; invalidates a pending
+ * sx_count. */
+sx_status sx_set_piece_cache_limit(sx_ctx* ctx, uint64_t max_pieces);
+
 /* Number of kernel launches the library has issued on this context so far. */
 uint64_t sx_launch_count(const sx_ctx* ctx);
 

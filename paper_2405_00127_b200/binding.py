@@ -22,7 +22,7 @@ ARC_DTYPE = np.dtype([("x0", "<f4"), ("y0", "<f4"), ("x1", "<f4"), ("y1", "<f4")
                       ("kind", "<u4"), ("pad", "<u4")])
 
 EXPORTS = ["sx_create", "sx_destroy", "sx_count", "sx_write", "stroke_expand", "stroke_expand_host", "sx_segment_info",
-           "sx_last_error", "sx_launch_count", "sx_strerror"]
+           "sx_last_error", "sx_set_piece_cache_limit", "sx_launch_count", "sx_strerror"]
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
 _lib = None
@@ -52,6 +52,7 @@ def lib():
         L.stroke_expand_host.argtypes = [vp] + stream_args + [vp, u64, C.POINTER(u64), vp, vp]
         L.sx_segment_info.argtypes = [vp] + [C.POINTER(vp)] * 5
         L.sx_last_error.argtypes = [vp, vp]
+        L.sx_set_piece_cache_limit.argtypes = [vp, u64]
         L.sx_launch_count.argtypes = [vp]
         L.sx_launch_count.restype = u64
         L.sx_strerror.argtypes = [i32]
@@ -202,6 +203,10 @@ def sx_segment_info(ctx, n_tags, device="cuda:0"):
 
 def sx_last_error(ctx, stream=None):
     return int(lib().sx_last_error(ctx, _stream_ptr(stream)))
+
+
+def sx_set_piece_cache_limit(ctx, max_pieces):
+    _check(lib().sx_set_piece_cache_limit(ctx, int(max_pieces)), "sx_set_piece_cache_limit")
 
 
 def sx_launch_count(ctx):

@@ -10,26 +10,165 @@
 
 #include "../../include/stroke_expand.h"
 #include "sx_scan.cuh"
-#include "sx_segment.cuh"
+#include "sx_cache.cuh"
 
 namespace sx {
 
 constexpr int kSegThreads = 128;
+constexpr int kWpThreads = 256;            // write kernel: threads per block = piece sides per tile
+constexpr int kWpPieces = kWpThreads / 2;  // descriptors per tile
+constexpr int kWpBlocksPerSM = 4;
 
-// (b) count pass: one thread per input segment runs Alg. 2 without the writes
+// (b) count pass.  One thread per input segment runs Alg. 2 without the writes; every accepted piece is
+// stored in the piece cache.  The loop is warp-synchronous at piece granularity: each round every lane
+// advances to its next accepted piece, the warp ballots, and descriptor slots come from a warp-private
+// chunk reserved with one atomic per kChunk slots (unused slots of a chunk are marked invalid).
 __global__ void __launch_bounds__(kSegThreads)
-k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__ err) {
-    uint32_t i = blockIdx.x * (uint32_t)kSegThreads + threadIdx.x;
-    if (i >= P.n_tags) return;
-    uint32_t n = 0;
-    if (*err == 0u) n = process_segment<false>(P, i, nullptr);
-    seg_count[i] = n;
+k_count(Params P, uint32_t* __restrict__ seg_count, float4* __restrict__ pieces, uint32_t piece_cap, uint32_t* piece_ctr,
+        const uint32_t* __restrict__ err) {
+    const uint32_t i = blockIdx.x * (uint32_t)kSegThreads + threadIdx.x;
+    const uint32_t lane = threadIdx.x & 31u;
+    const bool valid = i < P.n_tags && *err == 0u;
+    uint32_t n = 0, n_tail = 0;
+    bool active = false;
+    Seg s;
+    Style st;
+    FitState f;
+    float h = 0.0f;
+    if (valid) {
+        uint32_t tag = P.tags[i];
+        if (load_style(P, P.path_idx[i], &st, &h)) {
+            s = load_segment(P, i, tag);
+            if (s.kind == 1 || s.degenerate) n = 2;
+            else { active = true; f = fit_begin(s); }
+            n_tail = segment_tail<false>(P, i, tag, s, st, h, nullptr, 0);
+        }
+    }
+    uint32_t chunk_base = 0, chunk_used = kChunk;  // no chunk yet
+    while (__any_sync(0xffffffffu, active)) {
+        bool have = false;
+        Piece p;
+        uint32_t nm = 0, np = 0;
+        if (active) {
+            have = fit_next(P, s, f, p);
+            if (have) {
+                nm = (uint32_t)side_plan(p, -h, P.mode, P.tol_fl).total;
+                np = (uint32_t)side_plan(p, h, P.mode, P.tol_fl).total;
+            } else {
+                active = false;
+            }
+        }
+        const uint32_t ballot = __ballot_sync(0xffffffffu, have);
+        const uint32_t cnt = __popc(ballot);
+        if (cnt == 0u) continue;
+        if (chunk_used + cnt > (uint32_t)kChunk) {
+            for (uint32_t k = chunk_used + lane; k < (uint32_t)kChunk; k += 32u)
+                if (chunk_base + k < piece_cap) piece_invalidate(pieces + (uint64_t)(chunk_base + k) * kDescQuads);
+            if (lane == 0u) chunk_base = atomicAdd(piece_ctr, (uint32_t)kChunk);
+            chunk_base = __shfl_sync(0xffffffffu, chunk_base, 0);
+            chunk_used = 0u;
+        }
+        if (have) {
+            uint32_t slot = chunk_base + chunk_used + __popc(ballot & ((1u << lane) - 1u));
+            if (slot < piece_cap) piece_store(pieces + (uint64_t)slot * kDescQuads, p, h, i, n, nm, np);
+            n += nm + np;
+        }
+        chunk_used += cnt;
+    }
+    for (uint32_t k = chunk_used + lane; k < (uint32_t)kChunk; k += 32u)
+        if (chunk_base + k < piece_cap) piece_invalidate(pieces + (uint64_t)(chunk_base + k) * kDescQuads);
+    if (i < P.n_tags) seg_count[i] = n + n_tail;
 }
 
-// (d) write pass: one thread per input segment re-derives its pieces and stores its records
+// (d1) write pass over the piece cache: one thread per output record.
+__global__ void __launch_bounds__(kWpThreads, kWpBlocksPerSM)
+k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, const uint32_t* __restrict__ piece_ctr,
+               const uint64_t* __restrict__ seg_off, float4* __restrict__ out, uint64_t cap_records, uint32_t* err) {
+    __shared__ Piece s_piece[kWpPieces];
+    __shared__ SidePlan s_plan[kWpThreads];
+    __shared__ uint64_t s_base[kWpThreads];
+    __shared__ uint32_t s_pref[kWpThreads + 1];
+    __shared__ uint32_t s_warp[kWpThreads / 32];
+    const uint32_t reserved = *piece_ctr;
+    if (reserved > piece_cap) return;  // cache overflow: k_write_segments takes the whole call
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool arc = P.mode == kModeArc;
+    for (uint32_t tile = blockIdx.x; (uint64_t)tile * kWpPieces < reserved; tile += gridDim.x) {
+        // ---- stage: thread = (piece, side); rebuild the side plan, Z(1) once per piece
+        const uint32_t slot = tile * (uint32_t)kWpPieces + (uint32_t)(tid >> 1);
+        const int side = tid & 1;
+        uint32_t tot = 0;
+        if (slot < reserved) {
+            const float4* d = pieces + (uint64_t)slot * kDescQuads;
+            PieceHead hd = piece_head(d);
+            if (hd.seg != kInvalidSeg) {
+                Piece p;
+                float h;
+                piece_load(d, hd, p, &h);
+                SidePlan sp = side_plan(p, side ? h : -h, P.mode, P.tol_fl);
+                tot = (uint32_t)sp.total;
+                sp.seg = hd.seg;
+                uint64_t base = seg_off[hd.seg] + hd.rel + (side ? hd.n_minus : 0u);
+                if (base + tot > cap_records) { atomicOr(err, kErrCapacity); tot = 0; }
+                s_plan[tid] = sp;
+                s_base[tid] = base;
+                if (side == 0) { es_prepare(p); s_piece[tid >> 1] = p; }
+            }
+        }
+        // ---- block exclusive scan of the side totals
+        uint32_t incl = tot;
+#pragma unroll
+        for (int dd = 1; dd < 32; dd <<= 1) {
+            uint32_t o = __shfl_up_sync(0xffffffffu, incl, dd);
+            if (lane >= dd) incl += o;
+        }
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        uint32_t wex = 0, total = 0;
+#pragma unroll
+        for (int k = 0; k < kWpThreads / 32; k++) {
+            if (k == warp) wex = total;
+            total += s_warp[k];
+        }
+        s_pref[tid] = wex + incl - tot;
+        if (tid == 0) s_pref[kWpThreads] = total;
+        __syncthreads();
+        // ---- one thread per record
+        for (uint32_t r = (uint32_t)tid; r < total; r += (uint32_t)kWpThreads) {
+            int lo = 0, hi = kWpThreads;  // largest k with s_pref[k] <= r
+#pragma unroll
+            for (int step = 0; step < 8; step++) {
+                int mid = (lo + hi) >> 1;
+                if (s_pref[mid] <= r) lo = mid; else hi = mid;
+            }
+            const int k = lo;
+            const SidePlan& sp = s_plan[k];
+            Piece p = s_piece[k >> 1];
+            const bool mirror = (k & 1) != 0;
+            const uint32_t j = r - s_pref[k], nside = (uint32_t)sp.total;
+            V2 a, b;
+            float ang;
+            uint32_t kind;
+            side_record(p, sp, sp.eta, arc, mirror ? nside - 1u - j : j, &a, &b, &ang, &kind);
+            const uint64_t rec = s_base[k] + j;
+            if (mirror) { V2 t = a; a = b; b = t; ang = -ang; kind |= kPlus; }
+            if (!arc) {
+                out[rec] = make_float4(a.x, a.y, b.x, b.y);
+            } else {
+                out[2 * rec] = make_float4(a.x, a.y, b.x, b.y);
+                out[2 * rec + 1] = make_float4(ang, f_of_u(sp.seg), f_of_u(kind), 0.0f);
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// (d2) write pass over the segments: the records that are not Euler-spiral pieces (the two exact offset
+// lines of a straight segment, joins, caps).  When the piece cache overflowed it is the thread-per-segment
+// reference writer for the whole call instead.
 __global__ void __launch_bounds__(kSegThreads)
-k_write(Params P, const uint32_t* __restrict__ seg_count, const uint64_t* __restrict__ seg_off, float4* __restrict__ out,
-        uint64_t cap_records, uint32_t* err) {
+k_write_segments(Params P, const uint32_t* __restrict__ seg_count, const uint64_t* __restrict__ seg_off, float4* __restrict__ out,
+                 uint64_t cap_records, uint32_t piece_cap, const uint32_t* __restrict__ piece_ctr, uint32_t* err) {
     uint32_t i = blockIdx.x * (uint32_t)kSegThreads + threadIdx.x;
     if (i >= P.n_tags) return;
     uint32_t n = seg_count[i];
@@ -38,7 +177,16 @@ k_write(Params P, const uint32_t* __restrict__ seg_count, const uint64_t* __rest
     if (off + n > cap_records) { atomicOr(err, kErrCapacity); return; }
     Writer w;
     w.out = out; w.base = off; w.seg = i; w.mode = P.mode;
-    process_segment<true>(P, i, &w);
+    if (*piece_ctr > piece_cap) { process_segment<true>(P, i, &w); return; }
+    uint32_t tag = P.tags[i];
+    Style st;
+    float h;
+    load_style(P, P.path_idx[i], &st, &h);
+    Seg s = load_segment(P, i, tag);
+    uint32_t first;
+    if (s.kind == 1 || s.degenerate) { emit_straight(s, h, &w); first = 2u; }
+    else first = n - segment_tail<false>(P, i, tag, s, st, h, nullptr, 0);
+    segment_tail<true>(P, i, tag, s, st, h, &w, first);
 }
 
 }  // namespace sx
@@ -60,7 +208,11 @@ struct sx_ctx {
     uint64_t cap_segs;
     uint8_t* sync_area;   // [flags 64 B][d_total 64 B][alloc tile states][tag tile states]
     uint64_t sync_bytes;
-    uint64_t* h_pinned;   // pinned: [0] total, [1] flags
+    uint64_t* h_pinned;   // pinned: [0] total, [1] flags, [2] piece-cache slots reserved
+    float4* pieces;       // piece cache (sx_cache.cuh), piece_cap descriptors
+    uint64_t piece_cap;
+    uint64_t piece_limit; // 0 = no limit (sx_set_piece_cache_limit)
+    int sm_count;
     // last sx_count
     sx::Params P;
     uint64_t n_paths;
@@ -75,6 +227,7 @@ struct sx_ctx {
 
 static uint32_t* ctx_err(sx_ctx* c) { return reinterpret_cast<uint32_t*>(c->sync_area); }
 static uint32_t* ctx_ticket(sx_ctx* c, int k) { return reinterpret_cast<uint32_t*>(c->sync_area) + 4 + 4 * k; }
+static uint32_t* ctx_piece_ctr(sx_ctx* c) { return reinterpret_cast<uint32_t*>(c->sync_area) + 12; }
 static uint64_t* ctx_total(sx_ctx* c) { return reinterpret_cast<uint64_t*>(c->sync_area + 64); }
 
 static uint64_t round_up(uint64_t x, uint64_t m) { return (x + m - 1) / m * m; }
@@ -106,6 +259,18 @@ static sx_status ensure_scratch(sx_ctx* c, uint64_t n) {
     return SX_OK;
 }
 
+static sx_status ensure_pieces(sx_ctx* c, uint64_t need) {
+    if (c->piece_limit && need > c->piece_limit) need = c->piece_limit;
+    if (need <= c->piece_cap) return SX_OK;
+    if (c->pieces) SX_CUDA(cudaFree(c->pieces));
+    c->pieces = nullptr; c->piece_cap = 0;
+    uint64_t cap = c->piece_limit ? need : round_up(need, 1024);
+    if (cap > 0xfffffff0ull) cap = 0xfffffff0ull;
+    SX_CUDA(cudaMalloc(&c->pieces, cap * sx::kDescQuads * sizeof(float4)));
+    c->piece_cap = cap;
+    return SX_OK;
+}
+
 // ====================================================================== C-ABI
 extern "C" {
 
@@ -119,6 +284,8 @@ sx_status sx_create(sx_ctx** out, int32_t device) {
     sx_ctx* c = static_cast<sx_ctx*>(calloc(1, sizeof(sx_ctx)));
     if (!c) return SX_E_INVALID_ARG;
     c->device = device;
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
+    if (c->sm_count <= 0) c->sm_count = 148;
     cudaError_t e = cudaMallocHost(reinterpret_cast<void**>(&c->h_pinned), 64);
     if (e != cudaSuccess) { g_last_cuda = e; free(c); return SX_E_CUDA; }
     *out = c;
@@ -130,6 +297,7 @@ sx_status sx_destroy(sx_ctx* c) {
     cudaSetDevice(c->device);
     cudaDeviceSynchronize();
     cudaFree(c->pt_off);
+    cudaFree(c->pieces);
     cudaFree(c->sync_area);
     cudaFree(c->st_in);
     cudaFree(c->st_out);
@@ -172,33 +340,46 @@ sx_status sx_count(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, const floa
     c->total_known = false;
     c->total = 0;
 
-    // reset the error flag, the tickets, the total and the look-back states
-    SX_CUDA(cudaMemsetAsync(c->sync_area, 0, c->sync_bytes, s));
-    if (n_tags == 0) {
-        SX_CUDA(cudaMemsetAsync(d_path_offsets, 0, 8, s));
-    } else {
-        uint32_t n = P.n_tags;
-        uint32_t n_alloc_tiles = (n + sx::kCntTile - 1) / sx::kCntTile, n_tag_tiles = (n + sx::kTagTile - 1) / sx::kTagTile;
-        uint64_t* alloc_states = reinterpret_cast<uint64_t*>(c->sync_area + 128);
-        sx::TagTileState* tag_states = reinterpret_cast<sx::TagTileState*>(c->sync_area + 128 + round_up((uint64_t)(n_alloc_tiles + 1) * 8, 64));
-        sx::k_tag_scan<<<n_tag_tiles, sx::kScanThreads, 0, s>>>(d_tags, n, (uint32_t)n_points, (uint32_t)n_paths, c->pt_off, c->path_idx,
-                                                               c->sp_first, tag_states, ctx_ticket(c, 0), ctx_err(c));
-        sx::k_count<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(P, c->seg_count, ctx_err(c));
-        sx::k_alloc_scan<<<n_alloc_tiles, sx::kScanThreads, 0, s>>>(c->seg_count, n, d_tags, c->path_idx, (uint32_t)n_paths, c->seg_off,
-                                                                  d_path_offsets, ctx_total(c), alloc_states, ctx_ticket(c, 1), ctx_err(c));
-        c->launches += 3;
-        SX_CUDA(cudaGetLastError());
-    }
-    c->counted = true;
-    if (h_total) {
+    rc = ensure_pieces(c, 2 * n_tags + 4096);
+    if (rc != SX_OK) return rc;
+    for (int attempt = 0;; attempt++) {
+        // reset the error flag, the tickets, the piece-cache counter, the total and the look-back states
+        SX_CUDA(cudaMemsetAsync(c->sync_area, 0, c->sync_bytes, s));
+        if (n_tags == 0) {
+            SX_CUDA(cudaMemsetAsync(d_path_offsets, 0, 8, s));
+        } else {
+            uint32_t n = P.n_tags;
+            uint32_t n_alloc_tiles = (n + sx::kCntTile - 1) / sx::kCntTile, n_tag_tiles = (n + sx::kTagTile - 1) / sx::kTagTile;
+            uint64_t* alloc_states = reinterpret_cast<uint64_t*>(c->sync_area + 128);
+            sx::TagTileState* tag_states = reinterpret_cast<sx::TagTileState*>(c->sync_area + 128 + round_up((uint64_t)(n_alloc_tiles + 1) * 8, 64));
+            sx::k_tag_scan<<<n_tag_tiles, sx::kScanThreads, 0, s>>>(d_tags, n, (uint32_t)n_points, (uint32_t)n_paths, c->pt_off, c->path_idx,
+                                                                   c->sp_first, tag_states, ctx_ticket(c, 0), ctx_err(c));
+            sx::k_count<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(P, c->seg_count, c->pieces, (uint32_t)c->piece_cap,
+                                                                                              ctx_piece_ctr(c), ctx_err(c));
+            sx::k_alloc_scan<<<n_alloc_tiles, sx::kScanThreads, 0, s>>>(c->seg_count, n, d_tags, c->path_idx, (uint32_t)n_paths, c->seg_off,
+                                                                      d_path_offsets, ctx_total(c), alloc_states, ctx_ticket(c, 1), ctx_err(c));
+            c->launches += 3;
+            SX_CUDA(cudaGetLastError());
+        }
+        c->counted = true;
+        if (!h_total) break;  // asynchronous call: a cache overflow is handled on the device (k_write_segments)
         SX_CUDA(cudaMemcpyAsync(&c->h_pinned[0], ctx_total(c), 8, cudaMemcpyDeviceToHost, s));
         SX_CUDA(cudaMemcpyAsync(&c->h_pinned[1], ctx_err(c), 4, cudaMemcpyDeviceToHost, s));
+        SX_CUDA(cudaMemcpyAsync(&c->h_pinned[2], ctx_piece_ctr(c), 4, cudaMemcpyDeviceToHost, s));
         SX_CUDA(cudaStreamSynchronize(s));
         uint32_t flags = static_cast<uint32_t>(c->h_pinned[1] & 0xffffffffu);
+        uint64_t reserved = c->h_pinned[2] & 0xffffffffu;
+        if (flags & sx::kErrBadStream) { c->counted = false; *h_total = 0; return SX_E_BAD_STREAM; }
+        if (reserved > c->piece_cap && attempt == 0 && !(c->piece_limit && c->piece_cap >= c->piece_limit)) {
+            // the piece cache was too small: size it from what this call needed and count again
+            rc = ensure_pieces(c, reserved + reserved / 8 + 4096);
+            if (rc != SX_OK) return rc;
+            continue;
+        }
         *h_total = c->h_pinned[0];
         c->total = c->h_pinned[0];
         c->total_known = true;
-        if (flags & sx::kErrBadStream) { c->counted = false; *h_total = 0; return SX_E_BAD_STREAM; }
+        break;
     }
     return SX_OK;
 }
@@ -212,9 +393,12 @@ sx_status sx_write(sx_ctx* c, void* d_out_records, uint64_t cap_records, void* c
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     SX_CUDA(cudaSetDevice(c->device));
     uint32_t n = c->P.n_tags;
-    sx::k_write<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(c->P, c->seg_count, c->seg_off,
-                                                                                      static_cast<float4*>(d_out_records), cap_records, ctx_err(c));
-    c->launches += 1;
+    float4* out = static_cast<float4*>(d_out_records);
+    sx::k_write_pieces<<<c->sm_count * sx::kWpBlocksPerSM, sx::kWpThreads, 0, s>>>(c->P, c->pieces, (uint32_t)c->piece_cap, ctx_piece_ctr(c), c->seg_off,
+                                                                                 out, cap_records, ctx_err(c));
+    sx::k_write_segments<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(c->P, c->seg_count, c->seg_off, out, cap_records,
+                                                                                               (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_err(c));
+    c->launches += 2;
     SX_CUDA(cudaGetLastError());
     return SX_OK;
 }
@@ -312,6 +496,19 @@ sx_status sx_last_error(sx_ctx* c, void* cuda_stream) {
     uint32_t flags = static_cast<uint32_t>(c->h_pinned[1] & 0xffffffffu);
     if (flags & sx::kErrBadStream) return SX_E_BAD_STREAM;
     if (flags & sx::kErrCapacity) return SX_E_CAPACITY;
+    return SX_OK;
+}
+
+sx_status sx_set_piece_cache_limit(sx_ctx* c, uint64_t max_pieces) {
+    if (!c) return SX_E_INVALID_ARG;
+    cudaSetDevice(c->device);
+    cudaDeviceSynchronize();
+    c->piece_limit = max_pieces;
+    if (max_pieces && c->piece_cap > max_pieces) {
+        cudaFree(c->pieces);
+        c->pieces = nullptr; c->piece_cap = 0;
+    }
+    c->counted = false;
     return SX_OK;
 }
 

@@ -209,10 +209,13 @@ struct SidePlan {
     EvoPlan evo;     // of the super-critical range, if any
     bool cusp_a, cusp_b;
     int total;       // records of this side
+    float eta;       // signed offset of the side
+    uint32_t seg;    // source segment (filled by the write kernel)
 };
 
 SX_DEV SidePlan side_plan(const Piece& p, float eta, int mode, float tol_fl) {
     SidePlan s;
+    s.eta = eta; s.seg = 0u;
     float g0 = 1.0f - es_kappa(p, 0.0f) * eta, g1 = 1.0f - es_kappa(p, 1.0f) * eta;  // cusp0, cusp1 (L382-384)
     float tc = (g0 * g1 >= 0.0f) ? 1.0f : g0 / (g0 - g1);                            // L386
     float ra[2], rb[2];

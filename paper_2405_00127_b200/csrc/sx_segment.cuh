@@ -182,91 +182,124 @@ SX_DEV uint32_t emit_cap(const Params& P, const Style& st, V2 V, V2 T, float h, 
     return 1;
 }
 
-// ---------------------------------------------------------------- Alg. 2: cubic -> Euler spirals -> records
+// ---------------------------------------------------------------- Alg. 2: cubic -> Euler spirals
 // Iterative bisection with the two-word stack (t0_u, dt), pop by count-trailing-zeros (L444).  One pass
-// serves both sides: the fit does not depend on the offset.
-template <bool EMIT>
-SX_DEV uint32_t flatten_cubic(const Params& P, const Seg& s, float h, const Writer* w) {
-    uint32_t t0_u = 0, n = 0;
-    float dt = 1.0f;
-    V2 last_p = v2(0.0f, 0.0f), last_u = s.ts;
-    float last_qmag = sqrtf(len2(s.c1));
+// serves both sides: the fit does not depend on the offset.  The loop is written as a resumable
+// generator (fit_next returns one accepted piece per call) so that the thread-per-segment writer, the
+// count kernel and the piece cache all run the identical instruction sequence.
+struct FitState {
+    uint32_t t0_u;
+    float dt;
+    V2 last_p, last_u;
+    float last_qmag;
+};
+SX_DEV FitState fit_begin(const Seg& s) {
+    FitState f;
+    f.t0_u = 0u; f.dt = 1.0f;
+    f.last_p = v2(0.0f, 0.0f); f.last_u = s.ts;
+    f.last_qmag = sqrtf(len2(s.c1));
+    return f;
+}
+// advances Alg. 2 until the next accepted piece (true, piece in p) or the end of the segment (false)
+SX_DEV bool fit_next(const Params& P, const Seg& s, FitState& f, Piece& p) {
     for (;;) {
-        float t0 = (float)t0_u * dt;
-        if (t0 == 1.0f) break;
-        float t1 = t0 + dt;
+        float t0 = (float)f.t0_u * f.dt;
+        if (t0 == 1.0f) return false;
+        float t1 = t0 + f.dt;
         V2 next_p, next_u;
         float next_qmag, th0, th1, chord;
-        eval_cubic(s, t1, dt, &next_p, &next_qmag, &next_u);
-        V2 ch = next_p - last_p;
-        float err = fit_error(last_u, next_u, last_qmag, next_qmag, ch, dt, &th0, &th1, &chord);
-        if (err <= P.tol_es || dt <= kDtMin) {
-            Piece p;
+        eval_cubic(s, t1, f.dt, &next_p, &next_qmag, &next_u);
+        V2 ch = next_p - f.last_p;
+        float err = fit_error(f.last_u, next_u, f.last_qmag, next_qmag, ch, f.dt, &th0, &th1, &chord);
+        if (err <= P.tol_es || f.dt <= kDtMin) {
             p.base = s.P0; p.P3 = s.P3;
-            p.la = last_p; p.lb = next_p;
-            p.ua = last_u; p.ub = next_u;
+            p.la = f.last_p; p.lb = next_p;
+            p.ua = f.last_u; p.ub = next_u;
             p.ch = ch;
             p.at0 = (t0 == 0.0f); p.at1 = (t1 == 1.0f);
             piece_params(p, th0, th1, chord);
-            uint32_t nm = piece_side<EMIT>(p, -h, false, P, w, n);  // -h side, forward
-            n += nm;
-            uint32_t np = piece_side<EMIT>(p, h, true, P, w, n);    // +h side, mirrored
-            n += np;
-            t0_u += 1;
-            int shift = ctz32(t0_u);
-            t0_u >>= shift;
-            dt *= (float)(1u << shift);
-            last_p = next_p; last_u = next_u; last_qmag = next_qmag;
-        } else {
-            t0_u *= 2;
-            dt *= 0.5f;
+            f.t0_u += 1u;
+            int shift = ctz32(f.t0_u);
+            f.t0_u >>= shift;
+            f.dt *= (float)(1u << shift);
+            f.last_p = next_p; f.last_u = next_u; f.last_qmag = next_qmag;
+            return true;
         }
+        f.t0_u *= 2u;
+        f.dt *= 0.5f;
+    }
+}
+
+template <bool EMIT>
+SX_DEV uint32_t flatten_cubic(const Params& P, const Seg& s, float h, const Writer* w) {
+    uint32_t n = 0;
+    FitState f = fit_begin(s);
+    Piece p;
+    while (fit_next(P, s, f, p)) {
+        n += piece_side<EMIT>(p, -h, false, P, w, n);  // -h side, forward
+        n += piece_side<EMIT>(p, h, true, P, w, n);    // +h side, mirrored
     }
     return n;
 }
 
 // ---------------------------------------------------------------- Alg. 1: the whole segment
-template <bool EMIT>
-SX_DEV uint32_t process_segment(const Params& P, uint32_t i, Writer* w) {
-    uint32_t tag = P.tags[i];
-    uint32_t path = P.path_idx[i];
+SX_DEV bool load_style(const Params& P, uint32_t path, Style* st, float* h) {
 #ifdef __CUDA_ARCH__
     uint4 raw = __ldg(reinterpret_cast<const uint4*>(P.styles) + path);
 #else
     uint4 raw = reinterpret_cast<const uint4*>(P.styles)[path];
 #endif
-    Style st;
-    st.width = u2f(raw.x);
-    st.miter_limit = u2f(raw.y);
-    st.join = (int)(raw.z & 0xffu);
-    st.cap = (int)((raw.z >> 8) & 0xffu);
-    float h = 0.5f * st.width * P.scale;
-    if (!(h > 0.0f && h < INFINITY)) return 0;  // width <= 0 or non-finite: the path emits nothing
-    Seg s = load_segment(P, i, tag);
-    uint32_t n;
-    if (s.kind == 1 || s.degenerate) {
-        // straight fast path (R-1b): the two offset lines are exact
-        if (EMIT) {
-            w->put(0, offset_point(s.P0, s.ts, -h), offset_point(s.P3, s.te, -h), 0.0f, kOffset);
-            w->put(1, offset_point(s.P3, s.te, h), offset_point(s.P0, s.ts, h), 0.0f, kOffset | kPlus);
-        }
-        n = 2;
-    } else {
-        n = flatten_cubic<EMIT>(P, s, h, w);
-    }
+    st->width = u2f(raw.x);
+    st->miter_limit = u2f(raw.y);
+    st->join = (int)(raw.z & 0xffu);
+    st->cap = (int)((raw.z >> 8) & 0xffu);
+    *h = 0.5f * st->width * P.scale;
+    return *h > 0.0f && *h < INFINITY;  // width <= 0 or non-finite: the path emits nothing
+}
+
+// what follows the offset curves of segment i (Alg. 1): the join with its partner, or, on the last
+// segment of an open subpath, [end cap][start cap]
+template <bool EMIT>
+SX_DEV uint32_t segment_tail(const Params& P, uint32_t i, uint32_t tag, const Seg& s, const Style& st, float h, const Writer* w, uint32_t first) {
     bool sp_end = ((tag >> 2) | (tag >> 4)) & 1u;
     bool closed = (tag >> 7) & 1u;
+    uint32_t n = 0;
     if (!sp_end || closed) {
         uint32_t j = sp_end ? P.sp_first[i] : i + 1;
         V2 W, T1;
         load_segment_start(P, j, &W, &T1);
-        n += emit_join<EMIT>(P, st, s.P3, s.te, W, T1, h, w, n);
+        n += emit_join<EMIT>(P, st, s.P3, s.te, W, T1, h, w, first);
     } else {
         V2 F, Tf;
         load_segment_start(P, P.sp_first[i], &F, &Tf);
-        n += emit_cap<EMIT>(P, st, s.P3, s.te, h, w, n);
-        n += emit_cap<EMIT>(P, st, F, v2(-Tf.x, -Tf.y), h, w, n);
+        n += emit_cap<EMIT>(P, st, s.P3, s.te, h, w, first);
+        n += emit_cap<EMIT>(P, st, F, v2(-Tf.x, -Tf.y), h, w, first + n);
     }
+    return n;
+}
+
+// straight fast path (R-1b): the two offset lines of a line (or fully degenerate) segment are exact
+SX_DEV void emit_straight(const Seg& s, float h, const Writer* w) {
+    w->put(0, offset_point(s.P0, s.ts, -h), offset_point(s.P3, s.te, -h), 0.0f, kOffset);
+    w->put(1, offset_point(s.P3, s.te, h), offset_point(s.P0, s.ts, h), 0.0f, kOffset | kPlus);
+}
+
+// thread-per-segment reference path: everything segment i emits, in canonical order
+template <bool EMIT>
+SX_DEV uint32_t process_segment(const Params& P, uint32_t i, Writer* w) {
+    uint32_t tag = P.tags[i];
+    Style st;
+    float h;
+    if (!load_style(P, P.path_idx[i], &st, &h)) return 0;
+    Seg s = load_segment(P, i, tag);
+    uint32_t n;
+    if (s.kind == 1 || s.degenerate) {
+        if (EMIT) emit_straight(s, h, w);
+        n = 2;
+    } else {
+        n = flatten_cubic<EMIT>(P, s, h, w);
+    }
+    n += segment_tail<EMIT>(P, i, tag, s, st, h, w, n);
     return n;
 }
 

@@ -146,6 +146,33 @@ def test_host_buffer_entry_point_matches_device_entry_point(B, ctx, name, npaths
     assert np.array_equal(gd.angle.view(np.uint32), gh.angle.view(np.uint32))
 
 
+@pytest.mark.parametrize("name,npaths,mode,want_total", [("c1", 64, 0, True), ("c1", 64, 0, False), ("c2", 300, 1, False)])
+def test_piece_cache_overflow_falls_back_to_the_segment_writer(B, name, npaths, mode, want_total):
+    """A piece cache that is too small (sx_set_piece_cache_limit) must not change a single bit of the output: the
+    thread-per-segment writer takes over on the device, in the synchronous and in the asynchronous call."""
+    sc = S.make(name, n_paths=npaths)
+    dev = "cuda:0"
+    tags, pts, sty = B.scene_to_torch(sc, device=dev)
+    width = 4 if mode == 0 else 8
+    outs = []
+    for limit in (0, 96):
+        c = B.sx_create(0)
+        try:
+            B.sx_set_piece_cache_limit(c, limit)
+            poff = torch.empty(sc.n_paths + 1, dtype=torch.int64, device=dev)
+            total = B.sx_count(c, tags, pts, sty, sc.affine, sc.tolerance, mode, poff)
+            if not want_total:
+                B.sx_count(c, tags, pts, sty, sc.affine, sc.tolerance, mode, poff, want_total=False)
+            out = torch.full((total, width), float("nan"), dtype=torch.float32, device=dev)
+            B.sx_write(c, out, total)
+            torch.cuda.synchronize()
+            assert B.sx_last_error(c) == 0
+            outs.append((out.cpu().numpy().view(np.uint32), poff.cpu().numpy()))
+        finally:
+            B.sx_destroy(c)
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
 # ---------------------------------------------------------------- the same invariant checks the oracle passes
 @pytest.mark.parametrize("name,npaths,mode", [("c1", 64, 0), ("c2", 240, 0), ("c2", 240, 1), ("c3", 300, 0), ("c4", 200, 1), ("c5", 12, 0), ("c5", 12, 1)])
 def test_gpu_output_passes_the_invariants(B, ctx, name, npaths, mode):
