@@ -130,7 +130,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device(dev))
 
     mode = MODE_OF[args.workload]
-    sc = make_scene(args.workload)  # replicas only: every rank expands the whole scene
+    sc = make_scene(args.workload, n_paths=args.paths)  # replicas only: every rank expands the whole scene
     n_seg, n_paths = sc.n_segments, sc.n_paths
     tags, pts, sty = B.scene_to_torch(sc, device=dev)
     width = 8 if mode else 4
@@ -242,6 +242,7 @@ def main():
     ap.add_argument("--workload", default="c4", choices=sorted(MODE_OF))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--paths", type=int, default=None, help="profiling only: shrink the workload to this many paths")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -53,24 +53,42 @@ SX_DEV void piece_load(const float4* slot, const PieceHead& hd, Piece& p, float*
 }
 
 // ---------------------------------------------------------------- record j (forward-t order) of one side
-// Same vertices, in the same order, as piece_side<true> (sx_segment.cuh) walks sequentially.
+// Same vertices, in the same order, as piece_side<true> (sx_segment.cuh) walks sequentially.  The record
+// index is first DECODED into two vertex specifications (cheap integer logic, where the threads of a warp
+// may diverge); the expensive part -- subdivision parameter, Euler-spiral integral, normal offset -- then
+// runs once per end point in a single code path that every thread of the warp executes together.
+struct VertexSpec {
+    float t;      // parameter when src == 0
+    int i;        // subdivision index when src != 0
+    int src;      // 0: t given, 1: offset_t(i), 2: evolute_t(i)
+    bool evo;     // point on the evolute (r = 1/kappa) instead of the parallel curve (r = eta)
+};
+SX_DEV VertexSpec vs_fixed(float t, bool evo) { VertexSpec v; v.t = t; v.i = 0; v.src = 0; v.evo = evo; return v; }
+SX_DEV VertexSpec vs_offset(const OffPlan& o, uint32_t i) {
+    VertexSpec v; v.evo = false; v.i = (int)i; v.t = i == 0u ? o.ta : o.tb; v.src = (i == 0u || i == (uint32_t)o.n) ? 0 : 1; return v;
+}
+SX_DEV VertexSpec vs_evolute(const SidePlan& s, const OffPlan& o, uint32_t i) {
+    const uint32_t ne = (uint32_t)s.evo.n;
+    if (i == 0u) return vs_fixed(o.ta, !s.cusp_a);   // the evolute meets the offset curve at the cusp
+    if (i == ne) return vs_fixed(o.tb, !s.cusp_b);
+    VertexSpec v; v.evo = true; v.i = (int)i; v.t = 0.0f; v.src = 2; return v;
+}
+
 SX_DEV void side_record(Piece& p, const SidePlan& s, float eta, bool arc, uint32_t j, V2* a, V2* b, float* angle, uint32_t* kind) {
-    *angle = 0.0f;
+    VertexSpec va = vs_fixed(0.0f, false), vb = va;
+    OffPlan o = s.off[0];
+    bool want_angle = false;
+    *kind = kOffset;
 #pragma unroll
     for (int r = 0; r < 2; r++) {
         if (r >= s.nr) break;
-        const OffPlan o = r == 0 ? s.off[0] : s.off[1];
+        const OffPlan oo = r == 0 ? s.off[0] : s.off[1];
         const bool sup = r == 0 ? s.sup[0] : s.sup[1];
-        const uint32_t n = (uint32_t)o.n;
+        const uint32_t n = (uint32_t)oo.n;
         if (!sup) {
             if (j < n) {
-                float t0 = j == 0u ? o.ta : offset_t(p, o, eta, (int)j);
-                float t1 = j + 1u == n ? o.tb : offset_t(p, o, eta, (int)j + 1);
-                *a = es_offset(p, t0, eta);
-                *b = es_offset(p, t1, eta);
-                if (arc) *angle = es_dphi(p, t0, t1);
-                *kind = kOffset;
-                return;
+                o = oo; va = vs_offset(oo, j); vb = vs_offset(oo, j + 1u); want_angle = arc; *kind = kOffset;
+                break;
             }
             j -= n;
         } else {
@@ -78,32 +96,39 @@ SX_DEV void side_record(Piece& p, const SidePlan& s, float eta, bool arc, uint32
             const uint32_t nca = s.cusp_a ? 0u : 2u, ncb = s.cusp_b ? 0u : 2u, ne = (uint32_t)s.evo.n;
             const uint32_t tot = nca + 2u * ne + n + ncb;
             if (j < tot) {
+                o = oo;
                 if (j < nca) {
-                    *a = es_offset(p, o.ta, eta); *b = es_evolute(p, o.ta); *kind = kConnector;
+                    va = vs_fixed(oo.ta, false); vb = vs_fixed(oo.ta, true); *kind = kConnector;
                 } else if (j < nca + 2u * ne) {
                     uint32_t i = j - nca;
                     if (i >= ne) i -= ne;
-                    *a = i == 0u ? (s.cusp_a ? es_offset(p, o.ta, eta) : es_evolute(p, o.ta)) : es_evolute(p, evolute_t(p, s.evo, (int)i));
-                    *b = i + 1u == ne ? (s.cusp_b ? es_offset(p, o.tb, eta) : es_evolute(p, o.tb)) : es_evolute(p, evolute_t(p, s.evo, (int)i + 1));
-                    *kind = kEvolute;
+                    va = vs_evolute(s, oo, i); vb = vs_evolute(s, oo, i + 1u); *kind = kEvolute;
                 } else if (j < nca + 2u * ne + n) {
-                    uint32_t hi = n - (j - (nca + 2u * ne)), lo = hi - 1u;  // reversed offset (L403, L191): vertex hi -> vertex lo
-                    float t1 = hi == n ? o.tb : offset_t(p, o, eta, (int)hi);
-                    float t0 = lo == 0u ? o.ta : offset_t(p, o, eta, (int)lo);
-                    *a = es_offset(p, t1, eta);
-                    *b = es_offset(p, t0, eta);
-                    if (arc) *angle = es_dphi(p, t1, t0);
-                    *kind = kOffsetRev;
+                    uint32_t hi = n - (j - (nca + 2u * ne));  // reversed offset (L403, L191): vertex hi -> vertex hi-1
+                    va = vs_offset(oo, hi); vb = vs_offset(oo, hi - 1u); want_angle = arc; *kind = kOffsetRev;
                 } else {
-                    *a = es_evolute(p, o.tb); *b = es_offset(p, o.tb, eta); *kind = kConnector;
+                    va = vs_fixed(oo.tb, true); vb = vs_fixed(oo.tb, false); *kind = kConnector;
                 }
-                return;
+                break;
             }
             j -= tot;
         }
     }
-    *a = *b = v2(0.0f, 0.0f);
-    *kind = kOffset;
+    // ---- the convergent part
+    float tt[2];
+    V2 pt[2];
+#pragma unroll 1
+    for (int e = 0; e < 2; e++) {
+        const VertexSpec v = e == 0 ? va : vb;
+        float t = v.t;
+        if (v.src == 1) t = offset_t(p, o, eta, v.i);
+        else if (v.src == 2) t = evolute_t(p, s.evo, v.i);
+        const float r = v.evo ? 1.0f / es_kappa(p, t) : eta;
+        tt[e] = t;
+        pt[e] = normal_point(p, t, r);
+    }
+    *a = pt[0]; *b = pt[1];
+    *angle = want_angle ? es_dphi(p, tt[0], tt[1]) : 0.0f;
 }
 
 }  // namespace sx

@@ -164,8 +164,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
 }
 
 // (d2) write pass over the segments: the records that are not Euler-spiral pieces (the two exact offset
-// lines of a straight segment, joins, caps).  When the piece cache overflowed it is the thread-per-segment
-// reference writer for the whole call instead.
+// lines of a straight segment, joins, caps).
 __global__ void __launch_bounds__(kSegThreads)
 k_write_segments(Params P, const uint32_t* __restrict__ seg_count, const uint64_t* __restrict__ seg_off, float4* __restrict__ out,
                  uint64_t cap_records, uint32_t piece_cap, const uint32_t* __restrict__ piece_ctr, uint32_t* err) {
@@ -177,7 +176,7 @@ k_write_segments(Params P, const uint32_t* __restrict__ seg_count, const uint64_
     if (off + n > cap_records) { atomicOr(err, kErrCapacity); return; }
     Writer w;
     w.out = out; w.base = off; w.seg = i; w.mode = P.mode;
-    if (*piece_ctr > piece_cap) { process_segment<true>(P, i, &w); return; }
+    if (*piece_ctr > piece_cap) return;  // cache overflow: k_write_fallback takes the whole call
     uint32_t tag = P.tags[i];
     Style st;
     float h;
@@ -187,6 +186,23 @@ k_write_segments(Params P, const uint32_t* __restrict__ seg_count, const uint64_
     if (s.kind == 1 || s.degenerate) { emit_straight(s, h, &w); first = 2u; }
     else first = n - segment_tail<false>(P, i, tag, s, st, h, nullptr, 0);
     segment_tail<true>(P, i, tag, s, st, h, &w, first);
+}
+
+// (d3) thread-per-segment writer for a call whose pieces did not fit the cache (sx_set_piece_cache_limit, or
+// an asynchronous sx_count that outgrew the cache): repeats Alg. 2 per segment.  Exits at once otherwise.
+__global__ void __launch_bounds__(kSegThreads)
+k_write_fallback(Params P, const uint32_t* __restrict__ seg_count, const uint64_t* __restrict__ seg_off, float4* __restrict__ out,
+                 uint64_t cap_records, uint32_t piece_cap, const uint32_t* __restrict__ piece_ctr, uint32_t* err) {
+    if (*piece_ctr <= piece_cap) return;
+    uint32_t i = blockIdx.x * (uint32_t)kSegThreads + threadIdx.x;
+    if (i >= P.n_tags) return;
+    uint32_t n = seg_count[i];
+    if (n == 0u) return;
+    uint64_t off = seg_off[i];
+    if (off + n > cap_records) { atomicOr(err, kErrCapacity); return; }
+    Writer w;
+    w.out = out; w.base = off; w.seg = i; w.mode = P.mode;
+    process_segment<true>(P, i, &w);
 }
 
 }  // namespace sx
@@ -217,6 +233,7 @@ struct sx_ctx {
     sx::Params P;
     uint64_t n_paths;
     bool counted, total_known;
+    bool cache_fits;      // known on the host (synchronous sx_count): every piece of the last count is cached
     uint64_t total;
     uint64_t launches;
     // staging for stroke_expand_host
@@ -338,6 +355,7 @@ sx_status sx_count(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, const floa
     P.n_tags = static_cast<uint32_t>(n_tags);
     c->n_paths = n_paths;
     c->total_known = false;
+    c->cache_fits = false;
     c->total = 0;
 
     rc = ensure_pieces(c, 2 * n_tags + 4096);
@@ -379,6 +397,7 @@ sx_status sx_count(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, const floa
         *h_total = c->h_pinned[0];
         c->total = c->h_pinned[0];
         c->total_known = true;
+        c->cache_fits = reserved <= c->piece_cap;
         break;
     }
     return SX_OK;
@@ -399,6 +418,11 @@ sx_status sx_write(sx_ctx* c, void* d_out_records, uint64_t cap_records, void* c
     sx::k_write_segments<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(c->P, c->seg_count, c->seg_off, out, cap_records,
                                                                                                (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_err(c));
     c->launches += 2;
+    if (!c->cache_fits) {
+        sx::k_write_fallback<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(c->P, c->seg_count, c->seg_off, out, cap_records,
+                                                                                                   (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_err(c));
+        c->launches += 1;
+    }
     SX_CUDA(cudaGetLastError());
     return SX_OK;
 }

@@ -109,19 +109,21 @@ SX_DEV void es_eval(Piece& p, float t, V2* pos, V2* tan) {
 // canonical offset point of a global vertex V with unit tangent u: V + eta N, N = (-u.y, u.x)
 SX_DEV V2 offset_point(V2 V, V2 u, float eta) { return v2(fmaf(eta, -u.y, V.x), fmaf(eta, u.x, V.y)); }
 
-// point at signed normal distance r from the spiral at fraction t (r = eta: parallel curve; r = 1/kappa: evolute)
+// point at signed normal distance r from the spiral at fraction t (r = eta: parallel curve; r = 1/kappa: evolute).
+// At t = 0 and t = 1 the cubic's own point and tangent are used, so that adjacent pieces (and the join of the
+// next segment) share bits.  The spiral is evaluated unconditionally and the end-point cases are selected
+// afterwards, so that a warp evaluating a mix of interior and end vertices stays converged.
 SX_DEV V2 normal_point(Piece& p, float t, float r) {
-    if (t == 0.0f) {
-        if (p.at0) return offset_point(p.base, p.ua, r);
-        return v2(p.base.x + fmaf(r, -p.ua.y, p.la.x), p.base.y + fmaf(r, p.ua.x, p.la.y));
-    }
-    if (t == 1.0f) {
-        if (p.at1) return offset_point(p.P3, p.ub, r);
-        return v2(p.base.x + fmaf(r, -p.ub.y, p.lb.x), p.base.y + fmaf(r, p.ub.x, p.lb.y));
-    }
     V2 l, T;
     es_eval(p, t, &l, &T);
-    return v2(p.base.x + fmaf(r, -T.y, l.x), p.base.y + fmaf(r, T.x, l.y));
+    const bool e0 = t == 0.0f, e1 = t == 1.0f;
+    if (e0) { l = p.la; T = p.ua; }
+    if (e1) { l = p.lb; T = p.ub; }
+    const float ox = fmaf(r, -T.y, l.x), oy = fmaf(r, T.x, l.y);
+    V2 g = v2(p.base.x + ox, p.base.y + oy);
+    if (e0 && p.at0) g = offset_point(p.base, p.ua, r);
+    if (e1 && p.at1) g = offset_point(p.P3, p.ub, r);
+    return g;
 }
 SX_DEV V2 es_offset(Piece& p, float t, float eta) { return normal_point(p, t, eta); }
 SX_DEV V2 es_evolute(Piece& p, float t) { return normal_point(p, t, 1.0f / es_kappa(p, t)); }  // section 6
