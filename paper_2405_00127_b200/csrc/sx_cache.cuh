@@ -49,7 +49,6 @@ SX_DEV void piece_load(const float4* slot, const PieceHead& hd, Piece& p, float*
     p.ch = p.lb - p.la;  // the same subtraction fit_next performed
     p.k0 = d.x; p.k1 = d.y; p.L = d.z; *h = d.w;
     p.at0 = hd.at0; p.at1 = hd.at1;
-    p.zready = false;
 }
 
 // ---------------------------------------------------------------- record j (forward-t order) of one side
@@ -74,7 +73,7 @@ SX_DEV VertexSpec vs_evolute(const SidePlan& s, const OffPlan& o, uint32_t i) {
     VertexSpec v; v.evo = true; v.i = (int)i; v.t = 0.0f; v.src = 2; return v;
 }
 
-SX_DEV void side_record(Piece& p, const SidePlan& s, float eta, bool arc, uint32_t j, V2* a, V2* b, float* angle, uint32_t* kind) {
+SX_DEV void side_record(const Piece& p, const Spiral& z, const SidePlan& s, float eta, bool arc, uint32_t j, V2* a, V2* b, float* angle, uint32_t* kind) {
     VertexSpec va = vs_fixed(0.0f, false), vb = va;
     OffPlan o = s.off[0];
     bool want_angle = false;
@@ -115,8 +114,8 @@ SX_DEV void side_record(Piece& p, const SidePlan& s, float eta, bool arc, uint32
         }
     }
     // ---- the convergent part
-    float tt[2];
-    V2 pt[2];
+    float t0 = 0.0f, t1 = 0.0f;
+    V2 p0 = v2(0.0f, 0.0f), p1 = p0;
 #pragma unroll 1
     for (int e = 0; e < 2; e++) {
         const VertexSpec v = e == 0 ? va : vb;
@@ -124,11 +123,11 @@ SX_DEV void side_record(Piece& p, const SidePlan& s, float eta, bool arc, uint32
         if (v.src == 1) t = offset_t(p, o, eta, v.i);
         else if (v.src == 2) t = evolute_t(p, s.evo, v.i);
         const float r = v.evo ? 1.0f / es_kappa(p, t) : eta;
-        tt[e] = t;
-        pt[e] = normal_point(p, t, r);
+        const V2 g = normal_point(p, z, t, r);
+        if (e == 0) { t0 = t; p0 = g; } else { t1 = t; p1 = g; }
     }
-    *a = pt[0]; *b = pt[1];
-    *angle = want_angle ? es_dphi(p, tt[0], tt[1]) : 0.0f;
+    *a = p0; *b = p1;
+    *angle = want_angle ? es_dphi(p, t0, t1) : 0.0f;
 }
 
 }  // namespace sx

@@ -85,6 +85,7 @@ __global__ void __launch_bounds__(kWpThreads, kWpBlocksPerSM)
 k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, const uint32_t* __restrict__ piece_ctr,
                const uint64_t* __restrict__ seg_off, float4* __restrict__ out, uint64_t cap_records, uint32_t* err) {
     __shared__ Piece s_piece[kWpPieces];
+    __shared__ Spiral s_spiral[kWpPieces];
     __shared__ SidePlan s_plan[kWpThreads];
     __shared__ uint64_t s_base[kWpThreads];
     __shared__ uint32_t s_pref[kWpThreads + 1];
@@ -112,7 +113,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
                 if (base + tot > cap_records) { atomicOr(err, kErrCapacity); tot = 0; }
                 s_plan[tid] = sp;
                 s_base[tid] = base;
-                if (side == 0) { es_prepare(p); s_piece[tid >> 1] = p; }
+                if (side == 0) { es_prepare(p, s_spiral[tid >> 1]); s_piece[tid >> 1] = p; }
             }
         }
         // ---- block exclusive scan of the side totals
@@ -149,7 +150,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
             V2 a, b;
             float ang;
             uint32_t kind;
-            side_record(p, sp, sp.eta, arc, mirror ? nside - 1u - j : j, &a, &b, &ang, &kind);
+            side_record(p, s_spiral[k >> 1], sp, sp.eta, arc, mirror ? nside - 1u - j : j, &a, &b, &ang, &kind);
             const uint64_t rec = s_base[k] + j;
             if (mirror) { V2 t = a; a = b; b = t; ang = -ang; kind |= kPlus; }
             if (!arc) {

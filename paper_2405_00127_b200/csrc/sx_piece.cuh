@@ -39,9 +39,7 @@ struct Piece {
     V2 ua, ub;       // unit tangents of the cubic at the piece ends
     V2 ch;           // chord lb - la
     float k0, k1, L; // total turning, GHI k1, arc length chord / c (App. A; kappa(s) = k0 + k1 s, s in [-1/2,1/2], R-1)
-    float wr, wi;    // 1 / Z(1) (complex), filled by es_prepare
     bool at0, at1;   // the piece starts at t=0 / ends at t=1 of the segment
-    bool zready;
 };
 
 SX_DEV void piece_params(Piece& p, float th0, float th1, float chord) {
@@ -51,57 +49,84 @@ SX_DEV void piece_params(Piece& p, float th0, float th1, float chord) {
     if (!(cc > 0.05f)) cc = 0.05f;
     p.L = chord / cc;
     if (!(p.L > 1e-12f)) p.L = 1e-12f;
-    p.zready = false;
 }
 
 SX_DEV float es_kappa(const Piece& p, float t) { return (p.k0 + p.k1 * (t - 0.5f)) / p.L; }
 
 // ---------------------------------------------------------------- Euler-spiral integral (R-2)
-// Z(t) = int_0^t exp(i((k0-k1/2)u + k1 u^2/2)) du, 8-point Gauss-Legendre in fp32 (the phase spans at
-// most a few radians on an accepted piece, where the 8-point rule is at fp32 round-off).
-SX_DEV void es_integral(float k0, float k1, float t, float* zx, float* zy) {
-    const float gx[4] = {0.18343464249564980f, 0.52553240991632899f, 0.79666647741362674f, 0.96028985649753623f};
-    const float gw[4] = {0.36268378337836198f, 0.31370664587788729f, 0.22238103445337447f, 0.10122853629037626f};
-    float a = k0 - 0.5f * k1, hk = 0.5f * k1, ht = 0.5f * t;
-    float sx_ = 0.0f, sy_ = 0.0f;
-#pragma unroll
-    for (int j = 0; j < 4; j++) {
-        float u0 = ht * (1.0f - gx[j]), u1 = ht * (1.0f + gx[j]);
-        float p0 = u0 * fmaf(hk, u0, a), p1 = u1 * fmaf(hk, u1, a);
-        float s0, c0, s1, c1;
-        sincosf(p0, &s0, &c0);
-        sincosf(p1, &s1, &c1);
-        sx_ = fmaf(gw[j], c0 + c1, sx_);
-        sy_ = fmaf(gw[j], s0 + s1, sy_);
-    }
-    *zx = ht * sx_;
-    *zy = ht * sy_;
+// Z(t) = int_0^t exp(i phi(u)) du, phi(u) = (k0-k1/2) u + k1 u^2/2.  Evaluated from a per-piece table of
+// anchors Z(k/8), k = 0..8 (accumulated once per piece by 3-point Gauss-Legendre on each eighth), plus a
+// 3-point Gauss-Legendre rule from the nearest anchor to t (|t - k/8| <= 1/16).  On an accepted piece
+// |phi'| stays below ~20 rad per unit t (|k0| <= 4.2 by the 120-degree guard R-4, k1 ~ 6 (th1 - th0)), so
+// a vertex integrates over at most ~1 rad of phase, where the 3-point rule is at fp32 round-off; the cost
+// per vertex is 3 sincos instead of a full-interval high-order rule.
+constexpr int kAnchors = 8;
+struct Spiral {
+    float wr, wi;                          // 1 / Z(1) (complex)
+    float zx[kAnchors + 1], zy[kAnchors + 1];
+};
+
+// sin and cos of a moderate argument (|x| < ~1e3): two-constant Cody-Waite reduction by pi/2 and the
+// classic single-precision minimax kernels on [-pi/4, pi/4] (errors ~1e-7), all on the FMA pipe.
+SX_DEV void sx_sincos(float x, float* s, float* c) {
+    float k = rintf(x * 0.63661977236758134f);
+    float r = fmaf(k, -1.5707963705062866f, x);
+    r = fmaf(k, 4.3711390001862410e-8f, r);
+    float z = r * r;
+    float ps = fmaf(fmaf(fmaf(-1.9515295891e-4f, z, 8.3321608736e-3f), z, -1.6666654611e-1f), z * r, r);
+    float pc = fmaf(fmaf(fmaf(2.443315711809948e-5f, z, -1.388731625493765e-3f), z, 4.166664568298827e-2f), z * z, fmaf(-0.5f, z, 1.0f));
+    int q = (int)k;
+    float ss = (q & 1) ? pc : ps, cc = (q & 1) ? ps : pc;
+    *s = (q & 2) ? -ss : ss;
+    *c = ((q + 1) & 2) ? -cc : cc;
 }
 
-SX_DEV void es_prepare(Piece& p) {
-    if (p.zready) return;
-    float zx, zy;
-    es_integral(p.k0, p.k1, 1.0f, &zx, &zy);
+// int_{m-hd}^{m+hd} exp(i phi(u)) du by 3-point Gauss-Legendre (hd may be negative)
+SX_DEV void es_gl3(float a, float hk, float m, float hd, float* ix, float* iy) {
+    const float d = hd * 0.77459666924148338f;
+    const float u0 = m - d, u2 = m + d;
+    float s0, c0, s1, c1, s2, c2;
+    sx_sincos(u0 * fmaf(hk, u0, a), &s0, &c0);
+    sx_sincos(m * fmaf(hk, m, a), &s1, &c1);
+    sx_sincos(u2 * fmaf(hk, u2, a), &s2, &c2);
+    *ix = hd * fmaf(0.55555555555555556f, c0 + c2, 0.88888888888888889f * c1);
+    *iy = hd * fmaf(0.55555555555555556f, s0 + s2, 0.88888888888888889f * s1);
+}
+
+SX_DEV void es_prepare(const Piece& p, Spiral& sp) {
+    const float a = p.k0 - 0.5f * p.k1, hk = 0.5f * p.k1;
+    float zx = 0.0f, zy = 0.0f;
+    sp.zx[0] = 0.0f; sp.zy[0] = 0.0f;
+#pragma unroll 1
+    for (int k = 0; k < kAnchors; k++) {
+        float ix, iy;
+        es_gl3(a, hk, ((float)k + 0.5f) * (1.0f / kAnchors), 0.5f / kAnchors, &ix, &iy);
+        zx += ix; zy += iy;
+        sp.zx[k + 1] = zx; sp.zy[k + 1] = zy;
+    }
     float den = 1.0f / fmaf(zx, zx, zy * zy);
-    p.wr = zx * den;
-    p.wi = -zy * den;
-    p.zready = true;
+    sp.wr = zx * den;
+    sp.wi = -zy * den;
 }
 
 SX_DEV float es_phi(const Piece& p, float t) { return t * fmaf(0.5f * p.k1, t, p.k0 - 0.5f * p.k1); }
 // phi(tb) - phi(ta), evaluated as a difference (no cancellation)
 SX_DEV float es_dphi(const Piece& p, float ta, float tb) { return (tb - ta) * fmaf(0.5f * p.k1, ta + tb, p.k0 - 0.5f * p.k1); }
 
-// local position and unit tangent at piece fraction t (0 < t < 1): la + ch (x) Z(t)/Z(1) (L632)
-SX_DEV void es_eval(Piece& p, float t, V2* pos, V2* tan) {
-    es_prepare(p);
-    float zx, zy;
-    es_integral(p.k0, p.k1, t, &zx, &zy);
-    float wx = fmaf(zx, p.wr, -zy * p.wi), wy = fmaf(zx, p.wi, zy * p.wr);
+// local position and unit tangent at piece fraction t in [0,1]: la + ch (x) Z(t)/Z(1) (L632)
+SX_DEV void es_eval(const Piece& p, const Spiral& sp, float t, V2* pos, V2* tan) {
+    const float a = p.k0 - 0.5f * p.k1, hk = 0.5f * p.k1;
+    int k = (int)rintf(t * (float)kAnchors);
+    k = k < 0 ? 0 : (k > kAnchors ? kAnchors : k);
+    const float t0 = (float)k * (1.0f / kAnchors), hd = 0.5f * (t - t0);
+    float ix, iy;
+    es_gl3(a, hk, t0 + hd, hd, &ix, &iy);
+    const float zx = sp.zx[k] + ix, zy = sp.zy[k] + iy;
+    float wx = fmaf(zx, sp.wr, -zy * sp.wi), wy = fmaf(zx, sp.wi, zy * sp.wr);
     pos->x = fmaf(p.ch.x, wx, fmaf(-p.ch.y, wy, p.la.x));
     pos->y = fmaf(p.ch.x, wy, fmaf(p.ch.y, wx, p.la.y));
     float s, c;
-    sincosf(es_phi(p, t), &s, &c);
+    sx_sincos(es_phi(p, t), &s, &c);
     tan->x = fmaf(c, p.ua.x, -s * p.ua.y);
     tan->y = fmaf(s, p.ua.x, c * p.ua.y);
 }
@@ -113,9 +138,9 @@ SX_DEV V2 offset_point(V2 V, V2 u, float eta) { return v2(fmaf(eta, -u.y, V.x), 
 // At t = 0 and t = 1 the cubic's own point and tangent are used, so that adjacent pieces (and the join of the
 // next segment) share bits.  The spiral is evaluated unconditionally and the end-point cases are selected
 // afterwards, so that a warp evaluating a mix of interior and end vertices stays converged.
-SX_DEV V2 normal_point(Piece& p, float t, float r) {
+SX_DEV V2 normal_point(const Piece& p, const Spiral& sp, float t, float r) {
     V2 l, T;
-    es_eval(p, t, &l, &T);
+    es_eval(p, sp, t, &l, &T);
     const bool e0 = t == 0.0f, e1 = t == 1.0f;
     if (e0) { l = p.la; T = p.ua; }
     if (e1) { l = p.lb; T = p.ub; }
@@ -125,8 +150,8 @@ SX_DEV V2 normal_point(Piece& p, float t, float r) {
     if (e1 && p.at1) g = offset_point(p.P3, p.ub, r);
     return g;
 }
-SX_DEV V2 es_offset(Piece& p, float t, float eta) { return normal_point(p, t, eta); }
-SX_DEV V2 es_evolute(Piece& p, float t) { return normal_point(p, t, 1.0f / es_kappa(p, t)); }  // section 6
+SX_DEV V2 es_offset(const Piece& p, const Spiral& sp, float t, float eta) { return normal_point(p, sp, t, eta); }
+SX_DEV V2 es_evolute(const Piece& p, const Spiral& sp, float t) { return normal_point(p, sp, t, 1.0f / es_kappa(p, t)); }  // section 6
 
 // ---------------------------------------------------------------- subdivision plans
 struct OffPlan { int n; bool uniform; float ta, tb, ua, ub; };
@@ -220,30 +245,31 @@ SX_DEV SidePlan side_plan(const Piece& p, float eta, int mode, float tol_fl) {
     s.eta = eta; s.seg = 0u;
     float g0 = 1.0f - es_kappa(p, 0.0f) * eta, g1 = 1.0f - es_kappa(p, 1.0f) * eta;  // cusp0, cusp1 (L382-384)
     float tc = (g0 * g1 >= 0.0f) ? 1.0f : g0 / (g0 - g1);                            // L386
-    float ra[2], rb[2];
-    s.nr = 0;
-    s.sup[0] = s.sup[1] = false;
-    if (g0 >= 0.0f) { ra[s.nr] = 0.0f; rb[s.nr] = tc; s.sup[s.nr] = false; s.nr++; }
-    if (g0 < 0.0f || tc < 1.0f) {
-        if (g0 >= 0.0f) { ra[s.nr] = tc; rb[s.nr] = 1.0f; } else { ra[s.nr] = 0.0f; rb[s.nr] = tc; }
-        s.sup[s.nr] = true; s.nr++;
-    }
-    if (g0 < 0.0f && tc < 1.0f) { ra[s.nr] = tc; rb[s.nr] = 1.0f; s.sup[s.nr] = false; s.nr++; }
+    // g0 >= 0: regular on [0,tc], then super-critical on [tc,1] if there is a cusp; g0 < 0: super-critical on
+    // [0,tc], then regular on [tc,1] if there is a cusp (L388-411)
+    const bool first_sup = g0 < 0.0f;
+    s.nr = tc < 1.0f ? 2 : 1;
+    s.sup[0] = first_sup;
+    s.sup[1] = !first_sup;
     s.total = 0;
     s.cusp_a = s.cusp_b = false;
     s.evo.n = 0;
-#pragma unroll
-    for (int r = 0; r < 2; r++) {
-        if (r < s.nr) {
-            s.off[r] = offset_plan(p, eta, ra[r], rb[r], mode, tol_fl);
-            s.total += s.off[r].n;
-            if (s.sup[r]) {
-                s.cusp_a = (ra[r] != 0.0f);
-                s.cusp_b = (rb[r] != 1.0f);
-                s.evo = evolute_plan(p, ra[r], rb[r], tol_fl);
-                s.total += 2 * s.evo.n + (s.cusp_a ? 0 : 2) + (s.cusp_b ? 0 : 2);
-            }
-        }
+    s.off[0] = offset_plan(p, eta, 0.0f, tc, mode, tol_fl);
+    s.total += s.off[0].n;
+    float ea = 0.0f, eb = tc;
+    if (s.nr == 2) {
+        s.off[1] = offset_plan(p, eta, tc, 1.0f, mode, tol_fl);
+        s.total += s.off[1].n;
+        if (!first_sup) { ea = tc; eb = 1.0f; }
+    } else {
+        s.off[1] = s.off[0];
+        s.sup[1] = false;
+    }
+    if (first_sup || s.nr == 2) {
+        s.cusp_a = (ea != 0.0f);
+        s.cusp_b = (eb != 1.0f);
+        s.evo = evolute_plan(p, ea, eb, tol_fl);
+        s.total += 2 * s.evo.n + (s.cusp_a ? 0 : 2) + (s.cusp_b ? 0 : 2);
     }
     return s;
 }

@@ -40,7 +40,7 @@ struct SideSink {
 
 // ---------------------------------------------------------------- one side of one piece
 template <bool EMIT>
-SX_DEV uint32_t piece_side(Piece& p, float eta, bool mirror, const Params& P, const Writer* w, uint32_t first) {
+SX_DEV uint32_t piece_side(const Piece& p, const Spiral& z, float eta, bool mirror, const Params& P, const Writer* w, uint32_t first) {
     SidePlan s = side_plan(p, eta, P.mode, P.tol_fl);
     if (!EMIT) return (uint32_t)s.total;
     SideSink k;
@@ -51,23 +51,23 @@ SX_DEV uint32_t piece_side(Piece& p, float eta, bool mirror, const Params& P, co
         const OffPlan o = r == 0 ? s.off[0] : s.off[1];
         const bool sup = r == 0 ? s.sup[0] : s.sup[1];
         if (!sup) {
-            V2 prev = es_offset(p, o.ta, eta);
+            V2 prev = es_offset(p, z, o.ta, eta);
             float tp = o.ta;
             for (int i = 1; i <= o.n; i++) {
                 float t = i < o.n ? offset_t(p, o, eta, i) : o.tb;
-                V2 cur = es_offset(p, t, eta);
+                V2 cur = es_offset(p, z, t, eta);
                 k.put(idx++, prev, cur, arc ? es_dphi(p, tp, t) : 0.0f, kOffset);
                 prev = cur; tp = t;
             }
         } else {
             // evolute patch (section 6): the evolute meets the offset curve at the cusp
-            V2 Oa = es_offset(p, o.ta, eta), Ob = es_offset(p, o.tb, eta);
-            V2 Ea = s.cusp_a ? Oa : es_evolute(p, o.ta), Eb = s.cusp_b ? Ob : es_evolute(p, o.tb);
+            V2 Oa = es_offset(p, z, o.ta, eta), Ob = es_offset(p, z, o.tb, eta);
+            V2 Ea = s.cusp_a ? Oa : es_evolute(p, z, o.ta), Eb = s.cusp_b ? Ob : es_evolute(p, z, o.tb);
             if (!s.cusp_a) { k.put(idx, Oa, Ea, 0.0f, kConnector); k.put(idx + 1, Oa, Ea, 0.0f, kConnector); idx += 2; }  // "output twice", L197
             const int ne = s.evo.n;
             V2 pe = Ea;
             for (int i = 0; i < ne; i++) {
-                V2 b = (i == ne - 1) ? Eb : es_evolute(p, evolute_t(p, s.evo, i + 1));
+                V2 b = (i == ne - 1) ? Eb : es_evolute(p, z, evolute_t(p, s.evo, i + 1));
                 k.put(idx + i, pe, b, 0.0f, kEvolute);
                 k.put(idx + ne + i, pe, b, 0.0f, kEvolute);
                 pe = b;
@@ -77,7 +77,7 @@ SX_DEV uint32_t piece_side(Piece& p, float eta, bool mirror, const Params& P, co
             float tp = o.tb;
             for (int i = o.n - 1; i >= 0; i--) {
                 float t = i > 0 ? offset_t(p, o, eta, i) : o.ta;
-                V2 cur = i > 0 ? es_offset(p, t, eta) : Oa;
+                V2 cur = i > 0 ? es_offset(p, z, t, eta) : Oa;
                 k.put(idx++, prev, cur, arc ? es_dphi(p, tp, t) : 0.0f, kOffsetRev);
                 prev = cur; tp = t;
             }
@@ -235,9 +235,11 @@ SX_DEV uint32_t flatten_cubic(const Params& P, const Seg& s, float h, const Writ
     uint32_t n = 0;
     FitState f = fit_begin(s);
     Piece p;
+    Spiral z;
     while (fit_next(P, s, f, p)) {
-        n += piece_side<EMIT>(p, -h, false, P, w, n);  // -h side, forward
-        n += piece_side<EMIT>(p, h, true, P, w, n);    // +h side, mirrored
+        if (EMIT) es_prepare(p, z);
+        n += piece_side<EMIT>(p, z, -h, false, P, w, n);  // -h side, forward
+        n += piece_side<EMIT>(p, z, h, true, P, w, n);    // +h side, mirrored
     }
     return n;
 }
