@@ -51,83 +51,86 @@ SX_DEV void piece_load(const float4* slot, const PieceHead& hd, Piece& p, float*
     p.at0 = hd.at0; p.at1 = hd.at1;
 }
 
-// ---------------------------------------------------------------- record j (forward-t order) of one side
-// Same vertices, in the same order, as piece_side<true> (sx_segment.cuh) walks sequentially.  The record
-// index is first DECODED into two vertex specifications (cheap integer logic, where the threads of a warp
-// may diverge); the expensive part -- subdivision parameter, Euler-spiral integral, normal offset -- then
-// runs once per end point in a single code path that every thread of the warp executes together.
-struct VertexSpec {
-    float t;      // parameter when src == 0
-    int i;        // subdivision index when src != 0
-    int src;      // 0: t given, 1: offset_t(i), 2: evolute_t(i)
-    bool evo;     // point on the evolute (r = 1/kappa) instead of the parallel curve (r = eta)
+// ---------------------------------------------------------------- parts
+// The records of one side of one piece, in OUTPUT order, are a short list of PARTS (at most 8): chains of n
+// records over n+1 vertices.  Vertex m of a part is either one of the part's two END vertices -- a piece end
+// (t = 0 or t = 1, on the parallel curve or on the evolute) or the side's cusp point -- or the interior
+// subdivision vertex of index i0 +- m of an offset range (sections 4, 5) or of the evolute (section 6).  This
+// is piece_side<true> (sx_segment.cuh) turned into data: the writer's threads do not branch on what kind of
+// record they own.  The mirror image of the +h side (reverse order, end points swapped) is folded into the
+// table when it is built.
+enum : uint32_t { kEndT0 = 0u, kEndT1 = 1u, kEndCusp = 2u, kEndEvo = 4u };  // end-vertex code: which point | evolute flag
+struct __align__(8) Part {
+    uint64_t base;   // output index of the part's first record
+    uint32_t n;      // records
+    int32_t i0;      // vertex m has subdivision index i0 + dir * m
+    uint32_t info;   // 0-6 side slot, 7 dir < 0, 8-9 src (0 none, 1 offset range, 2 evolute), 10 range, 11 arc angle wanted,
+                     // 12-15 record kind, 16-18 end code of vertex 0, 19-21 end code of vertex n
+    uint32_t pad;
 };
-SX_DEV VertexSpec vs_fixed(float t, bool evo) { VertexSpec v; v.t = t; v.i = 0; v.src = 0; v.evo = evo; return v; }
-SX_DEV VertexSpec vs_offset(const OffPlan& o, uint32_t i) {
-    VertexSpec v; v.evo = false; v.i = (int)i; v.t = i == 0u ? o.ta : o.tb; v.src = (i == 0u || i == (uint32_t)o.n) ? 0 : 1; return v;
-}
-SX_DEV VertexSpec vs_evolute(const SidePlan& s, const OffPlan& o, uint32_t i) {
-    const uint32_t ne = (uint32_t)s.evo.n;
-    if (i == 0u) return vs_fixed(o.ta, !s.cusp_a);   // the evolute meets the offset curve at the cusp
-    if (i == ne) return vs_fixed(o.tb, !s.cusp_b);
-    VertexSpec v; v.evo = true; v.i = (int)i; v.t = 0.0f; v.src = 2; return v;
+SX_DEV uint32_t end_code(float t) { return t == 0.0f ? kEndT0 : (t == 1.0f ? kEndT1 : kEndCusp); }
+
+// number of parts of a side
+SX_DEV uint32_t side_part_count(const SidePlan& s) {
+    uint32_t c = (uint32_t)s.nr;  // one offset part per range
+    if (s.sup[0] || (s.nr == 2 && s.sup[1])) c += 2u + (s.cusp_a ? 0u : 2u) + (s.cusp_b ? 0u : 2u);
+    return c;
 }
 
-SX_DEV void side_record(const Piece& p, const Spiral& z, const SidePlan& s, float eta, bool arc, uint32_t j, V2* a, V2* b, float* angle, uint32_t* kind) {
-    VertexSpec va = vs_fixed(0.0f, false), vb = va;
-    OffPlan o = s.off[0];
-    bool want_angle = false;
-    *kind = kOffset;
+// writes the parts of a side (output order) to dst[0..count), and their tile-relative record prefixes to pref[]
+SX_DEV void side_parts(const SidePlan& s, uint32_t side_slot, bool mirror, bool arc, uint64_t side_base, uint32_t tile_prefix,
+                       uint32_t count, Part* dst, uint32_t* pref) {
+    uint32_t idx = 0, fwd = 0;  // forward part index, records before the part in forward order
+    const uint32_t total = (uint32_t)s.total;
+    auto push = [&](uint32_t n, int32_t i0, bool dirneg, uint32_t src, uint32_t ri, bool angle, uint32_t kind, uint32_t f0, uint32_t f1) {
+        Part q;
+        uint32_t pos = idx, before = fwd;
+        if (mirror) {  // reverse the list, reverse each chain
+            pos = count - 1u - idx; before = total - fwd - n;
+            i0 = dirneg ? i0 - (int32_t)n : i0 + (int32_t)n; dirneg = !dirneg;
+            uint32_t t = f0; f0 = f1; f1 = t;
+            kind |= kPlus;
+        }
+        q.base = side_base + before; q.n = n; q.i0 = i0; q.pad = 0u;
+        q.info = side_slot | (dirneg ? 128u : 0u) | (src << 8) | (ri << 10) | ((angle && arc) ? 2048u : 0u) | (kind << 12) | (f0 << 16) | (f1 << 19);
+        dst[pos] = q;
+        pref[pos] = tile_prefix + before;
+        idx++; fwd += n;
+    };
 #pragma unroll
     for (int r = 0; r < 2; r++) {
         if (r >= s.nr) break;
-        const OffPlan oo = r == 0 ? s.off[0] : s.off[1];
+        const OffPlan o = r == 0 ? s.off[0] : s.off[1];
         const bool sup = r == 0 ? s.sup[0] : s.sup[1];
-        const uint32_t n = (uint32_t)oo.n;
+        const uint32_t ca = end_code(o.ta), cb = end_code(o.tb);
         if (!sup) {
-            if (j < n) {
-                o = oo; va = vs_offset(oo, j); vb = vs_offset(oo, j + 1u); want_angle = arc; *kind = kOffset;
-                break;
-            }
-            j -= n;
+            push((uint32_t)o.n, 0, false, 1u, (uint32_t)r, true, kOffset, ca, cb);
         } else {
-            // evolute patch (section 6): connectors x2, evolute x2, reversed offset, connectors x2
-            const uint32_t nca = s.cusp_a ? 0u : 2u, ncb = s.cusp_b ? 0u : 2u, ne = (uint32_t)s.evo.n;
-            const uint32_t tot = nca + 2u * ne + n + ncb;
-            if (j < tot) {
-                o = oo;
-                if (j < nca) {
-                    va = vs_fixed(oo.ta, false); vb = vs_fixed(oo.ta, true); *kind = kConnector;
-                } else if (j < nca + 2u * ne) {
-                    uint32_t i = j - nca;
-                    if (i >= ne) i -= ne;
-                    va = vs_evolute(s, oo, i); vb = vs_evolute(s, oo, i + 1u); *kind = kEvolute;
-                } else if (j < nca + 2u * ne + n) {
-                    uint32_t hi = n - (j - (nca + 2u * ne));  // reversed offset (L403, L191): vertex hi -> vertex hi-1
-                    va = vs_offset(oo, hi); vb = vs_offset(oo, hi - 1u); want_angle = arc; *kind = kOffsetRev;
-                } else {
-                    va = vs_fixed(oo.tb, true); vb = vs_fixed(oo.tb, false); *kind = kConnector;
-                }
-                break;
-            }
-            j -= tot;
+            // evolute patch (section 6): connectors x2, evolute x2, reversed offset, connectors x2;
+            // the evolute meets the offset curve at the cusp
+            const uint32_t ea = s.cusp_a ? (uint32_t)kEndCusp : (ca | kEndEvo), eb = s.cusp_b ? (uint32_t)kEndCusp : (cb | kEndEvo);
+            if (!s.cusp_a) { push(1u, 0, false, 0u, 0u, false, kConnector, ca, ea); push(1u, 0, false, 0u, 0u, false, kConnector, ca, ea); }
+            push((uint32_t)s.evo.n, 0, false, 2u, 0u, false, kEvolute, ea, eb);
+            push((uint32_t)s.evo.n, 0, false, 2u, 0u, false, kEvolute, ea, eb);
+            push((uint32_t)o.n, o.n, true, 1u, (uint32_t)r, true, kOffsetRev, cb, ca);  // L403, L191
+            if (!s.cusp_b) { push(1u, 0, false, 0u, 0u, false, kConnector, eb, cb); push(1u, 0, false, 0u, 0u, false, kConnector, eb, cb); }
         }
     }
-    // ---- the convergent part
-    float t0 = 0.0f, t1 = 0.0f;
-    V2 p0 = v2(0.0f, 0.0f), p1 = p0;
-#pragma unroll 1
-    for (int e = 0; e < 2; e++) {
-        const VertexSpec v = e == 0 ? va : vb;
-        float t = v.t;
-        if (v.src == 1) t = offset_t(p, o, eta, v.i);
-        else if (v.src == 2) t = evolute_t(p, s.evo, v.i);
-        const float r = v.evo ? 1.0f / es_kappa(p, t) : eta;
-        const V2 g = normal_point(p, z, t, r);
-        if (e == 0) { t0 = t; p0 = g; } else { t1 = t; p1 = g; }
-    }
-    *a = p0; *b = p1;
-    *angle = want_angle ? es_dphi(p, t0, t1) : 0.0f;
+}
+
+// an END vertex of a part: same arithmetic as normal_point at t = 0 / t = 1; the cusp point is evaluated once per
+// side (normal_point at the cusp parameter) and shared by the parts that meet there
+SX_DEV V2 end_vertex(const Piece& p, uint32_t code, float eta, float4 cusp, float* t_out) {
+    const uint32_t which = code & 3u;
+    const bool e1 = which == kEndT1;
+    const float t = e1 ? 1.0f : 0.0f;
+    const V2 l = e1 ? p.lb : p.la, T = e1 ? p.ub : p.ua;
+    const float r = (code & kEndEvo) ? 1.0f / es_kappa(p, t) : eta;
+    V2 g = v2(p.base.x + fmaf(r, -T.y, l.x), p.base.y + fmaf(r, T.x, l.y));
+    if (e1 ? p.at1 : p.at0) g = offset_point(e1 ? p.P3 : p.base, T, r);
+    *t_out = t;
+    if (which == kEndCusp) { g = v2(cusp.x, cusp.y); *t_out = cusp.z; }
+    return g;
 }
 
 }  // namespace sx

@@ -15,9 +15,9 @@
 namespace sx {
 
 constexpr int kSegThreads = 128;
-constexpr int kWpThreads = 256;            // write kernel: threads per block = piece sides per tile
-constexpr int kWpPieces = kWpThreads / 2;  // descriptors per tile
-constexpr int kWpBlocksPerSM = 4;
+constexpr int kWpThreads = 256;            // write kernel: threads per block
+constexpr int kWpPieces = 64;              // descriptors per tile
+constexpr int kWpBlocksPerSM = 3;
 
 // (b) count pass.  One thread per input segment runs Alg. 2 without the writes; every accepted piece is
 // stored in the piece cache.  The loop is warp-synchronous at piece granularity: each round every lane
@@ -80,84 +80,161 @@ k_count(Params P, uint32_t* __restrict__ seg_count, float4* __restrict__ pieces,
     if (i < P.n_tags) seg_count[i] = n + n_tail;
 }
 
-// (d1) write pass over the piece cache: one thread per output record.
+// (d1) write pass over the piece cache: one thread per output record, no per-record branching.
+// A block stages a tile of kWpPieces descriptors.  Phase 1: warps 0-3, one thread per (piece, side), rebuild the
+// side plans (same device function as the count kernel, hence the same counts) while warps 4-7, one thread per
+// (piece, half), integrate the anchor table of the Euler spiral.  Phase 2: the side threads scan (parts, records),
+// evaluate the side's cusp point and write the PART table (sx_cache.cuh).  Phase 3: a warp takes 31 consecutive
+// records of the tile per iteration; lane k evaluates the START vertex of record k (lane 31 that of the next
+// record, for lane 30), the END vertex comes from the next lane by shuffle, or is a part end (no integral).
+// Records go out as 16-byte (line) or 2 x 16-byte (arc) stores to consecutive addresses.
+constexpr int kWpSides = 2 * kWpPieces;
+constexpr int kWpMaxParts = 8 * kWpSides;
+struct WpTile {
+    Piece piece[kWpPieces];
+    Spiral spiral[kWpPieces];
+    SidePlan plan[kWpSides];
+    float4 cusp[kWpSides];          // x, y, t of the side's cusp vertex
+    Part part[kWpMaxParts];
+    uint32_t ppref[kWpMaxParts + 1];
+    uint32_t wtot[kWpSides / 32][2];
+};
+
 __global__ void __launch_bounds__(kWpThreads, kWpBlocksPerSM)
 k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, const uint32_t* __restrict__ piece_ctr,
                const uint64_t* __restrict__ seg_off, float4* __restrict__ out, uint64_t cap_records, uint32_t* err) {
-    __shared__ Piece s_piece[kWpPieces];
-    __shared__ Spiral s_spiral[kWpPieces];
-    __shared__ SidePlan s_plan[kWpThreads];
-    __shared__ uint64_t s_base[kWpThreads];
-    __shared__ uint32_t s_pref[kWpThreads + 1];
-    __shared__ uint32_t s_warp[kWpThreads / 32];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    WpTile& S = *reinterpret_cast<WpTile*>(smem_raw);
     const uint32_t reserved = *piece_ctr;
-    if (reserved > piece_cap) return;  // cache overflow: k_write_segments takes the whole call
+    if (reserved > piece_cap) return;  // cache overflow: k_write_fallback takes the whole call
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool arc = P.mode == kModeArc;
     for (uint32_t tile = blockIdx.x; (uint64_t)tile * kWpPieces < reserved; tile += gridDim.x) {
-        // ---- stage: thread = (piece, side); rebuild the side plan, Z(1) once per piece
-        const uint32_t slot = tile * (uint32_t)kWpPieces + (uint32_t)(tid >> 1);
-        const int side = tid & 1;
-        uint32_t tot = 0;
+        // ---- phase 1
+        const int sub = tid & (kWpSides - 1);                       // (piece, side) or (piece, half)
+        const uint32_t slot = tile * (uint32_t)kWpPieces + (uint32_t)(sub >> 1);
+        const int side = sub & 1;
+        Piece p;
+        p.k0 = 0.0f; p.k1 = 0.0f;
+        float h = 0.0f;
+        PieceHead hd;
+        hd.seg = kInvalidSeg;
         if (slot < reserved) {
             const float4* d = pieces + (uint64_t)slot * kDescQuads;
-            PieceHead hd = piece_head(d);
-            if (hd.seg != kInvalidSeg) {
-                Piece p;
-                float h;
-                piece_load(d, hd, p, &h);
+            hd = piece_head(d);
+            if (hd.seg != kInvalidSeg) piece_load(d, hd, p, &h);
+        }
+        const bool live = hd.seg != kInvalidSeg;
+        uint32_t nparts = 0, nrec = 0;
+        uint64_t base = 0;
+        if (tid < kWpSides) {
+            if (live) {
                 SidePlan sp = side_plan(p, side ? h : -h, P.mode, P.tol_fl);
-                tot = (uint32_t)sp.total;
+                nrec = (uint32_t)sp.total;
+                base = seg_off[hd.seg] + hd.rel + (side ? hd.n_minus : 0u);
+                if (base + nrec > cap_records) { atomicOr(err, kErrCapacity); nrec = 0; }
+                else nparts = side_part_count(sp);
                 sp.seg = hd.seg;
-                uint64_t base = seg_off[hd.seg] + hd.rel + (side ? hd.n_minus : 0u);
-                if (base + tot > cap_records) { atomicOr(err, kErrCapacity); tot = 0; }
-                s_plan[tid] = sp;
-                s_base[tid] = base;
-                if (side == 0) { es_prepare(p, s_spiral[tid >> 1]); s_piece[tid >> 1] = p; }
+                S.plan[sub] = sp;
+                if (side == 0) S.piece[sub >> 1] = p;
+            }
+        } else {
+            // anchor table: each of the two threads of a piece integrates one half, then they exchange totals
+            float hx[kAnchors / 2], hy[kAnchors / 2];
+            es_anchor_half(p, side, hx, hy);
+            const float ox = __shfl_xor_sync(0xffffffffu, hx[kAnchors / 2 - 1], 1), oy = __shfl_xor_sync(0xffffffffu, hy[kAnchors / 2 - 1], 1);
+            if (live) {
+                Spiral& z = S.spiral[sub >> 1];
+                const float bx = side ? ox : 0.0f, by = side ? oy : 0.0f;
+#pragma unroll
+                for (int k = 0; k < kAnchors / 2; k++) { z.zx[side * (kAnchors / 2) + k + 1] = bx + hx[k]; z.zy[side * (kAnchors / 2) + k + 1] = by + hy[k]; }
+                if (side == 0) {
+                    z.zx[0] = 0.0f; z.zy[0] = 0.0f;
+                    const float zx = hx[kAnchors / 2 - 1] + ox, zy = hy[kAnchors / 2 - 1] + oy;  // Z(1)
+                    const float den = 1.0f / fmaf(zx, zx, zy * zy);
+                    z.wr = zx * den; z.wi = -zy * den;
+                }
             }
         }
-        // ---- block exclusive scan of the side totals
-        uint32_t incl = tot;
+        // ---- phase 2: scan (parts, records) over the side threads, then the part table
+        uint32_t ip = nparts, ir = nrec;
+        if (tid < kWpSides) {
 #pragma unroll
-        for (int dd = 1; dd < 32; dd <<= 1) {
-            uint32_t o = __shfl_up_sync(0xffffffffu, incl, dd);
-            if (lane >= dd) incl += o;
-        }
-        if (lane == 31) s_warp[warp] = incl;
-        __syncthreads();
-        uint32_t wex = 0, total = 0;
-#pragma unroll
-        for (int k = 0; k < kWpThreads / 32; k++) {
-            if (k == warp) wex = total;
-            total += s_warp[k];
-        }
-        s_pref[tid] = wex + incl - tot;
-        if (tid == 0) s_pref[kWpThreads] = total;
-        __syncthreads();
-        // ---- one thread per record
-        for (uint32_t r = (uint32_t)tid; r < total; r += (uint32_t)kWpThreads) {
-            int lo = 0, hi = kWpThreads;  // largest k with s_pref[k] <= r
-#pragma unroll
-            for (int step = 0; step < 8; step++) {
-                int mid = (lo + hi) >> 1;
-                if (s_pref[mid] <= r) lo = mid; else hi = mid;
+            for (int dd = 1; dd < 32; dd <<= 1) {
+                uint32_t a = __shfl_up_sync(0xffffffffu, ip, dd), b = __shfl_up_sync(0xffffffffu, ir, dd);
+                if (lane >= dd) { ip += a; ir += b; }
             }
-            const int k = lo;
-            const SidePlan& sp = s_plan[k];
-            Piece p = s_piece[k >> 1];
-            const bool mirror = (k & 1) != 0;
-            const uint32_t j = r - s_pref[k], nside = (uint32_t)sp.total;
-            V2 a, b;
-            float ang;
-            uint32_t kind;
-            side_record(p, s_spiral[k >> 1], sp, sp.eta, arc, mirror ? nside - 1u - j : j, &a, &b, &ang, &kind);
-            const uint64_t rec = s_base[k] + j;
-            if (mirror) { V2 t = a; a = b; b = t; ang = -ang; kind |= kPlus; }
-            if (!arc) {
-                out[rec] = make_float4(a.x, a.y, b.x, b.y);
-            } else {
-                out[2 * rec] = make_float4(a.x, a.y, b.x, b.y);
-                out[2 * rec + 1] = make_float4(ang, f_of_u(sp.seg), f_of_u(kind), 0.0f);
+            if (lane == 31) { S.wtot[warp][0] = ip; S.wtot[warp][1] = ir; }
+        }
+        __syncthreads();
+        uint32_t tparts = 0, trecs = 0;
+        {
+            uint32_t ep = 0, er = 0;
+#pragma unroll
+            for (int k = 0; k < kWpSides / 32; k++) {
+                if (k == warp) { ep = tparts; er = trecs; }
+                tparts += S.wtot[k][0]; trecs += S.wtot[k][1];
+            }
+            if (tid < kWpSides && nparts) {
+                const SidePlan& sp = S.plan[sub];
+                const float eta = side ? h : -h;
+                // the side's cusp vertex: the parallel curve at the cusp parameter (L380-386), evaluated once
+                const float tc = sp.nr == 2 ? sp.off[0].tb : (sp.cusp_b ? sp.off[0].tb : 0.0f);
+                if (tc != 0.0f && tc != 1.0f) {
+                    V2 c = normal_point(p, S.spiral[sub >> 1], tc, eta);
+                    S.cusp[sub] = make_float4(c.x, c.y, tc, 0.0f);
+                }
+                side_parts(sp, (uint32_t)sub, side != 0, arc, base, er + ir - nrec, nparts, &S.part[ep + ip - nparts], &S.ppref[ep + ip - nparts]);
+            }
+            if (tid == 0) S.ppref[tparts] = trecs;
+        }
+        __syncthreads();
+        // ---- phase 3: one thread per record (31 records + 1 look-ahead vertex per warp iteration)
+        for (uint32_t q = (uint32_t)warp; q * 31u < trecs; q += (uint32_t)(kWpThreads / 32)) {
+            const uint32_t r = q * 31u + (uint32_t)lane;
+            const bool act = r < trecs;
+            V2 A = v2(0.0f, 0.0f), B = A;
+            float tA = 0.0f, tB = 0.0f;
+            bool last = true, want_angle = false;
+            uint64_t rec = 0;
+            uint32_t kind = 0, sg = 0;
+            const Piece* pp = &S.piece[0];
+            if (act) {
+                uint32_t lo = 0, hi = tparts;  // largest part with ppref <= r
+#pragma unroll 1
+                while (hi - lo > 1u) {
+                    uint32_t mid = (lo + hi) >> 1;
+                    if (S.ppref[mid] <= r) lo = mid; else hi = mid;
+                }
+                const Part pt = S.part[lo];
+                const uint32_t m = r - S.ppref[lo];
+                const uint32_t ss = pt.info & 127u;
+                pp = &S.piece[ss >> 1];
+                const SidePlan& sp = S.plan[ss];
+                const float eta = sp.eta;
+                const float4 cusp = S.cusp[ss];
+                rec = pt.base + m; kind = (pt.info >> 12) & 15u; sg = sp.seg; want_angle = (pt.info & 2048u) != 0u;
+                last = m + 1u == pt.n;
+                if (m == 0u) {
+                    A = end_vertex(*pp, (pt.info >> 16) & 7u, eta, cusp, &tA);
+                } else {
+                    const int idx = (pt.info & 128u) ? pt.i0 - (int)m : pt.i0 + (int)m;
+                    const bool evo = ((pt.info >> 8) & 3u) == 2u;
+                    tA = evo ? evolute_t(*pp, sp.evo, idx) : offset_t(*pp, (pt.info & 1024u) ? sp.off[1] : sp.off[0], eta, idx);
+                    A = normal_point(*pp, S.spiral[ss >> 1], tA, evo ? 1.0f / es_kappa(*pp, tA) : eta);
+                }
+                if (last) B = end_vertex(*pp, (pt.info >> 19) & 7u, eta, cusp, &tB);
+            }
+            const float nx = __shfl_down_sync(0xffffffffu, A.x, 1), ny = __shfl_down_sync(0xffffffffu, A.y, 1), nt = __shfl_down_sync(0xffffffffu, tA, 1);
+            if (!last) { B = v2(nx, ny); tB = nt; }
+            if (act && lane < 31) {
+                if (!arc) {
+                    out[rec] = make_float4(A.x, A.y, B.x, B.y);
+                } else {
+                    out[2 * rec] = make_float4(A.x, A.y, B.x, B.y);
+                    out[2 * rec + 1] = make_float4(want_angle ? es_dphi(*pp, tA, tB) + 0.0f : 0.0f,  // + 0: no negative zero
+                                                 f_of_u(sg), f_of_u(kind), 0.0f);
+                }
             }
         }
         __syncthreads();
@@ -306,6 +383,8 @@ sx_status sx_create(sx_ctx** out, int32_t device) {
     if (c->sm_count <= 0) c->sm_count = 148;
     cudaError_t e = cudaMallocHost(reinterpret_cast<void**>(&c->h_pinned), 64);
     if (e != cudaSuccess) { g_last_cuda = e; free(c); return SX_E_CUDA; }
+    e = cudaFuncSetAttribute(sx::k_write_pieces, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(sx::WpTile));
+    if (e != cudaSuccess) { g_last_cuda = e; cudaFreeHost(c->h_pinned); free(c); return SX_E_CUDA; }
     *out = c;
     return SX_OK;
 }
@@ -414,7 +493,7 @@ sx_status sx_write(sx_ctx* c, void* d_out_records, uint64_t cap_records, void* c
     SX_CUDA(cudaSetDevice(c->device));
     uint32_t n = c->P.n_tags;
     float4* out = static_cast<float4*>(d_out_records);
-    sx::k_write_pieces<<<c->sm_count * sx::kWpBlocksPerSM, sx::kWpThreads, 0, s>>>(c->P, c->pieces, (uint32_t)c->piece_cap, ctx_piece_ctr(c), c->seg_off,
+    sx::k_write_pieces<<<c->sm_count * sx::kWpBlocksPerSM, sx::kWpThreads, sizeof(sx::WpTile), s>>>(c->P, c->pieces, (uint32_t)c->piece_cap, ctx_piece_ctr(c), c->seg_off,
                                                                                  out, cap_records, ctx_err(c));
     sx::k_write_segments<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(c->P, c->seg_count, c->seg_off, out, cap_records,
                                                                                                (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_err(c));

@@ -47,6 +47,32 @@ SX_DEV V2 operator-(V2 a, V2 b) { return v2(a.x - b.x, a.y - b.y); }
 SX_DEV float dot(V2 a, V2 b) { return a.x * b.x + a.y * b.y; }
 SX_DEV float cross(V2 a, V2 b) { return a.x * b.y - a.y * b.x; }
 SX_DEV float len2(V2 a) { return a.x * a.x + a.y * a.y; }
+// Two grades of arithmetic.  Plain operators, sqrtf, sinf, asinf ... are IEEE / CUDA's
+// accurate library versions (no -use_fast_math): used for everything a coordinate or a subdivision parameter is
+// computed from.  The *_fast helpers below (MUFU approximations, ~2 ulp) are used where a value only feeds a
+// tolerance comparison or a ceil(): the cubic -> spiral error estimate and the subdivision-count formulas.
+SX_DEV float div_fast(float a, float b) { return __fdividef(a, b); }
+SX_DEV float sqrt_fast(float a) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
+SX_DEV float cbrt_fast(float a) { return a > 0.0f ? __powf(a, 0.33333333333333333f) : 0.0f; }
+// atan2 for the end-tangent angles of a piece: one approximate division, odd minimax polynomial on [0,1]
+// (max error ~1e-7 rad), quadrant fix-up by selects
+SX_DEV float atan2_fast(float y, float x) {
+    const float ax = fabsf(x), ay = fabsf(y);
+    const float mx = fmaxf(ax, ay), mn = fminf(ax, ay);
+    const float a = mx > 0.0f ? __fdividef(mn, mx) : 0.0f;
+    const float s = a * a;
+    float r = fmaf(s, 0.00282363896258175373077393f, -0.0159569028764963150024414f);
+    r = fmaf(r, s, 0.0425049886107444763183594f);
+    r = fmaf(r, s, -0.0748900920152664184570312f);
+    r = fmaf(r, s, 0.106347933411598205566406f);
+    r = fmaf(r, s, -0.142027363181114196777344f);
+    r = fmaf(r, s, 0.199926957488059997558594f);
+    r = fmaf(r, s, -0.333331018686294555664062f);
+    r = fmaf(r * s, a, a);
+    if (ay > ax) r = 1.57079637050628662109375f - r;
+    if (x < 0.0f) r = 3.14159274101257324218750f - r;
+    return y < 0.0f ? -r : r;
+}
 SX_DEV V2 unit(V2 a) { float l = sqrtf(len2(a)); return v2(a.x / l, a.y / l); }
 
 #ifdef __CUDA_ARCH__
@@ -189,12 +215,12 @@ SX_DEV float fit_error(V2 u0, V2 u1, float q0mag, float q1mag, V2 ch, float dt, 
     V2 uc = v2(ch.x / chord, ch.y / chord);
     float s0 = cross(u0, uc), c0 = dot(u0, uc);
     float s1 = cross(uc, u1), c1 = dot(uc, u1);
-    float th0 = atan2f(s0, c0), th1 = atan2f(s1, c1);
+    float th0 = atan2f(s0, c0), th1 = atan2f(s1, c1);  // accurate: the angles fix k0, k1 and hence every subdivision parameter
     *th0_out = th0;
     *th1_out = th1;
     if (c0 < -0.5f || c1 < -0.5f) return 2.0f * chord;
-    float d0 = q0mag * dt / chord, d1 = q1mag * dt / chord;
-    float db0 = 2.0f / (3.0f * (1.0f + c0)), db1 = 2.0f / (3.0f * (1.0f + c1));
+    float d0 = div_fast(q0mag * dt, chord), d1 = div_fast(q1mag * dt, chord);
+    float db0 = div_fast(2.0f, 3.0f * (1.0f + c0)), db1 = div_fast(2.0f, 3.0f * (1.0f + c1));
     float s01 = s0 * c1 + c0 * s1;
     float area = 0.15f * (2.0f * d0 * s0 + 2.0f * d1 * s1 - d0 * d1 * s01);
     float areb = 0.15f * (2.0f * db0 * s0 + 2.0f * db1 * s1 - db0 * db1 * s01);
@@ -203,7 +229,7 @@ SX_DEV float fit_error(V2 u0, V2 u1, float q0mag, float q1mag, V2 ch, float dt, 
     float e1 = 4.6255e-6f * k2 * k2 * ksum + 7.5e-3f * k2 * kdif;
     float e2 = 1.55f * fabsf(area - areb);
     float dd0 = db0 - d0, dd1 = db1 - d1;
-    float e3 = (0.005f * ksum + 0.07f * kdif) * sqrtf(dd0 * dd0 + dd1 * dd1);
+    float e3 = (0.005f * ksum + 0.07f * kdif) * sqrt_fast(dd0 * dd0 + dd1 * dd1);
     return chord * (e1 + e2 + e3);
 }
 
@@ -214,23 +240,23 @@ SX_DEV void ghi(float th0, float th1, float* k1_out, float* c_out) {
     float k2 = k * k, k4 = k2 * k2, k6 = k4 * k2;
     float D2 = D * D, D3 = D2 * D, D4 = D2 * D2, D5 = D4 * D, D6 = D4 * D2, D7 = D6 * D;
     float k1 = 6.0f * D;
-    k1 -= D3 / 70.0f;
-    k1 -= D5 / 10780.0f;
+    k1 -= D3 * (1.0f / 70.0f);
+    k1 -= D5 * (1.0f / 10780.0f);
     k1 += D7 * 2.769178184818219e-7f;
-    k1 -= k2 * D / 10.0f;
-    k1 += k2 * D3 / 4200.0f;
+    k1 -= k2 * D * (1.0f / 10.0f);
+    k1 += k2 * D3 * (1.0f / 4200.0f);
     k1 += k2 * D5 * 1.6959677820260655e-5f;
-    k1 -= k4 * D / 1400.0f;
+    k1 -= k4 * D * (1.0f / 1400.0f);
     k1 += k4 * D3 * 6.84915970574303e-5f;
     k1 -= k6 * D * 7.936475029053326e-6f;
     float c = 1.0f;
-    c -= D2 / 40.0f;
+    c -= D2 * (1.0f / 40.0f);
     c += D4 * 0.00034226190482569864f;
     c -= D6 * 1.9349474568904524e-6f;
-    c -= k2 / 24.0f;
+    c -= k2 * (1.0f / 24.0f);
     c += k2 * D2 * 0.0024702380951963226f;
     c -= k2 * D4 * 3.7297408997537985e-5f;
-    c += k4 / 1920.0f;
+    c += k4 * (1.0f / 1920.0f);
     c -= k4 * D2 * 4.87350869747975e-5f;
     c -= k6 * 3.1001936068463107e-6f;
     *k1_out = k1;

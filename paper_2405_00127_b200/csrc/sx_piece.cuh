@@ -9,6 +9,9 @@
 namespace sx {
 
 // ---------------------------------------------------------------- section 4.2: f_approx and its inverse
+// This is the PARAMETER path (curvature -> x -> u -> t): IEEE division / square root and CUDA's accurate sinf, asinf,
+// cbrtf, because t is ill-conditioned in x on nearly circular pieces (dt/dx = L / (2 eta k1)): one ulp in f_approx
+// moves a vertex by up to ~5e-4 px along the curve, and the oracle evaluates this path in fp32 too.
 // f_approx (L149), odd extension (L157), middle piece sign-preserving (R-3b)
 SX_DEV float f_approx(float x) {
     float a = fabsf(x), r;
@@ -51,7 +54,7 @@ SX_DEV void piece_params(Piece& p, float th0, float th1, float chord) {
     if (!(p.L > 1e-12f)) p.L = 1e-12f;
 }
 
-SX_DEV float es_kappa(const Piece& p, float t) { return (p.k0 + p.k1 * (t - 0.5f)) / p.L; }
+SX_DEV float es_kappa(const Piece& p, float t) { return (p.k0 + p.k1 * (t - 0.5f)) / (p.L); }
 
 // ---------------------------------------------------------------- Euler-spiral integral (R-2)
 // Z(t) = int_0^t exp(i phi(u)) du, phi(u) = (k0-k1/2) u + k1 u^2/2.  Evaluated from a per-piece table of
@@ -93,18 +96,32 @@ SX_DEV void es_gl3(float a, float hk, float m, float hd, float* ix, float* iy) {
     *iy = hd * fmaf(0.55555555555555556f, s0 + s2, 0.88888888888888889f * s1);
 }
 
-SX_DEV void es_prepare(const Piece& p, Spiral& sp) {
+// one half (0: [0,1/2], 1: [1/2,1]) of the anchor table: cumulative sums of the half's sub-integrals, relative to
+// the half's start.  es_prepare = both halves by one thread; the write kernel gives one half to each side thread.
+SX_DEV void es_anchor_half(const Piece& p, int half, float* hx, float* hy) {
     const float a = p.k0 - 0.5f * p.k1, hk = 0.5f * p.k1;
     float zx = 0.0f, zy = 0.0f;
-    sp.zx[0] = 0.0f; sp.zy[0] = 0.0f;
-#pragma unroll 1
-    for (int k = 0; k < kAnchors; k++) {
+#pragma unroll
+    for (int k = 0; k < kAnchors / 2; k++) {
         float ix, iy;
-        es_gl3(a, hk, ((float)k + 0.5f) * (1.0f / kAnchors), 0.5f / kAnchors, &ix, &iy);
+        es_gl3(a, hk, ((float)(half * (kAnchors / 2) + k) + 0.5f) * (1.0f / kAnchors), 0.5f / kAnchors, &ix, &iy);
         zx += ix; zy += iy;
-        sp.zx[k + 1] = zx; sp.zy[k + 1] = zy;
+        hx[k] = zx; hy[k] = zy;
     }
-    float den = 1.0f / fmaf(zx, zx, zy * zy);
+}
+
+SX_DEV void es_prepare(const Piece& p, Spiral& sp) {
+    float ax[kAnchors / 2], ay[kAnchors / 2], bx[kAnchors / 2], by[kAnchors / 2];
+    es_anchor_half(p, 0, ax, ay);
+    es_anchor_half(p, 1, bx, by);
+    sp.zx[0] = 0.0f; sp.zy[0] = 0.0f;
+#pragma unroll
+    for (int k = 0; k < kAnchors / 2; k++) {
+        sp.zx[k + 1] = ax[k]; sp.zy[k + 1] = ay[k];
+        sp.zx[kAnchors / 2 + k + 1] = ax[kAnchors / 2 - 1] + bx[k]; sp.zy[kAnchors / 2 + k + 1] = ay[kAnchors / 2 - 1] + by[k];
+    }
+    const float zx = ax[kAnchors / 2 - 1] + bx[kAnchors / 2 - 1], zy = ay[kAnchors / 2 - 1] + by[kAnchors / 2 - 1];
+    const float den = (1.0f) / (fmaf(zx, zx, zy * zy));
     sp.wr = zx * den;
     sp.wi = -zy * den;
 }
@@ -164,7 +181,7 @@ SX_DEV OffPlan offset_plan(const Piece& p, float eta, float ta, float tb, int mo
     float n_f, ah = fabsf(eta);
     if (mode == kModeArc) {
         // L177 with s = L, kappa' = k1/L^2, scaled by the range fraction (R-12)
-        float n_full = cbrtf(p.L * fabsf(p.k1) * (1.0f + 0.4f * fabsf(eta * p.k1) / p.L) / (120.0f * tol_fl));
+        float n_full = cbrt_fast(div_fast(p.L * fabsf(p.k1) * (1.0f + 0.4f * div_fast(fabsf(eta * p.k1), p.L)), 120.0f * tol_fl));
         n_f = ceilf((tb - ta) * n_full);
     } else {
         float ka = es_kappa(p, ta), kb = es_kappa(p, tb);
@@ -172,12 +189,12 @@ SX_DEV OffPlan offset_plan(const Piece& p, float eta, float ta, float tb, int mo
         float xm = 0.5f * (xa + xb);
         if (fabsf(xb - xa) < 0.015625f * fmaxf(1.0f, fabsf(xm))) {
             float km = 0.5f * (ka + kb);  // constant density sqrt|k(1-k eta)| (R-7; limit is L73)
-            n_f = ceilf((tb - ta) * p.L * sqrtf(fabsf(km * (1.0f - km * eta)) / (8.0f * tol_fl)));
+            n_f = ceilf((tb - ta) * p.L * sqrt_fast(div_fast(fabsf(km * (1.0f - km * eta)), 8.0f * tol_fl)));
         } else {
             o.ua = f_approx(xa);
             o.ub = f_approx(xb);
-            float kp = fabsf(p.k1) / (p.L * p.L);
-            n_f = ceilf(fabsf(o.ub - o.ua) / (4.0f * kp * ah * sqrtf(ah) * sqrtf(8.0f * tol_fl)));  // L83
+            float kp = div_fast(fabsf(p.k1), p.L * p.L);
+            n_f = ceilf(div_fast(fabsf(o.ub - o.ua), 4.0f * kp * ah * sqrt_fast(ah) * sqrt_fast(8.0f * tol_fl)));  // L83
             o.uniform = false;
         }
     }
@@ -192,7 +209,7 @@ SX_DEV float offset_t(const Piece& p, const OffPlan& o, float eta, int i) {
         float u = o.ua + fr * (o.ub - o.ua);
         float x = f_approx_inv(u);
         float kap = (x + 1.0f) / (2.0f * eta);
-        t = 0.5f + (kap * p.L - p.k0) / p.k1;
+        t = 0.5f + (kap * p.L - p.k0) / (p.k1);
     }
     return clampf(t, o.ta, o.tb);
 }
@@ -202,15 +219,15 @@ SX_DEV EvoPlan evolute_plan(const Piece& p, float ta, float tb, float tol_fl) {
     EvoPlan e;
     e.ta = ta; e.tb = tb; e.wa = 0.0f; e.wb = 0.0f; e.uniform = true;
     float ka = es_kappa(p, ta), kb = es_kappa(p, tb), km = 0.5f * (ka + kb);
-    float kp = fabsf(p.k1) / (p.L * p.L);
+    float kp = (fabsf(p.k1)) / (p.L * p.L);
     e.skp = ka < 0.0f ? -kp : kp;
     float n_f;
     if (fabsf(kb - ka) < 0.015625f * fabsf(km)) {
-        n_f = ceilf((tb - ta) * p.L * sqrtf(fabsf(kp / km) / (8.0f * tol_fl)));
+        n_f = ceilf((tb - ta) * p.L * sqrt_fast(div_fast(fabsf(div_fast(kp, km)), 8.0f * tol_fl)));
     } else {
         e.wa = sqrtf(fabsf(ka) / kp);
         e.wb = sqrtf(fabsf(kb) / kp);
-        n_f = ceilf(fabsf(2.0f * e.wb - 2.0f * e.wa) * sqrtf(1.0f / (8.0f * tol_fl)));
+        n_f = ceilf(fabsf(2.0f * e.wb - 2.0f * e.wa) * sqrt_fast(div_fast(1.0f, 8.0f * tol_fl)));
         e.uniform = false;
     }
     e.n = count_clamp(n_f);
@@ -222,7 +239,7 @@ SX_DEV float evolute_t(const Piece& p, const EvoPlan& e, int i) {
     else {
         float w = e.wa + fr * (e.wb - e.wa);
         float kap = e.skp * w * w;
-        t = 0.5f + (kap * p.L - p.k0) / p.k1;
+        t = 0.5f + (kap * p.L - p.k0) / (p.k1);
     }
     return clampf(t, e.ta, e.tb);
 }

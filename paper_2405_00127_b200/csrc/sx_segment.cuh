@@ -33,8 +33,8 @@ struct SideSink {
     uint32_t total;
     bool mirror;
     SX_DEV void put(uint32_t idx, V2 a, V2 b, float angle, uint32_t kind) const {
-        if (mirror) w->put(first + (total - 1u - idx), b, a, -angle, kind | kPlus);
-        else w->put(first + idx, a, b, angle, kind);
+        if (mirror) w->put(first + (total - 1u - idx), b, a, 0.0f - angle, kind | kPlus);  // never a negative zero
+        else w->put(first + idx, a, b, angle + 0.0f, kind);
     }
 };
 
@@ -102,7 +102,7 @@ SX_DEV void emit_round(const Writer* w, uint32_t first, int n, V2 V, V2 r, V2 A,
         V2 cur = B;
         if (i < n) {
             float a = phi * (float)i / (float)n, sa, ca;
-            sincosf(a, &sa, &ca);
+            sx_sincos(a, &sa, &ca);
             cur.x = V.x + fmaf(ca, r.x, -sa * r.y);
             cur.y = V.y + fmaf(sa, r.x, ca * r.y);
         }
