@@ -19,15 +19,20 @@ constexpr int kWpThreads = 256;            // write kernel: threads per block
 constexpr int kWpPieces = 64;              // descriptors per tile
 constexpr int kWpBlocksPerSM = 3;
 
-// (b) count pass.  One thread per input segment runs Alg. 2 without the writes; every accepted piece is
-// stored in the piece cache.  The loop is warp-synchronous at piece granularity: each round every lane
-// advances to its next accepted piece, the warp ballots, and descriptor slots come from a warp-private
-// chunk reserved with one atomic per kChunk slots (unused slots of a chunk are marked invalid).
+// (b) count pass.  One thread per input segment runs Alg. 2 without the writes; every accepted piece is stored in
+// the piece cache.  The block works in rounds: every thread advances its segment to its next accepted piece
+// (fit_next); the round's pieces are compacted through shared memory and their 2 x T side plans are spread over
+// ALL threads of the block (a segment that is a line, or already finished, still plans for its neighbours); one
+// atomic per round reserves exactly T descriptor slots.
 __global__ void __launch_bounds__(kSegThreads)
 k_count(Params P, uint32_t* __restrict__ seg_count, float4* __restrict__ pieces, uint32_t piece_cap, uint32_t* piece_ctr,
         const uint32_t* __restrict__ err) {
-    const uint32_t i = blockIdx.x * (uint32_t)kSegThreads + threadIdx.x;
-    const uint32_t lane = threadIdx.x & 31u;
+    __shared__ float4 s_q[kSegThreads];          // k0, k1, L, h of the round's pieces
+    __shared__ uint32_t s_n[2 * kSegThreads];    // their side totals (-h, +h)
+    __shared__ uint32_t s_wcnt[kSegThreads / 32];
+    __shared__ uint32_t s_base;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t i = blockIdx.x * (uint32_t)kSegThreads + (uint32_t)tid;
     const bool valid = i < P.n_tags && *err == 0u;
     uint32_t n = 0, n_tail = 0;
     bool active = false;
@@ -44,39 +49,40 @@ k_count(Params P, uint32_t* __restrict__ seg_count, float4* __restrict__ pieces,
             n_tail = segment_tail<false>(P, i, tag, s, st, h, nullptr, 0);
         }
     }
-    uint32_t chunk_base = 0, chunk_used = kChunk;  // no chunk yet
-    while (__any_sync(0xffffffffu, active)) {
+    for (;;) {
         bool have = false;
         Piece p;
-        uint32_t nm = 0, np = 0;
         if (active) {
             have = fit_next(P, s, f, p);
-            if (have) {
-                nm = (uint32_t)side_plan(p, -h, P.mode, P.tol_fl).total;
-                np = (uint32_t)side_plan(p, h, P.mode, P.tol_fl).total;
-            } else {
-                active = false;
-            }
+            if (!have) active = false;
         }
         const uint32_t ballot = __ballot_sync(0xffffffffu, have);
-        const uint32_t cnt = __popc(ballot);
-        if (cnt == 0u) continue;
-        if (chunk_used + cnt > (uint32_t)kChunk) {
-            for (uint32_t k = chunk_used + lane; k < (uint32_t)kChunk; k += 32u)
-                if (chunk_base + k < piece_cap) piece_invalidate(pieces + (uint64_t)(chunk_base + k) * kDescQuads);
-            if (lane == 0u) chunk_base = atomicAdd(piece_ctr, (uint32_t)kChunk);
-            chunk_base = __shfl_sync(0xffffffffu, chunk_base, 0);
-            chunk_used = 0u;
+        if (lane == 0) s_wcnt[warp] = __popc(ballot);
+        __syncthreads();
+        uint32_t T = 0, wbase = 0;
+#pragma unroll
+        for (int k = 0; k < kSegThreads / 32; k++) {
+            if (k == warp) wbase = T;
+            T += s_wcnt[k];
         }
+        if (T == 0u) break;
+        const uint32_t idx = wbase + __popc(ballot & ((1u << lane) - 1u));
+        if (have) s_q[idx] = make_float4(p.k0, p.k1, p.L, h);
+        if (tid == 0) s_base = atomicAdd(piece_ctr, T);
+        __syncthreads();
+        for (uint32_t j = (uint32_t)tid; j < 2u * T; j += (uint32_t)kSegThreads) {
+            const float4 q = s_q[j >> 1];
+            Piece pp;
+            pp.k0 = q.x; pp.k1 = q.y; pp.L = q.z;
+            s_n[j] = (uint32_t)side_plan(pp, (j & 1u) ? q.w : -q.w, P.mode, P.tol_fl).total;
+        }
+        __syncthreads();
         if (have) {
-            uint32_t slot = chunk_base + chunk_used + __popc(ballot & ((1u << lane) - 1u));
+            const uint32_t nm = s_n[2u * idx], np = s_n[2u * idx + 1u], slot = s_base + idx;
             if (slot < piece_cap) piece_store(pieces + (uint64_t)slot * kDescQuads, p, h, i, n, nm, np);
             n += nm + np;
         }
-        chunk_used += cnt;
     }
-    for (uint32_t k = chunk_used + lane; k < (uint32_t)kChunk; k += 32u)
-        if (chunk_base + k < piece_cap) piece_invalidate(pieces + (uint64_t)(chunk_base + k) * kDescQuads);
     if (i < P.n_tags) seg_count[i] = n + n_tail;
 }
 

@@ -14,11 +14,21 @@ namespace sx {
 // moves a vertex by up to ~5e-4 px along the curve, and the oracle evaluates this path in fp32 too.
 // f_approx (L149), odd extension (L157), middle piece sign-preserving (R-3b)
 SX_DEV float f_approx(float x) {
-    float a = fabsf(x), r;
-    if (a < 0.8f) r = sinf(kC1 * a) / kC1;
-    else if (a < 1.25f) { float v = a - 1.0f; float w = fabsf(v) * sqrtf(fabsf(v)); r = kSqrt8Over3 * (v < 0.0f ? -w : w) + kQuarterPi; }
-    else if (a < 2.1f) r = 0.6406f * a * a - 0.81f * a + kC2;
-    else r = 0.5f * a * a - 0.156f * a + kC3;
+    // All four pieces are evaluated and one is selected: the threads of a warp sit on different pieces, and a
+    // branch per piece would serialise them.  sin on [0, 0.88] by its Taylor series to y^11 (truncation 6e-9).
+    const float a = fabsf(x);
+    const float y = kC1 * fminf(a, 0.8f), y2 = y * y;
+    float sn = fmaf(y2, -2.5052108385441720e-8f, 2.7557319223985893e-6f);
+    sn = fmaf(sn, y2, -1.9841269841269841e-4f);
+    sn = fmaf(sn, y2, 8.3333333333333333e-3f);
+    sn = fmaf(sn, y2, -1.6666666666666667e-1f);
+    sn = fmaf(sn * y2, y, y);
+    const float r0 = sn / kC1;
+    const float v = a - 1.0f, w = fabsf(v) * sqrtf(fabsf(v));
+    const float r1 = kSqrt8Over3 * (v < 0.0f ? -w : w) + kQuarterPi;
+    const float r2 = 0.6406f * a * a - 0.81f * a + kC2;
+    const float r3 = 0.5f * a * a - 0.156f * a + kC3;
+    const float r = a < 0.8f ? r0 : (a < 1.25f ? r1 : (a < 2.1f ? r2 : r3));
     return x < 0.0f ? -r : r;
 }
 // each piece of L149 solved for x
