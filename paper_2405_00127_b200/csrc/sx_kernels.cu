@@ -19,34 +19,59 @@ constexpr int kWpThreads = 256;            // write kernel: threads per block
 constexpr int kWpPieces = 64;              // descriptors per tile
 constexpr int kWpBlocksPerSM = 3;
 
-// (b) count pass.  One thread per input segment runs Alg. 2 without the writes; every accepted piece is stored in
-// the piece cache.  The block works in rounds: every thread advances its segment to its next accepted piece
-// (fit_next); the round's pieces are compacted through shared memory and their 2 x T side plans are spread over
-// ALL threads of the block (a segment that is a line, or already finished, still plans for its neighbours); one
-// atomic per round reserves exactly T descriptor slots.
+// (b) count pass: the number of records of every segment, and the piece cache.
+// Part 1, one thread per segment of the block's tile: straight segments (2 exact offset lines + join / caps).
+// Part 2, one thread per entry of the compact curve list built by the tag scan (so that a scene that mixes lines
+// and curves still fills its warps with curves).  The block works in rounds: every thread advances its curve to
+// its next accepted piece (fit_next, Alg. 2); the round's pieces are compacted through shared memory and
+// their 2 x T side plans are spread over ALL threads of the block (a thread whose curve is finished still plans
+// for its neighbours); one atomic per round reserves exactly T descriptor slots of the piece cache.
 __global__ void __launch_bounds__(kSegThreads)
-k_count(Params P, uint32_t* __restrict__ seg_count, float4* __restrict__ pieces, uint32_t piece_cap, uint32_t* piece_ctr,
-        const uint32_t* __restrict__ err) {
+k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__ curve_idx, const uint32_t* __restrict__ n_curves_p,
+        float4* __restrict__ pieces, uint32_t piece_cap, uint32_t* piece_ctr, const uint32_t* __restrict__ err) {
     __shared__ float4 s_q[kSegThreads];          // k0, k1, L, h of the round's pieces
     __shared__ uint32_t s_n[2 * kSegThreads];    // their side totals (-h, +h)
     __shared__ uint32_t s_wcnt[kSegThreads / 32];
     __shared__ uint32_t s_base;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t i = blockIdx.x * (uint32_t)kSegThreads + (uint32_t)tid;
-    const bool valid = i < P.n_tags && *err == 0u;
-    uint32_t n = 0, n_tail = 0;
+    const bool ok = *err == 0u;
+    {   // ---- part 1: straight segments of this block's tile
+        const uint32_t i = blockIdx.x * (uint32_t)kSegThreads + (uint32_t)tid;
+        if (i < P.n_tags) {
+            const uint32_t tag = P.tags[i];
+            if (!ok) seg_count[i] = 0u;
+            else if ((tag & 3u) == 1u) {
+                Style st;
+                float h;
+                uint32_t n = 0;
+                if (load_style(P, P.path_idx[i], &st, &h)) {
+                    Seg s = load_segment(P, i, tag);
+                    n = 2u + segment_tail<false>(P, i, tag, s, st, h, nullptr, 0);
+                }
+                seg_count[i] = n;
+            }
+        }
+    }
+    // ---- part 2: curves
+    const uint32_t n_curves = ok ? *n_curves_p : 0u;
+    const uint32_t rank = blockIdx.x * (uint32_t)kSegThreads + (uint32_t)tid;
+    if (blockIdx.x * (uint32_t)kSegThreads >= n_curves) return;
     bool active = false;
+    uint32_t i = 0, n = 0, n_tail = 0;
     Seg s;
-    Style st;
     FitState f;
     float h = 0.0f;
-    if (valid) {
-        uint32_t tag = P.tags[i];
-        if (load_style(P, P.path_idx[i], &st, &h)) {
+    if (rank < n_curves) {
+        i = curve_idx[rank];
+        const uint32_t tag = P.tags[i];
+        Style st;
+        if (!load_style(P, P.path_idx[i], &st, &h)) {
+            seg_count[i] = 0u;
+        } else {
             s = load_segment(P, i, tag);
-            if (s.kind == 1 || s.degenerate) n = 2;
-            else { active = true; f = fit_begin(s); }
             n_tail = segment_tail<false>(P, i, tag, s, st, h, nullptr, 0);
+            if (s.degenerate) seg_count[i] = 2u + n_tail;  // all control points coincide: straight path (R-5)
+            else { active = true; f = fit_begin(s); }
         }
     }
     for (;;) {
@@ -54,7 +79,7 @@ k_count(Params P, uint32_t* __restrict__ seg_count, float4* __restrict__ pieces,
         Piece p;
         if (active) {
             have = fit_next(P, s, f, p);
-            if (!have) active = false;
+            if (!have) { seg_count[i] = n + n_tail; active = false; }
         }
         const uint32_t ballot = __ballot_sync(0xffffffffu, have);
         if (lane == 0) s_wcnt[warp] = __popc(ballot);
@@ -65,7 +90,7 @@ k_count(Params P, uint32_t* __restrict__ seg_count, float4* __restrict__ pieces,
             if (k == warp) wbase = T;
             T += s_wcnt[k];
         }
-        if (T == 0u) break;
+        if (T == 0u) break;  // fit_next yields a piece every round until the curve ends
         const uint32_t idx = wbase + __popc(ballot & ((1u << lane) - 1u));
         if (have) s_q[idx] = make_float4(p.k0, p.k1, p.L, h);
         if (tid == 0) s_base = atomicAdd(piece_ctr, T);
@@ -83,7 +108,6 @@ k_count(Params P, uint32_t* __restrict__ seg_count, float4* __restrict__ pieces,
             n += nm + np;
         }
     }
-    if (i < P.n_tags) seg_count[i] = n + n_tail;
 }
 
 // (d1) write pass over the piece cache: one thread per output record, no per-record branching.
@@ -146,21 +170,11 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
             }
         } else {
             // anchor table: each of the two threads of a piece integrates one half, then they exchange totals
-            float hx[kAnchors / 2], hy[kAnchors / 2];
-            es_anchor_half(p, side, hx, hy);
-            const float ox = __shfl_xor_sync(0xffffffffu, hx[kAnchors / 2 - 1], 1), oy = __shfl_xor_sync(0xffffffffu, hy[kAnchors / 2 - 1], 1);
-            if (live) {
-                Spiral& z = S.spiral[sub >> 1];
-                const float bx = side ? ox : 0.0f, by = side ? oy : 0.0f;
-#pragma unroll
-                for (int k = 0; k < kAnchors / 2; k++) { z.zx[side * (kAnchors / 2) + k + 1] = bx + hx[k]; z.zy[side * (kAnchors / 2) + k + 1] = by + hy[k]; }
-                if (side == 0) {
-                    z.zx[0] = 0.0f; z.zy[0] = 0.0f;
-                    const float zx = hx[kAnchors / 2 - 1] + ox, zy = hy[kAnchors / 2 - 1] + oy;  // Z(1)
-                    const float den = 1.0f / fmaf(zx, zx, zy * zy);
-                    z.wr = zx * den; z.wi = -zy * den;
-                }
-            }
+            const int K = es_intervals(p.k0, p.k1);
+            float hx[kAnchors / 2], hy[kAnchors / 2], tx, ty;
+            const int cnt = es_anchor_half(p, K, side, hx, hy, &tx, &ty);
+            const float ox = __shfl_xor_sync(0xffffffffu, tx, 1), oy = __shfl_xor_sync(0xffffffffu, ty, 1);
+            if (live) es_anchor_store(S.spiral[sub >> 1], K, side, cnt, hx, hy, tx, ty, ox, oy);
         }
         // ---- phase 2: scan (parts, records) over the side threads, then the part table
         uint32_t ip = nparts, ir = nrec;
@@ -303,7 +317,7 @@ static thread_local cudaError_t g_last_cuda = cudaSuccess;
 struct sx_ctx {
     int device;
     // scratch of the call in flight
-    uint32_t *pt_off, *path_idx, *sp_first, *seg_count;
+    uint32_t *pt_off, *path_idx, *sp_first, *seg_count, *curve_idx;
     uint64_t* seg_off;
     uint64_t cap_segs;
     uint8_t* sync_area;   // [flags 64 B][d_total 64 B][alloc tile states][tag tile states]
@@ -329,6 +343,7 @@ struct sx_ctx {
 static uint32_t* ctx_err(sx_ctx* c) { return reinterpret_cast<uint32_t*>(c->sync_area); }
 static uint32_t* ctx_ticket(sx_ctx* c, int k) { return reinterpret_cast<uint32_t*>(c->sync_area) + 4 + 4 * k; }
 static uint32_t* ctx_piece_ctr(sx_ctx* c) { return reinterpret_cast<uint32_t*>(c->sync_area) + 12; }
+static uint32_t* ctx_n_curves(sx_ctx* c) { return reinterpret_cast<uint32_t*>(c->sync_area) + 13; }
 static uint64_t* ctx_total(sx_ctx* c) { return reinterpret_cast<uint64_t*>(c->sync_area + 64); }
 
 static uint64_t round_up(uint64_t x, uint64_t m) { return (x + m - 1) / m * m; }
@@ -347,14 +362,15 @@ static sx_status ensure_scratch(sx_ctx* c, uint64_t n) {
         if (c->pt_off) SX_CUDA(cudaFree(c->pt_off));
         c->pt_off = nullptr; c->cap_segs = 0;
         uint64_t cap = round_up(n + n / 8 + 64, 64);
-        // one allocation: 4 u32 arrays then the u64 offsets (all 256-byte aligned since cap % 64 == 0)
+        // one allocation: 5 u32 arrays then the u64 offsets (all 256-byte aligned since cap % 64 == 0)
         uint8_t* p;
-        SX_CUDA(cudaMalloc(&p, cap * (4 * 4 + 8)));
+        SX_CUDA(cudaMalloc(&p, cap * (6 * 4 + 8)));
         c->pt_off = reinterpret_cast<uint32_t*>(p);
         c->path_idx = c->pt_off + cap;
         c->sp_first = c->path_idx + cap;
         c->seg_count = c->sp_first + cap;
-        c->seg_off = reinterpret_cast<uint64_t*>(c->seg_count + cap);
+        c->curve_idx = c->seg_count + cap;
+        c->seg_off = reinterpret_cast<uint64_t*>(c->curve_idx + 2 * cap);
         c->cap_segs = cap;
     }
     return SX_OK;
@@ -457,8 +473,8 @@ sx_status sx_count(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, const floa
             uint64_t* alloc_states = reinterpret_cast<uint64_t*>(c->sync_area + 128);
             sx::TagTileState* tag_states = reinterpret_cast<sx::TagTileState*>(c->sync_area + 128 + round_up((uint64_t)(n_alloc_tiles + 1) * 8, 64));
             sx::k_tag_scan<<<n_tag_tiles, sx::kScanThreads, 0, s>>>(d_tags, n, (uint32_t)n_points, (uint32_t)n_paths, c->pt_off, c->path_idx,
-                                                                   c->sp_first, tag_states, ctx_ticket(c, 0), ctx_err(c));
-            sx::k_count<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(P, c->seg_count, c->pieces, (uint32_t)c->piece_cap,
+                                                                   c->sp_first, c->curve_idx, ctx_n_curves(c), tag_states, ctx_ticket(c, 0), ctx_err(c));
+            sx::k_count<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(P, c->seg_count, c->curve_idx, ctx_n_curves(c), c->pieces, (uint32_t)c->piece_cap,
                                                                                               ctx_piece_ctr(c), ctx_err(c));
             sx::k_alloc_scan<<<n_alloc_tiles, sx::kScanThreads, 0, s>>>(c->seg_count, n, d_tags, c->path_idx, (uint32_t)n_paths, c->seg_off,
                                                                       d_path_offsets, ctx_total(c), alloc_states, ctx_ticket(c, 1), ctx_err(c));

@@ -68,16 +68,22 @@ SX_DEV float es_kappa(const Piece& p, float t) { return (p.k0 + p.k1 * (t - 0.5f
 
 // ---------------------------------------------------------------- Euler-spiral integral (R-2)
 // Z(t) = int_0^t exp(i phi(u)) du, phi(u) = (k0-k1/2) u + k1 u^2/2.  Evaluated from a per-piece table of
-// anchors Z(k/8), k = 0..8 (accumulated once per piece by 3-point Gauss-Legendre on each eighth), plus a
-// 3-point Gauss-Legendre rule from the nearest anchor to t (|t - k/8| <= 1/16).  On an accepted piece
-// |phi'| stays below ~20 rad per unit t (|k0| <= 4.2 by the 120-degree guard R-4, k1 ~ 6 (th1 - th0)), so
-// a vertex integrates over at most ~1 rad of phase, where the 3-point rule is at fp32 round-off; the cost
-// per vertex is 3 sincos instead of a full-interval high-order rule.
+// anchors Z(k/K), k = 0..K (accumulated once per piece by 3-point Gauss-Legendre on each interval), plus a 3-point
+// rule from the nearest anchor to t (|t - k/K| <= 1/(2K)).  K = 1, 2, 4 or 8 is chosen per piece so that the phase
+// advances by at most ~1 rad per interval (max |phi'| <= |k0 - k1/2| + |k1|; on an accepted piece that is below
+// ~20: |k0| <= 4.2 by the 120-degree guard R-4, k1 ~ 6 (th1 - th0)), where the 3-point rule's error, ~Phi^6 / 2e6
+// of the interval, is at fp32 round-off.  Typical pieces (CAD scene: total turning ~0.3 rad) take K = 1: three sincos
+// for Z(1) and three per interior vertex.
 constexpr int kAnchors = 8;
 struct Spiral {
     float wr, wi;                          // 1 / Z(1) (complex)
+    float K;                               // number of intervals (1, 2, 4, 8)
     float zx[kAnchors + 1], zy[kAnchors + 1];
 };
+SX_DEV int es_intervals(float k0, float k1) {
+    const float span = fabsf(k0 - 0.5f * k1) + fabsf(k1);
+    return span <= 1.0f ? 1 : (span <= 2.0f ? 2 : (span <= 4.0f ? 4 : 8));
+}
 
 // sin and cos of a moderate argument (|x| < ~1e3): two-constant Cody-Waite reduction by pi/2 and the
 // classic single-precision minimax kernels on [-pi/4, pi/4] (errors ~1e-7), all on the FMA pipe.
@@ -106,34 +112,50 @@ SX_DEV void es_gl3(float a, float hk, float m, float hd, float* ix, float* iy) {
     *iy = hd * fmaf(0.55555555555555556f, s0 + s2, 0.88888888888888889f * s1);
 }
 
-// one half (0: [0,1/2], 1: [1/2,1]) of the anchor table: cumulative sums of the half's sub-integrals, relative to
-// the half's start.  es_prepare = both halves by one thread; the write kernel gives one half to each side thread.
-SX_DEV void es_anchor_half(const Piece& p, int half, float* hx, float* hy) {
+// one half of the anchor table: half 0 integrates intervals [0, max(K/2,1)), half 1 intervals [K/2, K) (none when
+// K = 1); cumulative sums relative to the half's start in hx/hy[0..count), the half's total in *tx, *ty.
+// es_prepare = both halves by one thread; the write kernel gives one half to each of two threads.
+SX_DEV int es_anchor_half(const Piece& p, int K, int half, float* hx, float* hy, float* tx, float* ty) {
     const float a = p.k0 - 0.5f * p.k1, hk = 0.5f * p.k1;
+    const float w = 1.0f / (float)K;
+    const int first = half ? K / 2 : 0, count = half ? K / 2 : (K > 1 ? K / 2 : 1);
     float zx = 0.0f, zy = 0.0f;
 #pragma unroll
     for (int k = 0; k < kAnchors / 2; k++) {
-        float ix, iy;
-        es_gl3(a, hk, ((float)(half * (kAnchors / 2) + k) + 0.5f) * (1.0f / kAnchors), 0.5f / kAnchors, &ix, &iy);
-        zx += ix; zy += iy;
+        if (k < count) {
+            float ix, iy;
+            es_gl3(a, hk, ((float)(first + k) + 0.5f) * w, 0.5f * w, &ix, &iy);
+            zx += ix; zy += iy;
+        }
         hx[k] = zx; hy[k] = zy;
+    }
+    *tx = zx; *ty = zy;
+    return count;
+}
+// stores a half's anchors (offset by the other half's total for half 1) and, by half 0, Z(0), K and 1/Z(1)
+SX_DEV void es_anchor_store(Spiral& sp, int K, int half, int count, const float* hx, const float* hy, float tx, float ty, float ox, float oy) {
+    const int first = half ? K / 2 : 0;
+    const float bx = half ? ox : 0.0f, by = half ? oy : 0.0f;
+#pragma unroll
+    for (int k = 0; k < kAnchors / 2; k++)
+        if (k < count) { sp.zx[first + k + 1] = bx + hx[k]; sp.zy[first + k + 1] = by + hy[k]; }
+    if (half == 0) {
+        sp.zx[0] = 0.0f; sp.zy[0] = 0.0f;
+        sp.K = (float)K;
+        const float zx = tx + ox, zy = ty + oy;  // Z(1)
+        const float den = 1.0f / fmaf(zx, zx, zy * zy);
+        sp.wr = zx * den;
+        sp.wi = -zy * den;
     }
 }
 
 SX_DEV void es_prepare(const Piece& p, Spiral& sp) {
-    float ax[kAnchors / 2], ay[kAnchors / 2], bx[kAnchors / 2], by[kAnchors / 2];
-    es_anchor_half(p, 0, ax, ay);
-    es_anchor_half(p, 1, bx, by);
-    sp.zx[0] = 0.0f; sp.zy[0] = 0.0f;
-#pragma unroll
-    for (int k = 0; k < kAnchors / 2; k++) {
-        sp.zx[k + 1] = ax[k]; sp.zy[k + 1] = ay[k];
-        sp.zx[kAnchors / 2 + k + 1] = ax[kAnchors / 2 - 1] + bx[k]; sp.zy[kAnchors / 2 + k + 1] = ay[kAnchors / 2 - 1] + by[k];
-    }
-    const float zx = ax[kAnchors / 2 - 1] + bx[kAnchors / 2 - 1], zy = ay[kAnchors / 2 - 1] + by[kAnchors / 2 - 1];
-    const float den = (1.0f) / (fmaf(zx, zx, zy * zy));
-    sp.wr = zx * den;
-    sp.wi = -zy * den;
+    const int K = es_intervals(p.k0, p.k1);
+    float ax[kAnchors / 2], ay[kAnchors / 2], bx[kAnchors / 2], by[kAnchors / 2], atx, aty, btx, bty;
+    const int ca = es_anchor_half(p, K, 0, ax, ay, &atx, &aty);
+    const int cb = es_anchor_half(p, K, 1, bx, by, &btx, &bty);
+    es_anchor_store(sp, K, 1, cb, bx, by, btx, bty, atx, aty);
+    es_anchor_store(sp, K, 0, ca, ax, ay, atx, aty, btx, bty);
 }
 
 SX_DEV float es_phi(const Piece& p, float t) { return t * fmaf(0.5f * p.k1, t, p.k0 - 0.5f * p.k1); }
@@ -143,9 +165,11 @@ SX_DEV float es_dphi(const Piece& p, float ta, float tb) { return (tb - ta) * fm
 // local position and unit tangent at piece fraction t in [0,1]: la + ch (x) Z(t)/Z(1) (L632)
 SX_DEV void es_eval(const Piece& p, const Spiral& sp, float t, V2* pos, V2* tan) {
     const float a = p.k0 - 0.5f * p.k1, hk = 0.5f * p.k1;
-    int k = (int)rintf(t * (float)kAnchors);
-    k = k < 0 ? 0 : (k > kAnchors ? kAnchors : k);
-    const float t0 = (float)k * (1.0f / kAnchors), hd = 0.5f * (t - t0);
+    const float K = sp.K;
+    float kf = rintf(t * K);
+    kf = kf < 0.0f ? 0.0f : (kf > K ? K : kf);
+    const int k = (int)kf;
+    const float t0 = kf / K, hd = 0.5f * (t - t0);  // K is a power of two: exact
     float ix, iy;
     es_gl3(a, hk, t0 + hd, hd, &ix, &iy);
     const float zx = sp.zx[k] + ix, zy = sp.zy[k] + iy;

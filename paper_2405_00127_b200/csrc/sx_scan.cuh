@@ -4,7 +4,8 @@
 //     the offsets are prefix sums over the "tag monoid".  Ours is (points, paths, first) with
 //     points += count + subpath_end (L470), paths += path_end, first = max(index+1 of subpath ends):
 //     the exclusive prefix gives segment i its first point, its path and the first segment of its
-//     subpath (which replaces the paper's stroke-cap-marker segment, L483-489).
+//     subpath (which replaces the paper's stroke-cap-marker segment, L483-489).  A fourth component counts the
+//     curve segments (quadratics and cubics) and yields their compact index list for the count kernel.
 // (c) k_alloc_scan: exclusive prefix sum of the per-segment record counts -> record offsets (replaces
 //     the paper's atomic bump allocation, L448), the per-path offsets and the total.
 //
@@ -26,18 +27,18 @@ constexpr int kCntTile = kScanThreads * kCntItems;    // 2048
 
 enum : uint32_t { kErrBadStream = 1u, kErrCapacity = 2u };
 
-struct TagAgg { uint32_t pt, path, first; };
-__device__ __forceinline__ TagAgg tag_identity() { TagAgg a; a.pt = 0; a.path = 0; a.first = 0; return a; }
+struct TagAgg { uint32_t pt, path, first, curve; };
+__device__ __forceinline__ TagAgg tag_identity() { TagAgg a; a.pt = 0; a.path = 0; a.first = 0; a.curve = 0; return a; }
 __device__ __forceinline__ TagAgg tag_combine(TagAgg a, TagAgg b) {
-    TagAgg r; r.pt = a.pt + b.pt; r.path = a.path + b.path; r.first = a.first > b.first ? a.first : b.first; return r;
+    TagAgg r; r.pt = a.pt + b.pt; r.path = a.path + b.path; r.first = a.first > b.first ? a.first : b.first; r.curve = a.curve + b.curve; return r;
 }
 __device__ __forceinline__ TagAgg tag_shfl_up(TagAgg a, int d) {
     TagAgg r; r.pt = __shfl_up_sync(0xffffffffu, a.pt, d); r.path = __shfl_up_sync(0xffffffffu, a.path, d);
-    r.first = __shfl_up_sync(0xffffffffu, a.first, d); return r;
+    r.first = __shfl_up_sync(0xffffffffu, a.first, d); r.curve = __shfl_up_sync(0xffffffffu, a.curve, d); return r;
 }
 __device__ __forceinline__ TagAgg tag_shfl_xor(TagAgg a, int d) {
     TagAgg r; r.pt = __shfl_xor_sync(0xffffffffu, a.pt, d); r.path = __shfl_xor_sync(0xffffffffu, a.path, d);
-    r.first = __shfl_xor_sync(0xffffffffu, a.first, d); return r;
+    r.first = __shfl_xor_sync(0xffffffffu, a.first, d); r.curve = __shfl_xor_sync(0xffffffffu, a.curve, d); return r;
 }
 
 // look-back descriptor of one tag tile: status 0 = nothing yet, 1 = aggregate valid, 2 = inclusive valid
@@ -48,7 +49,8 @@ __device__ __forceinline__ uint64_t ld_volatile_u64(const uint64_t* p) { return 
 
 __global__ void __launch_bounds__(kScanThreads)
 k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint32_t n_paths, uint32_t* __restrict__ pt_off,
-           uint32_t* __restrict__ path_idx, uint32_t* __restrict__ sp_first, TagTileState* states, uint32_t* ticket, uint32_t* err) {
+           uint32_t* __restrict__ path_idx, uint32_t* __restrict__ sp_first, uint32_t* __restrict__ curve_idx, uint32_t* n_curves,
+           TagTileState* states, uint32_t* ticket, uint32_t* err) {
     __shared__ uint32_t s_tile;
     __shared__ TagAgg s_warp[kScanThreads / 32];
     __shared__ TagAgg s_prefix;
@@ -78,6 +80,7 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
         bad |= valid && (cnt == 0u || (tag & 8u));
         mine.pt += cnt + end;
         mine.path += (tag >> 4) & 1u;
+        mine.curve += (valid && cnt >= 2u) ? 1u : 0u;
         if (end) mine.first = base + k + 1u;
     }
     if (bad) atomicOr(err, kErrBadStream);
@@ -100,7 +103,7 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
     if (warp == 0) {
         TagTileState* me = states + tile;
         if (lane == 0 && tile > 0) {
-            me->agg = make_uint4(tile_agg.pt, tile_agg.path, tile_agg.first, 0u);
+            me->agg = make_uint4(tile_agg.pt, tile_agg.path, tile_agg.first, tile_agg.curve);
             __threadfence();
             *reinterpret_cast<volatile uint32_t*>(&me->status) = 1u;
         }
@@ -114,7 +117,7 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
             TagAgg v = tag_identity();
             if (j >= 0) {
                 const volatile uint4* src = st == 2u ? &states[j].inc : &states[j].agg;
-                v.pt = src->x; v.path = src->y; v.first = src->z;
+                v.pt = src->x; v.path = src->y; v.first = src->z; v.curve = src->w;
             }
             uint32_t m = __ballot_sync(0xffffffffu, st == 2u);
             int stop = __ffs((int)m) - 1;  // nearest predecessor with an inclusive prefix (lanes with j < 0 report 2)
@@ -128,7 +131,7 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
         if (lane == 0) {
             s_prefix = excl;
             TagAgg inc = tag_combine(excl, tile_agg);
-            me->inc = make_uint4(inc.pt, inc.path, inc.first, 0u);
+            me->inc = make_uint4(inc.pt, inc.path, inc.first, inc.curve);
             __threadfence();
             *reinterpret_cast<volatile uint32_t*>(&me->status) = 2u;
         }
@@ -144,6 +147,7 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
         uint32_t tag = (w[k >> 2] >> (8 * (k & 3))) & 0xffu;
         uint32_t cnt = tag & 3u, end = ((tag >> 2) | (tag >> 4)) & 1u;
         o_pt[k] = run.pt; o_path[k] = run.path; o_first[k] = run.first;
+        if (base + k < n && cnt >= 2u) curve_idx[run.curve++] = base + k;  // compact list of the curve segments, in order
         run.pt += cnt + end;
         run.path += (tag >> 4) & 1u;
         if (end) run.first = base + k + 1u;
@@ -165,6 +169,7 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
         uint32_t k = n - 1u - base;
         uint32_t last = (w[k >> 2] >> (8 * (k & 3))) & 0xffu;
         if (!(last & 16u) || run.pt != n_points || run.path != n_paths) atomicOr(err, kErrBadStream);
+        *n_curves = run.curve;
     }
 }
 
