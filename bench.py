@@ -28,6 +28,9 @@ if ROOT not in sys.path:
 METRIC = "input path segments/sec expanded (device-timed)"
 UNIT = "segments/s"
 MODE_OF = {"c3": 0, "c4": 1, "c5": 0, "c1": 0, "c2": 0}
+# dram__bytes_read.sum + dram__bytes_write.sum of the write pass per launch, from the committed ncu captures
+# (profiles/r1_final_counters.md); None = not captured for that workload
+NCU_TRAFFIC = {"c4": None, "c5": None}
 REF_SAMPLE_PATHS = {"c4": 20000, "c5": 1000, "c3": 20000, "c1": 256, "c2": 2000}
 
 
@@ -72,6 +75,22 @@ class ClockSampler(threading.Thread):
         self.join(timeout=2)
         med = int(np.median(self.samples)) if self.samples else None
         return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def max_over_ranks(seconds, world, device=None):
+    """Device-timed seconds of this rank -> the maximum over all ranks (identity at world 1)."""
+    if world <= 1:
+        return float(seconds)
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([seconds], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def job_throughput(units_per_rank_per_step, steps, world, seconds_max):
+    """Whole-job throughput of `world` replicas (weak scaling): all ranks' units over the slowest rank's time."""
+    return world * units_per_rank_per_step * steps / seconds_max
 
 
 def make_scene(workload, n_paths=None):
@@ -178,10 +197,7 @@ def run_ours(args):
     t_count = sum(e[0].elapsed_time(e[1]) for e in evs) * 1e-3
     t_write = sum(e[1].elapsed_time(e[2]) for e in evs) * 1e-3
     t_total = sum(e[0].elapsed_time(e[2]) for e in evs) * 1e-3
-    if world > 1:
-        tt = torch.tensor([t_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_total = float(tt.item())
+    t_total = max_over_ranks(t_total, world, dev)
 
     # ---- end to end through the host-buffer entry point (pinned host memory, copies inside the timed region)
     htags, hpts, hsty = B.scene_to_torch(sc, pin=True)
@@ -196,10 +212,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     t_e2e = time.perf_counter() - t0
     assert m == total
-    if world > 1:
-        tt = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_e2e = float(tt.item())
+    t_e2e = max_over_ranks(t_e2e, world, dev)
     h2d = tags.numel() + pts.numel() * 4 + sty.numel()
     d2h = total * width * 4 + (n_paths + 1) * 8
 
@@ -208,19 +221,26 @@ def run_ours(args):
         # algorithmic bytes of the dominant kernel (write): the streams it must read + the records it must write
         alg_bytes = tags.numel() + pts.numel() * 4 + sty.numel() + total * width * 4
         ach = alg_bytes / (t_write / args.steps) / 1e9
-        line = {"metric": METRIC, "value": world * n_seg * args.steps / t_total, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        alg_step = alg_bytes + (n_paths + 1) * 8  # + the per-path offsets written by the allocation scan
+        line = {"metric": METRIC, "value": job_throughput(n_seg, args.steps, world, t_total), "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": args.workload, "segments": n_seg, "paths": n_paths, "records": int(total),
                            "mode": "arc" if mode else "line", "tolerance": float(sc.tolerance), "l2": "flushed between steps (256 MiB fill)",
                            "parallelism": "replicas only" if world > 1 else "single GPU"},
-                "output_records_per_s": world * total * args.steps / t_total,
+                "output_records_per_s": job_throughput(total, args.steps, world, t_total),
                 "kernel_ms": {"scan+count+alloc_scan": 1e3 * t_count / args.steps, "write": 1e3 * t_write / args.steps},
                 "gpu_launches": int(launches), "clocks": clocks,
-                "e2e": {"value": world * n_seg * e2e_steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "e2e": {"value": job_throughput(n_seg, e2e_steps, world, t_e2e), "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                         "ms_per_step": 1e3 * t_e2e / e2e_steps},
-                "roofline": {"kernel": "k_write", "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                             "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": int(alg_bytes)}}
+                "roofline": {"kernel": "write pass (d): k_write_pieces + k_write_segments, timed together around sx_write",
+                             "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                             "traffic": NCU_TRAFFIC.get(args.workload) if args.paths is None else None,
+                             "peak_source": peak_src, "algorithmic_bytes_per_launch": int(alg_bytes),
+                             "whole_step": {"achieved": alg_step / (t_total / args.steps) / 1e9, "frac": alg_step / (t_total / args.steps) / 1e9 / peak,
+                                            "algorithmic_bytes": int(alg_step)},
+                             "fp32_issue_peak_lane_ops_per_s": 148 * 128 * 1.965e9,
+                             "note": "measured regime is FP32/ALU issue, not HBM (DESIGN.md section 8, profiles/)"}}
         # ---- the oracle timed beside it on this box's host cores (single thread), bounded sample
         if world == 1 and not args.no_cpu_baseline:
             npaths = REF_SAMPLE_PATHS[args.workload] * 5
