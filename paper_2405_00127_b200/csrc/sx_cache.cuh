@@ -125,7 +125,7 @@ SX_DEV V2 end_vertex(const Piece& p, uint32_t code, float eta, float4 cusp, floa
     const bool e1 = which == kEndT1;
     const float t = e1 ? 1.0f : 0.0f;
     const V2 l = e1 ? p.lb : p.la, T = e1 ? p.ub : p.ua;
-    const float r = (code & kEndEvo) ? 1.0f / es_kappa(p, t) : eta;
+    const float r = (code & kEndEvo) ? es_radius(p, t) : eta;
     V2 g = v2(p.base.x + fmaf(r, -T.y, l.x), p.base.y + fmaf(r, T.x, l.y));
     if (e1 ? p.at1 : p.at0) g = offset_point(e1 ? p.P3 : p.base, T, r);
     *t_out = t;

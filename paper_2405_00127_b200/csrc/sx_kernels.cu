@@ -17,7 +17,7 @@ namespace sx {
 constexpr int kSegThreads = 128;
 constexpr int kWpThreads = 256;            // write kernel: threads per block
 constexpr int kWpPieces = 64;              // descriptors per tile
-constexpr int kWpBlocksPerSM = 3;
+constexpr int kWpBlocksPerSM = 4;
 
 // (b) count pass: the number of records of every segment, and the piece cache.
 // Part 1, one thread per segment of the block's tile: straight segments (2 exact offset lines + join / caps).
@@ -241,7 +241,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
                     const int idx = (pt.info & 128u) ? pt.i0 - (int)m : pt.i0 + (int)m;
                     const bool evo = ((pt.info >> 8) & 3u) == 2u;
                     tA = evo ? evolute_t(*pp, sp.evo, idx) : offset_t(*pp, (pt.info & 1024u) ? sp.off[1] : sp.off[0], eta, idx);
-                    A = normal_point(*pp, S.spiral[ss >> 1], tA, evo ? 1.0f / es_kappa(*pp, tA) : eta);
+                    A = normal_point(*pp, S.spiral[ss >> 1], tA, evo ? es_radius(*pp, tA) : eta);
                 }
                 if (last) B = end_vertex(*pp, (pt.info >> 19) & 7u, eta, cusp, &tB);
             }

@@ -65,6 +65,9 @@ SX_DEV void piece_params(Piece& p, float th0, float th1, float chord) {
 }
 
 SX_DEV float es_kappa(const Piece& p, float t) { return (p.k0 + p.k1 * (t - 0.5f)) / (p.L); }
+// radius of curvature 1/kappa(t), for evolute points (section 6): one MUFU-grade division (the evolute is
+// within |h| <= ~100 px of the curve, 2 ulp of the radius is ~1e-5 px)
+SX_DEV float es_radius(const Piece& p, float t) { return div_fast(p.L, p.k0 + p.k1 * (t - 0.5f)); }
 
 // ---------------------------------------------------------------- Euler-spiral integral (R-2)
 // Z(t) = int_0^t exp(i phi(u)) du, phi(u) = (k0-k1/2) u + k1 u^2/2.  Evaluated from a per-piece table of
@@ -202,7 +205,7 @@ SX_DEV V2 normal_point(const Piece& p, const Spiral& sp, float t, float r) {
     return g;
 }
 SX_DEV V2 es_offset(const Piece& p, const Spiral& sp, float t, float eta) { return normal_point(p, sp, t, eta); }
-SX_DEV V2 es_evolute(const Piece& p, const Spiral& sp, float t) { return normal_point(p, sp, t, 1.0f / es_kappa(p, t)); }  // section 6
+SX_DEV V2 es_evolute(const Piece& p, const Spiral& sp, float t) { return normal_point(p, sp, t, es_radius(p, t)); }  // section 6
 
 // ---------------------------------------------------------------- subdivision plans
 struct OffPlan { int n; bool uniform; float ta, tb, ua, ub; };
