@@ -114,7 +114,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    mode = MODE_OF[args.workload]
+    mode = MODE_OF[args.workload] if args.mode is None else int(args.mode == "arc")
     npaths = REF_SAMPLE_PATHS[args.workload]
     sc = make_scene(args.workload, n_paths=npaths)
     for _ in range(args.warmup):
@@ -148,7 +148,7 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(dev))
 
-    mode = MODE_OF[args.workload]
+    mode = MODE_OF[args.workload] if args.mode is None else int(args.mode == "arc")
     sc = make_scene(args.workload, n_paths=args.paths)  # replicas only: every rank expands the whole scene
     n_seg, n_paths = sc.n_segments, sc.n_paths
     tags, pts, sty = B.scene_to_torch(sc, device=dev)
@@ -262,6 +262,7 @@ def main():
     ap.add_argument("--workload", default="c4", choices=sorted(MODE_OF))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mode", default=None, choices=["line", "arc"], help="override the workload's output mode")
     ap.add_argument("--paths", type=int, default=None, help="profiling only: shrink the workload to this many paths")
     args = ap.parse_args()
     if args.impl == "reference":
