@@ -5,8 +5,8 @@
 // Euler-spiral piece as an 80-byte descriptor; the write kernel never repeats the cubic -> spiral fit.
 // It maps one thread to one OUTPUT RECORD (the per-output-point balance the paper leaves as future
 // work, L585): a block stages a tile of descriptors in shared memory, rebuilds the two side plans of
-// each piece (same device functions as the count kernel, hence the same counts), scans the plan totals
-// and lets every thread locate its record by binary search.
+// each piece (same device functions as the count kernel, hence the same counts), turns them into a
+// table of PARTS (below) and lets every thread locate its record by binary search over the parts.
 #pragma once
 #include "sx_segment.cuh"
 
@@ -15,7 +15,6 @@ namespace sx {
 constexpr uint32_t kInvalidSeg = 0xffffffffu;
 constexpr uint32_t kRelMask = 0x3fffffffu, kAt0Bit = 1u << 30, kAt1Bit = 1u << 31;
 constexpr int kDescQuads = 5;   // 5 x 16 B
-constexpr int kChunk = 32;      // descriptor slots a warp reserves per atomic
 
 SX_DEV float f_of_u(uint32_t u) { return __uint_as_float(u); }
 SX_DEV uint32_t u_of_f(float f) { return __float_as_uint(f); }
