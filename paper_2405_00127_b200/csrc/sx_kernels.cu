@@ -18,6 +18,8 @@ constexpr int kSegThreads = 128;
 constexpr int kWpThreads = 256;            // write kernel: threads per block
 constexpr int kWpPieces = 64;              // descriptors per tile
 constexpr int kWpBlocksPerSM = 4;
+constexpr int kShortSide = 2;               // records of a "short" side (scene statistic of the count kernel)
+constexpr int kDirectMax = 6;               // DIRECT variant: records of a side its own staging thread writes
 
 // (b) count pass: the number of records of every segment, and the piece cache.
 // Part 1, one thread per segment of the block's tile: straight segments (2 exact offset lines + join / caps).
@@ -28,11 +30,12 @@ constexpr int kWpBlocksPerSM = 4;
 // for its neighbours); one atomic per round reserves exactly T descriptor slots of the piece cache.
 __global__ void __launch_bounds__(kSegThreads)
 k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__ curve_idx, const uint32_t* __restrict__ n_curves_p,
-        float4* __restrict__ pieces, uint32_t piece_cap, uint32_t* piece_ctr, const uint32_t* __restrict__ err) {
+        float4* __restrict__ pieces, uint32_t piece_cap, uint32_t* piece_ctr, uint32_t* side_stats, const uint32_t* __restrict__ err) {
     __shared__ float4 s_q[kSegThreads];          // k0, k1, L, h of the round's pieces
     __shared__ uint32_t s_n[2 * kSegThreads];    // their side totals (-h, +h)
     __shared__ uint32_t s_wcnt[kSegThreads / 32];
     __shared__ uint32_t s_base;
+    __shared__ uint32_t s_stat[2];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool ok = *err == 0u;
     {   // ---- part 1: straight segments of this block's tile
@@ -56,6 +59,8 @@ k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__
     const uint32_t n_curves = ok ? *n_curves_p : 0u;
     const uint32_t rank = blockIdx.x * (uint32_t)kSegThreads + (uint32_t)tid;
     if (blockIdx.x * (uint32_t)kSegThreads >= n_curves) return;
+    if (tid < 2) s_stat[tid] = 0u;
+    uint32_t st_all = 0, st_short = 0;  // sides planned by this thread / of which one short regular range
     bool active = false;
     uint32_t i = 0, n = 0, n_tail = 0;
     Seg s;
@@ -90,7 +95,7 @@ k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__
             if (k == warp) wbase = T;
             T += s_wcnt[k];
         }
-        if (T == 0u) break;  // fit_next yields a piece every round until the curve ends
+        if (T == 0u) break;  // fit_next yields a piece every round until the curve ends (block-uniform)
         const uint32_t idx = wbase + __popc(ballot & ((1u << lane) - 1u));
         if (have) s_q[idx] = make_float4(p.k0, p.k1, p.L, h);
         if (tid == 0) s_base = atomicAdd(piece_ctr, T);
@@ -99,7 +104,10 @@ k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__
             const float4 q = s_q[j >> 1];
             Piece pp;
             pp.k0 = q.x; pp.k1 = q.y; pp.L = q.z;
-            s_n[j] = (uint32_t)side_plan(pp, (j & 1u) ? q.w : -q.w, P.mode, P.tol_fl).total;
+            const SidePlan sp = side_plan(pp, (j & 1u) ? q.w : -q.w, P.mode, P.tol_fl);
+            s_n[j] = (uint32_t)sp.total;
+            st_all++;
+            st_short += (sp.nr == 1 && !sp.sup[0] && sp.total <= kShortSide) ? 1u : 0u;
         }
         __syncthreads();
         if (have) {
@@ -108,6 +116,12 @@ k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__
             n += nm + np;
         }
     }
+    // scene statistic for the write kernel's choice of variant: how many sides are one short regular range
+    st_all = __reduce_add_sync(0xffffffffu, st_all);
+    st_short = __reduce_add_sync(0xffffffffu, st_short);
+    if (lane == 0) { atomicAdd(&s_stat[0], st_all); atomicAdd(&s_stat[1], st_short); }
+    __syncthreads();
+    if (tid < 2 && s_stat[tid]) atomicAdd(side_stats + tid, s_stat[tid]);
 }
 
 // (d1) write pass over the piece cache: one thread per output record, no per-record branching.
@@ -130,13 +144,20 @@ struct WpTile {
     uint32_t wtot[kWpSides / 32][2];
 };
 
+// Two variants, chosen on the DEVICE from the count kernel's scene statistic (both are launched, one exits at once):
+// DIRECT = true when at least 80 % of the sides are one short regular range (CAD-like scenes: 2-3 records per
+// side): such sides are then written by their own staging thread, without tables -- when (nearly) a whole warp
+// is like that.  On evolute-heavy scenes the extra path only costs registers, hence the separate instantiation.
+template <bool DIRECT>
 __global__ void __launch_bounds__(kWpThreads, kWpBlocksPerSM)
 k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, const uint32_t* __restrict__ piece_ctr,
-               const uint64_t* __restrict__ seg_off, float4* __restrict__ out, uint64_t cap_records, uint32_t* err) {
+               const uint32_t* __restrict__ side_stats, const uint64_t* __restrict__ seg_off, float4* __restrict__ out,
+               uint64_t cap_records, uint32_t* err) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WpTile& S = *reinterpret_cast<WpTile*>(smem_raw);
     const uint32_t reserved = *piece_ctr;
     if (reserved > piece_cap) return;  // cache overflow: k_write_fallback takes the whole call
+    if (((uint64_t)side_stats[1] * 10u >= (uint64_t)side_stats[0] * 8u) != DIRECT) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool arc = P.mode == kModeArc;
     for (uint32_t tile = blockIdx.x; (uint64_t)tile * kWpPieces < reserved; tile += gridDim.x) {
@@ -155,7 +176,8 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
             if (hd.seg != kInvalidSeg) piece_load(d, hd, p, &h);
         }
         const bool live = hd.seg != kInvalidSeg;
-        uint32_t nparts = 0, nrec = 0;
+        uint32_t nparts = 0, nrec = 0, ndirect = 0;
+        bool simple = false;
         uint64_t base = 0;
         if (tid < kWpSides) {
             if (live) {
@@ -164,9 +186,13 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
                 base = seg_off[hd.seg] + hd.rel + (side ? hd.n_minus : 0u);
                 if (base + nrec > cap_records) { atomicOr(err, kErrCapacity); nrec = 0; }
                 else nparts = side_part_count(sp);
+                simple = DIRECT && nparts == 1u && !sp.sup[0] && nrec <= (uint32_t)kDirectMax;
                 sp.seg = hd.seg;
                 S.plan[sub] = sp;
                 if (side == 0) S.piece[sub >> 1] = p;
+            }
+            if (DIRECT) {  // a mixed warp would wait for its few direct writers: all or (nearly) nothing
+                if (__popc(__ballot_sync(0xffffffffu, simple)) >= 28 && simple) { ndirect = nrec; nrec = 0; nparts = 0; }
             }
         } else {
             // anchor table: each of the two threads of a piece integrates one half, then they exchange totals
@@ -207,6 +233,32 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
                 side_parts(sp, (uint32_t)sub, side != 0, arc, base, er + ir - nrec, nparts, &S.part[ep + ip - nparts], &S.ppref[ep + ip - nparts]);
             }
             if (tid == 0) S.ppref[tparts] = trecs;
+            if (DIRECT && tid < kWpSides && ndirect) {
+                // vertices 0..n of the range in forward order, records stored mirrored for the +h side; the same vertex
+                // functions as phase 3, hence bit-identical records
+                const OffPlan o = S.plan[sub].off[0];
+                const Spiral& z = S.spiral[sub >> 1];
+                const float eta = side ? h : -h;
+                const float4 nocusp = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                const uint32_t kind = side ? (uint32_t)(kOffset | kPlus) : (uint32_t)kOffset;
+                float tp;
+                V2 prev = end_vertex(p, kEndT0, eta, nocusp, &tp);
+                for (uint32_t i = 1; i <= ndirect; i++) {
+                    float t;
+                    V2 cur;
+                    if (i < ndirect) { t = offset_t(p, o, eta, (int)i); cur = normal_point(p, z, t, eta); }
+                    else cur = end_vertex(p, kEndT1, eta, nocusp, &t);
+                    const uint64_t rec = base + (side ? ndirect - i : i - 1u);
+                    const V2 A = side ? cur : prev, B = side ? prev : cur;
+                    if (!arc) {
+                        out[rec] = make_float4(A.x, A.y, B.x, B.y);
+                    } else {
+                        out[2 * rec] = make_float4(A.x, A.y, B.x, B.y);
+                        out[2 * rec + 1] = make_float4((side ? es_dphi(p, t, tp) : es_dphi(p, tp, t)) + 0.0f, f_of_u(hd.seg), f_of_u(kind), 0.0f);
+                    }
+                    prev = cur; tp = t;
+                }
+            }
         }
         __syncthreads();
         // ---- phase 3: one thread per record (31 records + 1 look-ahead vertex per warp iteration)
@@ -343,6 +395,7 @@ struct sx_ctx {
 static uint32_t* ctx_err(sx_ctx* c) { return reinterpret_cast<uint32_t*>(c->sync_area); }
 static uint32_t* ctx_ticket(sx_ctx* c, int k) { return reinterpret_cast<uint32_t*>(c->sync_area) + 4 + 4 * k; }
 static uint32_t* ctx_piece_ctr(sx_ctx* c) { return reinterpret_cast<uint32_t*>(c->sync_area) + 12; }
+static uint32_t* ctx_side_stats(sx_ctx* c) { return reinterpret_cast<uint32_t*>(c->sync_area) + 14; }
 static uint32_t* ctx_n_curves(sx_ctx* c) { return reinterpret_cast<uint32_t*>(c->sync_area) + 13; }
 static uint64_t* ctx_total(sx_ctx* c) { return reinterpret_cast<uint64_t*>(c->sync_area + 64); }
 
@@ -405,7 +458,8 @@ sx_status sx_create(sx_ctx** out, int32_t device) {
     if (c->sm_count <= 0) c->sm_count = 148;
     cudaError_t e = cudaMallocHost(reinterpret_cast<void**>(&c->h_pinned), 64);
     if (e != cudaSuccess) { g_last_cuda = e; free(c); return SX_E_CUDA; }
-    e = cudaFuncSetAttribute(sx::k_write_pieces, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(sx::WpTile));
+    e = cudaFuncSetAttribute(sx::k_write_pieces<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(sx::WpTile));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sx::k_write_pieces<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(sx::WpTile));
     if (e != cudaSuccess) { g_last_cuda = e; cudaFreeHost(c->h_pinned); free(c); return SX_E_CUDA; }
     *out = c;
     return SX_OK;
@@ -475,7 +529,7 @@ sx_status sx_count(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, const floa
             sx::k_tag_scan<<<n_tag_tiles, sx::kScanThreads, 0, s>>>(d_tags, n, (uint32_t)n_points, (uint32_t)n_paths, c->pt_off, c->path_idx,
                                                                    c->sp_first, c->curve_idx, ctx_n_curves(c), tag_states, ctx_ticket(c, 0), ctx_err(c));
             sx::k_count<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(P, c->seg_count, c->curve_idx, ctx_n_curves(c), c->pieces, (uint32_t)c->piece_cap,
-                                                                                              ctx_piece_ctr(c), ctx_err(c));
+                                                                                              ctx_piece_ctr(c), ctx_side_stats(c), ctx_err(c));
             sx::k_alloc_scan<<<n_alloc_tiles, sx::kScanThreads, 0, s>>>(c->seg_count, n, d_tags, c->path_idx, (uint32_t)n_paths, c->seg_off,
                                                                       d_path_offsets, ctx_total(c), alloc_states, ctx_ticket(c, 1), ctx_err(c));
             c->launches += 3;
@@ -515,11 +569,13 @@ sx_status sx_write(sx_ctx* c, void* d_out_records, uint64_t cap_records, void* c
     SX_CUDA(cudaSetDevice(c->device));
     uint32_t n = c->P.n_tags;
     float4* out = static_cast<float4*>(d_out_records);
-    sx::k_write_pieces<<<c->sm_count * sx::kWpBlocksPerSM, sx::kWpThreads, sizeof(sx::WpTile), s>>>(c->P, c->pieces, (uint32_t)c->piece_cap, ctx_piece_ctr(c), c->seg_off,
-                                                                                 out, cap_records, ctx_err(c));
+    sx::k_write_pieces<false><<<c->sm_count * sx::kWpBlocksPerSM, sx::kWpThreads, sizeof(sx::WpTile), s>>>(
+        c->P, c->pieces, (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_side_stats(c), c->seg_off, out, cap_records, ctx_err(c));
+    sx::k_write_pieces<true><<<c->sm_count * sx::kWpBlocksPerSM, sx::kWpThreads, sizeof(sx::WpTile), s>>>(
+        c->P, c->pieces, (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_side_stats(c), c->seg_off, out, cap_records, ctx_err(c));
     sx::k_write_segments<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(c->P, c->seg_count, c->seg_off, out, cap_records,
                                                                                                (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_err(c));
-    c->launches += 2;
+    c->launches += 3;
     if (!c->cache_fits) {
         sx::k_write_fallback<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(c->P, c->seg_count, c->seg_off, out, cap_records,
                                                                                                    (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_err(c));
