@@ -59,14 +59,13 @@ SX_DEV void piece_load(const float4* slot, const PieceHead& hd, Piece& p, float*
 // record they own.  The mirror image of the +h side (reverse order, end points swapped) is folded into the
 // table when it is built.
 enum : uint32_t { kEndT0 = 0u, kEndT1 = 1u, kEndCusp = 2u, kEndEvo = 4u };  // end-vertex code: which point | evolute flag
-struct __align__(8) Part {
+struct __align__(16) Part {
     uint64_t base;   // output index of the part's first record
-    uint32_t n;      // records
-    int32_t i0;      // vertex m has subdivision index i0 + dir * m
+    uint16_t n;      // records (a single subdivision count is clamped to 65535)
+    uint16_t i0;     // vertex m has subdivision index i0 + dir * m
     uint32_t info;   // 0-6 side slot, 7 dir < 0, 8-9 src (0 none, 1 offset range, 2 evolute), 10 range, 11 arc angle wanted,
                      // 12-15 record kind, 16-18 end code of vertex 0, 19-21 end code of vertex n
-    uint32_t pad;
-};
+};  // 16 bytes
 SX_DEV uint32_t end_code(float t) { return t == 0.0f ? kEndT0 : (t == 1.0f ? kEndT1 : kEndCusp); }
 
 // number of parts of a side
@@ -90,7 +89,7 @@ SX_DEV void side_parts(const SidePlan& s, uint32_t side_slot, bool mirror, bool 
             uint32_t t = f0; f0 = f1; f1 = t;
             kind |= kPlus;
         }
-        q.base = side_base + before; q.n = n; q.i0 = i0; q.pad = 0u;
+        q.base = side_base + before; q.n = (uint16_t)n; q.i0 = (uint16_t)i0;
         q.info = side_slot | (dirneg ? 128u : 0u) | (src << 8) | (ri << 10) | ((angle && arc) ? 2048u : 0u) | (kind << 12) | (f0 << 16) | (f1 << 19);
         dst[pos] = q;
         pref[pos] = tile_prefix + before;

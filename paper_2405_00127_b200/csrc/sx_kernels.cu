@@ -286,11 +286,11 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
                 const float eta = sp.eta;
                 const float4 cusp = S.cusp[ss];
                 rec = pt.base + m; kind = (pt.info >> 12) & 15u; sg = sp.seg; want_angle = (pt.info & 2048u) != 0u;
-                last = m + 1u == pt.n;
+                last = m + 1u == (uint32_t)pt.n;
                 if (m == 0u) {
                     A = end_vertex(*pp, (pt.info >> 16) & 7u, eta, cusp, &tA);
                 } else {
-                    const int idx = (pt.info & 128u) ? pt.i0 - (int)m : pt.i0 + (int)m;
+                    const int idx = (pt.info & 128u) ? (int)pt.i0 - (int)m : (int)pt.i0 + (int)m;
                     const bool evo = ((pt.info >> 8) & 3u) == 2u;
                     tA = evo ? evolute_t(*pp, sp.evo, idx) : offset_t(*pp, (pt.info & 1024u) ? sp.off[1] : sp.off[0], eta, idx);
                     A = normal_point(*pp, S.spiral[ss >> 1], tA, evo ? es_radius(*pp, tA) : eta);
