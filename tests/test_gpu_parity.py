@@ -365,3 +365,16 @@ def test_full_size_c4_sampled(B, ctx):
 @pytest.mark.parametrize("mode", [0, 1])
 def test_full_size_c5_sampled(B, ctx, mode):
     _sampled_full_size(B, ctx, "c5", mode, 60, 9 + mode)
+
+
+def test_long_chains_tight_tolerance(B, ctx):
+    """A tolerance of 0.002 px gives sides with hundreds of records: parts much longer than the 31 records a warp takes
+    per iteration and than a tile, non-uniform (f_approx) subdivision, both write-kernel variants' table path."""
+    sc = S.make("c1", n_paths=6)
+    sc["tolerance"] = 0.002
+    for mode in (0, 1):
+        g = gpu_run(B, ctx, sc, mode)
+        r = oracle_run(sc, mode)
+        compare(sc, mode, g, r)
+        assert ck.watertight_violations(g.xy, g.path_off) == 0
+    assert g.seg_count.max() > 200
