@@ -12,7 +12,7 @@
 
 namespace sx {
 
-constexpr uint32_t kInvalidSeg = 0xffffffffu;
+constexpr uint32_t kInvalidSeg = 0xffffffffu;  // "no piece" marker of a staging thread beyond the cache's end
 constexpr uint32_t kRelMask = 0x3fffffffu, kAt0Bit = 1u << 30, kAt1Bit = 1u << 31;
 constexpr int kDescQuads = 5;   // 5 x 16 B
 
@@ -28,7 +28,6 @@ SX_DEV void piece_store(float4* slot, const Piece& p, float h, uint32_t seg, uin
     uint32_t r = (rel & kRelMask) | (p.at0 ? kAt0Bit : 0u) | (p.at1 ? kAt1Bit : 0u);
     slot[4] = make_float4(f_of_u(seg), f_of_u(r), f_of_u(n_minus), f_of_u(n_plus));
 }
-SX_DEV void piece_invalidate(float4* slot) { slot[4] = make_float4(f_of_u(kInvalidSeg), 0.0f, 0.0f, 0.0f); }
 
 struct PieceHead { uint32_t seg, rel, n_minus, n_plus; bool at0, at1; };
 SX_DEV PieceHead piece_head(const float4* slot) {

@@ -1,4 +1,6 @@
-// sx_kernels.cu -- count kernel (b), write kernel (d) and the C-ABI of include/stroke_expand.h.
+// sx_kernels.cu -- count kernel (b), the write kernels (d1 pieces, d2 segments, d3 fallback) and the C-ABI of
+// include/stroke_expand.h.  The two scans (a), (c) are in sx_scan.cuh, the curve mathematics in sx_math.cuh /
+// sx_piece.cuh, the thread-per-segment reference walk in sx_segment.cuh, the piece cache and part tables in sx_cache.cuh.
 //
 // Build: nvcc -gencode arch=compute_100a,code=sm_100a -fmad=false -lineinfo -shared (see ../build.py).
 // -fmad=false is part of the design: see the arithmetic discipline note in sx_math.cuh.
