@@ -16,7 +16,8 @@
 
 namespace sx {
 
-constexpr int kSegThreads = 128;
+constexpr int kSegThreads = 128;           // thread-per-segment kernels (d2, d3)
+constexpr int kCntThreads = 32;            // count kernel: curves (and segments) per block
 constexpr int kWpThreads = 256;            // write kernel: threads per block
 constexpr int kWpPieces = 64;              // descriptors per tile
 constexpr int kWpBlocksPerSM = 4;
@@ -30,18 +31,18 @@ constexpr int kDirectMax = 6;               // DIRECT variant: records of a side
 // its next accepted piece (fit_next, Alg. 2); the round's pieces are compacted through shared memory and
 // their 2 x T side plans are spread over ALL threads of the block (a thread whose curve is finished still plans
 // for its neighbours); one atomic per round reserves exactly T descriptor slots of the piece cache.
-__global__ void __launch_bounds__(kSegThreads)
+__global__ void __launch_bounds__(kCntThreads)
 k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__ curve_idx, const uint32_t* __restrict__ n_curves_p,
         float4* __restrict__ pieces, uint32_t piece_cap, uint32_t* piece_ctr, uint32_t* side_stats, const uint32_t* __restrict__ err) {
-    __shared__ float4 s_q[kSegThreads];          // k0, k1, L, h of the round's pieces
-    __shared__ uint32_t s_n[2 * kSegThreads];    // their side totals (-h, +h)
-    __shared__ uint32_t s_wcnt[kSegThreads / 32];
+    __shared__ float4 s_q[kCntThreads];          // k0, k1, L, h of the round's pieces
+    __shared__ uint32_t s_n[2 * kCntThreads];    // their side totals (-h, +h)
+    __shared__ uint32_t s_wcnt[kCntThreads / 32];
     __shared__ uint32_t s_base;
     __shared__ uint32_t s_stat[2];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool ok = *err == 0u;
     {   // ---- part 1: straight segments of this block's tile
-        const uint32_t i = blockIdx.x * (uint32_t)kSegThreads + (uint32_t)tid;
+        const uint32_t i = blockIdx.x * (uint32_t)kCntThreads + (uint32_t)tid;
         if (i < P.n_tags) {
             const uint32_t tag = P.tags[i];
             if (!ok) seg_count[i] = 0u;
@@ -59,8 +60,8 @@ k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__
     }
     // ---- part 2: curves
     const uint32_t n_curves = ok ? *n_curves_p : 0u;
-    const uint32_t rank = blockIdx.x * (uint32_t)kSegThreads + (uint32_t)tid;
-    if (blockIdx.x * (uint32_t)kSegThreads >= n_curves) return;
+    const uint32_t rank = blockIdx.x * (uint32_t)kCntThreads + (uint32_t)tid;
+    if (blockIdx.x * (uint32_t)kCntThreads >= n_curves) return;
     if (tid < 2) s_stat[tid] = 0u;
     uint32_t st_all = 0, st_short = 0;  // sides planned by this thread / of which one short regular range
     bool active = false;
@@ -93,7 +94,7 @@ k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__
         __syncthreads();
         uint32_t T = 0, wbase = 0;
 #pragma unroll
-        for (int k = 0; k < kSegThreads / 32; k++) {
+        for (int k = 0; k < kCntThreads / 32; k++) {
             if (k == warp) wbase = T;
             T += s_wcnt[k];
         }
@@ -102,7 +103,7 @@ k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__
         if (have) s_q[idx] = make_float4(p.k0, p.k1, p.L, h);
         if (tid == 0) s_base = atomicAdd(piece_ctr, T);
         __syncthreads();
-        for (uint32_t j = (uint32_t)tid; j < 2u * T; j += (uint32_t)kSegThreads) {
+        for (uint32_t j = (uint32_t)tid; j < 2u * T; j += (uint32_t)kCntThreads) {
             const float4 q = s_q[j >> 1];
             Piece pp;
             pp.k0 = q.x; pp.k1 = q.y; pp.L = q.z;
@@ -530,7 +531,7 @@ sx_status sx_count(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, const floa
             sx::TagTileState* tag_states = reinterpret_cast<sx::TagTileState*>(c->sync_area + 128 + round_up((uint64_t)(n_alloc_tiles + 1) * 8, 64));
             sx::k_tag_scan<<<n_tag_tiles, sx::kScanThreads, 0, s>>>(d_tags, n, (uint32_t)n_points, (uint32_t)n_paths, c->pt_off, c->path_idx,
                                                                    c->sp_first, c->curve_idx, ctx_n_curves(c), tag_states, ctx_ticket(c, 0), ctx_err(c));
-            sx::k_count<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(P, c->seg_count, c->curve_idx, ctx_n_curves(c), c->pieces, (uint32_t)c->piece_cap,
+            sx::k_count<<<(n + sx::kCntThreads - 1) / sx::kCntThreads, sx::kCntThreads, 0, s>>>(P, c->seg_count, c->curve_idx, ctx_n_curves(c), c->pieces, (uint32_t)c->piece_cap,
                                                                                               ctx_piece_ctr(c), ctx_side_stats(c), ctx_err(c));
             sx::k_alloc_scan<<<n_alloc_tiles, sx::kScanThreads, 0, s>>>(c->seg_count, n, d_tags, c->path_idx, (uint32_t)n_paths, c->seg_off,
                                                                       d_path_offsets, ctx_total(c), alloc_states, ctx_ticket(c, 1), ctx_err(c));
