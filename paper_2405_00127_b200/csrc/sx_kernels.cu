@@ -19,8 +19,7 @@ namespace sx {
 constexpr int kSegThreads = 128;           // thread-per-segment kernels (d2, d3)
 constexpr int kCntThreads = 32;            // count kernel: curves (and segments) per block
 constexpr int kWpThreads = 256;            // write kernel: threads per block
-constexpr int kWpPieces = 64;              // descriptors per tile
-constexpr int kWpBlocksPerSM = 4;
+constexpr int kWpBlocksPerSM = 3;
 constexpr int kShortSide = 2;               // records of a "short" side (scene statistic of the count kernel)
 constexpr int kDirectMax = 6;               // DIRECT variant: records of a side its own staging thread writes
 
@@ -127,47 +126,53 @@ k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__
     if (tid < 2 && s_stat[tid]) atomicAdd(side_stats + tid, s_stat[tid]);
 }
 
-// (d1) write pass over the piece cache: one thread per output record, no per-record branching.
-// A block stages a tile of kWpPieces descriptors.  Phase 1: warps 0-3, one thread per (piece, side), rebuild the
-// side plans (same device function as the count kernel, hence the same counts) while warps 4-7, one thread per
-// (piece, half), integrate the anchor table of the Euler spiral.  Phase 2: the side threads scan (parts, records),
-// evaluate the side's cusp point and write the PART table (sx_cache.cuh).  Phase 3: a warp takes 31 consecutive
-// records of the tile per iteration; lane k evaluates the START vertex of record k (lane 31 that of the next
-// record, for lane 30), the END vertex comes from the next lane by shuffle, or is a part end (no integral).
-// Records go out as 16-byte (line) or 2 x 16-byte (arc) stores to consecutive addresses.
-constexpr int kWpSides = 2 * kWpPieces;
-constexpr int kWpMaxParts = 8 * kWpSides;
-struct WpTile {
-    Piece piece[kWpPieces];
-    Spiral spiral[kWpPieces];
-    SidePlan plan[kWpSides];
-    float4 cusp[kWpSides];          // x, y, t of the side's cusp vertex
-    Part part[kWpMaxParts];
-    uint32_t ppref[kWpMaxParts + 1];
-    uint32_t wtot[kWpSides / 32][2];
+// (d1) write pass over the piece cache: one thread per output record, no per-record branching, no block barriers.
+// Every WARP works on its own tile of kWtPieces = 16 descriptors, staged in its own slice of shared memory; the
+// warps of a block never wait for one another (a block-wide tile spent a quarter of its time at its three barriers).
+//   stage   lane = (piece, side): rebuilds the side plan (same device function as the count kernel, hence the same
+//           counts), integrates its half of the piece's anchor table (the lane pair exchanges totals by shuffle),
+//           evaluates the side's cusp vertex;
+//   table   a warp scan of (parts, records) places the side's PARTS (sx_cache.cuh) in the tile's part table;
+//   write   the warp takes 31 consecutive records of the tile per iteration: lane k evaluates the START vertex of
+//           record k (lane 31 that of the next record, for lane 30); the END vertex comes from the next lane by
+//           shuffle, or is a part end (piece end point / cusp point: no integral).
+// Records go out as 16-byte (line) or 2 x 16-byte (arc) stores to consecutive addresses within a part.  A tile whose
+// sides have more than kWtParts parts in all (the worst case is 8 per side) is processed in two halves.
+constexpr int kWtPieces = 16;
+constexpr int kWtSides = 32;
+constexpr int kWtParts = 128;
+constexpr int kWpWarps = kWpThreads / 32;
+struct WarpTile {
+    Piece piece[kWtPieces];
+    Spiral spiral[kWtPieces];
+    SidePlan plan[kWtSides];
+    float4 cusp[kWtSides];          // x, y, t of the side's cusp vertex
+    Part part[kWtParts];
+    uint32_t ppref[kWtParts + 1];
+    uint32_t pad[3];
 };
 
 // Two variants, chosen on the DEVICE from the count kernel's scene statistic (both are launched, one exits at once):
 // DIRECT = true when at least 80 % of the sides are one short regular range (CAD-like scenes: 2-3 records per
-// side): such sides are then written by their own staging thread, without tables -- when (nearly) a whole warp
-// is like that.  On evolute-heavy scenes the extra path only costs registers, hence the separate instantiation.
+// side): such sides are then written by their own staging lane, without tables -- when (nearly) the whole warp is
+// like that.  On evolute-heavy scenes the extra path only costs registers, hence the separate instantiation.
 template <bool DIRECT>
 __global__ void __launch_bounds__(kWpThreads, kWpBlocksPerSM)
 k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, const uint32_t* __restrict__ piece_ctr,
                const uint32_t* __restrict__ side_stats, const uint64_t* __restrict__ seg_off, float4* __restrict__ out,
                uint64_t cap_records, uint32_t* err) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    WpTile& S = *reinterpret_cast<WpTile*>(smem_raw);
     const uint32_t reserved = *piece_ctr;
     if (reserved > piece_cap) return;  // cache overflow: k_write_fallback takes the whole call
     if (((uint64_t)side_stats[1] * 10u >= (uint64_t)side_stats[0] * 8u) != DIRECT) return;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    WarpTile& S = reinterpret_cast<WarpTile*>(smem_raw)[warp];
     const bool arc = P.mode == kModeArc;
-    for (uint32_t tile = blockIdx.x; (uint64_t)tile * kWpPieces < reserved; tile += gridDim.x) {
-        // ---- phase 1
-        const int sub = tid & (kWpSides - 1);                       // (piece, side) or (piece, half)
-        const uint32_t slot = tile * (uint32_t)kWpPieces + (uint32_t)(sub >> 1);
-        const int side = sub & 1;
+    const uint32_t n_warps = gridDim.x * (uint32_t)kWpWarps;
+    const int side = lane & 1;
+    for (uint32_t tile = blockIdx.x * (uint32_t)kWpWarps + (uint32_t)warp; (uint64_t)tile * kWtPieces < reserved; tile += n_warps) {
+        // ---- stage
+        const uint32_t slot = tile * (uint32_t)kWtPieces + (uint32_t)(lane >> 1);
         Piece p;
         p.k0 = 0.0f; p.k1 = 0.0f;
         float h = 0.0f;
@@ -176,143 +181,134 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
         if (slot < reserved) {
             const float4* d = pieces + (uint64_t)slot * kDescQuads;
             hd = piece_head(d);
-            if (hd.seg != kInvalidSeg) piece_load(d, hd, p, &h);
+            piece_load(d, hd, p, &h);
         }
         const bool live = hd.seg != kInvalidSeg;
+        const float eta = side ? h : -h;
         uint32_t nparts = 0, nrec = 0, ndirect = 0;
-        bool simple = false;
         uint64_t base = 0;
-        if (tid < kWpSides) {
-            if (live) {
-                SidePlan sp = side_plan(p, side ? h : -h, P.mode, P.tol_fl);
-                nrec = (uint32_t)sp.total;
-                base = seg_off[hd.seg] + hd.rel + (side ? hd.n_minus : 0u);
-                if (base + nrec > cap_records) { atomicOr(err, kErrCapacity); nrec = 0; }
-                else nparts = side_part_count(sp);
-                simple = DIRECT && nparts == 1u && !sp.sup[0] && nrec <= (uint32_t)kDirectMax;
-                sp.seg = hd.seg;
-                S.plan[sub] = sp;
-                if (side == 0) S.piece[sub >> 1] = p;
-            }
-            if (DIRECT) {  // a mixed warp would wait for its few direct writers: all or (nearly) nothing
-                if (__popc(__ballot_sync(0xffffffffu, simple)) >= 28 && simple) { ndirect = nrec; nrec = 0; nparts = 0; }
-            }
-        } else {
-            // anchor table: each of the two threads of a piece integrates one half, then they exchange totals
+        bool simple = false, two_ranges = false;
+        float tc = 0.0f;
+        if (live) {
+            SidePlan sp = side_plan(p, eta, P.mode, P.tol_fl);
+            nrec = (uint32_t)sp.total;
+            base = seg_off[hd.seg] + hd.rel + (side ? hd.n_minus : 0u);
+            if (base + nrec > cap_records) { atomicOr(err, kErrCapacity); nrec = 0; }
+            else nparts = side_part_count(sp);
+            simple = DIRECT && nparts == 1u && !sp.sup[0] && nrec <= (uint32_t)kDirectMax;
+            two_ranges = sp.nr == 2;
+            tc = sp.off[0].tb;
+            sp.seg = hd.seg;
+            S.plan[lane] = sp;
+            if (side == 0) S.piece[lane >> 1] = p;
+        }
+        {   // anchor table: each of the two lanes of a piece integrates one half, then they exchange totals
             const int K = es_intervals(p.k0, p.k1);
             float hx[kAnchors / 2], hy[kAnchors / 2], tx, ty;
             const int cnt = es_anchor_half(p, K, side, hx, hy, &tx, &ty);
             const float ox = __shfl_xor_sync(0xffffffffu, tx, 1), oy = __shfl_xor_sync(0xffffffffu, ty, 1);
-            if (live) es_anchor_store(S.spiral[sub >> 1], K, side, cnt, hx, hy, tx, ty, ox, oy);
+            if (live) es_anchor_store(S.spiral[lane >> 1], K, side, cnt, hx, hy, tx, ty, ox, oy);
         }
-        // ---- phase 2: scan (parts, records) over the side threads, then the part table
-        uint32_t ip = nparts, ir = nrec;
-        if (tid < kWpSides) {
-#pragma unroll
-            for (int dd = 1; dd < 32; dd <<= 1) {
-                uint32_t a = __shfl_up_sync(0xffffffffu, ip, dd), b = __shfl_up_sync(0xffffffffu, ir, dd);
-                if (lane >= dd) { ip += a; ir += b; }
-            }
-            if (lane == 31) { S.wtot[warp][0] = ip; S.wtot[warp][1] = ir; }
+        if (DIRECT) {  // a mixed warp would wait for its few direct writers: all or (nearly) nothing
+            if (__popc(__ballot_sync(0xffffffffu, simple)) >= 28 && simple) { ndirect = nrec; nrec = 0; nparts = 0; }
         }
-        __syncthreads();
-        uint32_t tparts = 0, trecs = 0;
-        {
-            uint32_t ep = 0, er = 0;
-#pragma unroll
-            for (int k = 0; k < kWpSides / 32; k++) {
-                if (k == warp) { ep = tparts; er = trecs; }
-                tparts += S.wtot[k][0]; trecs += S.wtot[k][1];
-            }
-            if (tid < kWpSides && nparts) {
-                const SidePlan& sp = S.plan[sub];
-                const float eta = side ? h : -h;
-                // the side's cusp vertex: the parallel curve at the cusp parameter (L380-386), evaluated once
-                const float tc = sp.nr == 2 ? sp.off[0].tb : (sp.cusp_b ? sp.off[0].tb : 0.0f);
-                if (tc != 0.0f && tc != 1.0f) {
-                    V2 c = normal_point(p, S.spiral[sub >> 1], tc, eta);
-                    S.cusp[sub] = make_float4(c.x, c.y, tc, 0.0f);
-                }
-                side_parts(sp, (uint32_t)sub, side != 0, arc, base, er + ir - nrec, nparts, &S.part[ep + ip - nparts], &S.ppref[ep + ip - nparts]);
-            }
-            if (tid == 0) S.ppref[tparts] = trecs;
-            if (DIRECT && tid < kWpSides && ndirect) {
-                // vertices 0..n of the range in forward order, records stored mirrored for the +h side; the same vertex
-                // functions as phase 3, hence bit-identical records
-                const OffPlan o = S.plan[sub].off[0];
-                const Spiral& z = S.spiral[sub >> 1];
-                const float eta = side ? h : -h;
-                const float4 nocusp = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-                const uint32_t kind = side ? (uint32_t)(kOffset | kPlus) : (uint32_t)kOffset;
-                float tp;
-                V2 prev = end_vertex(p, kEndT0, eta, nocusp, &tp);
-                for (uint32_t i = 1; i <= ndirect; i++) {
-                    float t;
-                    V2 cur;
-                    if (i < ndirect) { t = offset_t(p, o, eta, (int)i); cur = normal_point(p, z, t, eta); }
-                    else cur = end_vertex(p, kEndT1, eta, nocusp, &t);
-                    const uint64_t rec = base + (side ? ndirect - i : i - 1u);
-                    const V2 A = side ? cur : prev, B = side ? prev : cur;
-                    if (!arc) {
-                        out[rec] = make_float4(A.x, A.y, B.x, B.y);
-                    } else {
-                        out[2 * rec] = make_float4(A.x, A.y, B.x, B.y);
-                        out[2 * rec + 1] = make_float4((side ? es_dphi(p, t, tp) : es_dphi(p, tp, t)) + 0.0f, f_of_u(hd.seg), f_of_u(kind), 0.0f);
-                    }
-                    prev = cur; tp = t;
-                }
-            }
+        __syncwarp();
+        // the side's cusp vertex: the parallel curve at the cusp parameter (L380-386), evaluated once and shared by the
+        // parts that meet there (a side has a cusp iff it has two ranges)
+        if (live && two_ranges) {
+            V2 c = normal_point(p, S.spiral[lane >> 1], tc, eta);
+            S.cusp[lane] = make_float4(c.x, c.y, tc, 0.0f);
         }
-        __syncthreads();
-        // ---- phase 3: one thread per record (31 records + 1 look-ahead vertex per warp iteration)
-        for (uint32_t q = (uint32_t)warp; q * 31u < trecs; q += (uint32_t)(kWpThreads / 32)) {
-            const uint32_t r = q * 31u + (uint32_t)lane;
-            const bool act = r < trecs;
-            V2 A = v2(0.0f, 0.0f), B = A;
-            float tA = 0.0f, tB = 0.0f;
-            bool last = true, want_angle = false;
-            uint64_t rec = 0;
-            uint32_t kind = 0, sg = 0;
-            const Piece* pp = &S.piece[0];
-            if (act) {
-                uint32_t lo = 0, hi = tparts;  // largest part with ppref <= r
-#pragma unroll 1
-                while (hi - lo > 1u) {
-                    uint32_t mid = (lo + hi) >> 1;
-                    if (S.ppref[mid] <= r) lo = mid; else hi = mid;
-                }
-                const Part pt = S.part[lo];
-                const uint32_t m = r - S.ppref[lo];
-                const uint32_t ss = pt.info & 127u;
-                pp = &S.piece[ss >> 1];
-                const SidePlan& sp = S.plan[ss];
-                const float eta = sp.eta;
-                const float4 cusp = S.cusp[ss];
-                rec = pt.base + m; kind = (pt.info >> 12) & 15u; sg = sp.seg; want_angle = (pt.info & 2048u) != 0u;
-                last = m + 1u == (uint32_t)pt.n;
-                if (m == 0u) {
-                    A = end_vertex(*pp, (pt.info >> 16) & 7u, eta, cusp, &tA);
-                } else {
-                    const int idx = (pt.info & 128u) ? (int)pt.i0 - (int)m : (int)pt.i0 + (int)m;
-                    const bool evo = ((pt.info >> 8) & 3u) == 2u;
-                    tA = evo ? evolute_t(*pp, sp.evo, idx) : offset_t(*pp, (pt.info & 1024u) ? sp.off[1] : sp.off[0], eta, idx);
-                    A = normal_point(*pp, S.spiral[ss >> 1], tA, evo ? es_radius(*pp, tA) : eta);
-                }
-                if (last) B = end_vertex(*pp, (pt.info >> 19) & 7u, eta, cusp, &tB);
-            }
-            const float nx = __shfl_down_sync(0xffffffffu, A.x, 1), ny = __shfl_down_sync(0xffffffffu, A.y, 1), nt = __shfl_down_sync(0xffffffffu, tA, 1);
-            if (!last) { B = v2(nx, ny); tB = nt; }
-            if (act && lane < 31) {
+        if (DIRECT && ndirect) {
+            // vertices 0..n of the range in forward order, records stored mirrored for the +h side; the same vertex
+            // functions as the table path, hence bit-identical records
+            const OffPlan o = S.plan[lane].off[0];
+            const Spiral& z = S.spiral[lane >> 1];
+            const float4 nocusp = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            const uint32_t kind = side ? (uint32_t)(kOffset | kPlus) : (uint32_t)kOffset;
+            float tp;
+            V2 prev = end_vertex(p, kEndT0, eta, nocusp, &tp);
+            for (uint32_t i = 1; i <= ndirect; i++) {
+                float t;
+                V2 cur;
+                if (i < ndirect) { t = offset_t(p, o, eta, (int)i); cur = normal_point(p, z, t, eta); }
+                else cur = end_vertex(p, kEndT1, eta, nocusp, &t);
+                const uint64_t rec = base + (side ? ndirect - i : i - 1u);
+                const V2 A = side ? cur : prev, B = side ? prev : cur;
                 if (!arc) {
                     out[rec] = make_float4(A.x, A.y, B.x, B.y);
                 } else {
                     out[2 * rec] = make_float4(A.x, A.y, B.x, B.y);
-                    out[2 * rec + 1] = make_float4(want_angle ? es_dphi(*pp, tA, tB) + 0.0f : 0.0f,  // + 0: no negative zero
-                                                 f_of_u(sg), f_of_u(kind), 0.0f);
+                    out[2 * rec + 1] = make_float4((side ? es_dphi(p, t, tp) : es_dphi(p, tp, t)) + 0.0f, f_of_u(hd.seg), f_of_u(kind), 0.0f);
                 }
+                prev = cur; tp = t;
             }
         }
-        __syncthreads();
+        // ---- table + write, in one pass, or in two halves of the warp's sides when the parts do not fit
+        const uint32_t all_parts = __reduce_add_sync(0xffffffffu, nparts);
+        const int n_pass = all_parts > (uint32_t)kWtParts ? 2 : 1;
+        for (int pass = 0; pass < n_pass; pass++) {
+            const bool mine = n_pass == 1 || (lane >> 4) == pass;
+            const uint32_t np_ = mine ? nparts : 0u, nr_ = mine ? nrec : 0u;
+            uint32_t ip = np_, ir = nr_;
+#pragma unroll
+            for (int dd = 1; dd < 32; dd <<= 1) {
+                uint32_t a2 = __shfl_up_sync(0xffffffffu, ip, dd), b2 = __shfl_up_sync(0xffffffffu, ir, dd);
+                if (lane >= dd) { ip += a2; ir += b2; }
+            }
+            const uint32_t tparts = __shfl_sync(0xffffffffu, ip, 31), trecs = __shfl_sync(0xffffffffu, ir, 31);
+            if (np_) side_parts(S.plan[lane], (uint32_t)lane, side != 0, arc, base, ir - nr_, np_, &S.part[ip - np_], &S.ppref[ip - np_]);
+            if (lane == 0) S.ppref[tparts] = trecs;
+            __syncwarp();
+            for (uint32_t q = 0; q * 31u < trecs; q++) {
+                const uint32_t r = q * 31u + (uint32_t)lane;
+                const bool act = r < trecs;
+                V2 A = v2(0.0f, 0.0f), B = A;
+                float tA = 0.0f, tB = 0.0f;
+                bool last = true, want_angle = false;
+                uint64_t rec = 0;
+                uint32_t kind = 0, sg = 0;
+                const Piece* pp = &S.piece[0];
+                if (act) {
+                    uint32_t lo = 0, hi = tparts;  // largest part with ppref <= r
+#pragma unroll 1
+                    while (hi - lo > 1u) {
+                        uint32_t mid = (lo + hi) >> 1;
+                        if (S.ppref[mid] <= r) lo = mid; else hi = mid;
+                    }
+                    const Part pt = S.part[lo];
+                    const uint32_t m = r - S.ppref[lo];
+                    const uint32_t ss = pt.info & 127u;
+                    pp = &S.piece[ss >> 1];
+                    const SidePlan& sp = S.plan[ss];
+                    const float e2 = sp.eta;
+                    const float4 cusp = S.cusp[ss];
+                    rec = pt.base + m; kind = (pt.info >> 12) & 15u; sg = sp.seg; want_angle = (pt.info & 2048u) != 0u;
+                    last = m + 1u == (uint32_t)pt.n;
+                    if (m == 0u) {
+                        A = end_vertex(*pp, (pt.info >> 16) & 7u, e2, cusp, &tA);
+                    } else {
+                        const int idx = (pt.info & 128u) ? (int)pt.i0 - (int)m : (int)pt.i0 + (int)m;
+                        const bool evo = ((pt.info >> 8) & 3u) == 2u;
+                        tA = evo ? evolute_t(*pp, sp.evo, idx) : offset_t(*pp, (pt.info & 1024u) ? sp.off[1] : sp.off[0], e2, idx);
+                        A = normal_point(*pp, S.spiral[ss >> 1], tA, evo ? es_radius(*pp, tA) : e2);
+                    }
+                    if (last) B = end_vertex(*pp, (pt.info >> 19) & 7u, e2, cusp, &tB);
+                }
+                const float nx = __shfl_down_sync(0xffffffffu, A.x, 1), ny = __shfl_down_sync(0xffffffffu, A.y, 1), nt = __shfl_down_sync(0xffffffffu, tA, 1);
+                if (!last) { B = v2(nx, ny); tB = nt; }
+                if (act && lane < 31) {
+                    if (!arc) {
+                        out[rec] = make_float4(A.x, A.y, B.x, B.y);
+                    } else {
+                        out[2 * rec] = make_float4(A.x, A.y, B.x, B.y);
+                        out[2 * rec + 1] = make_float4(want_angle ? es_dphi(*pp, tA, tB) + 0.0f : 0.0f,  // + 0: no negative zero
+                                                     f_of_u(sg), f_of_u(kind), 0.0f);
+                    }
+                }
+            }
+            __syncwarp();
+        }
     }
 }
 
@@ -461,8 +457,8 @@ sx_status sx_create(sx_ctx** out, int32_t device) {
     if (c->sm_count <= 0) c->sm_count = 148;
     cudaError_t e = cudaMallocHost(reinterpret_cast<void**>(&c->h_pinned), 64);
     if (e != cudaSuccess) { g_last_cuda = e; free(c); return SX_E_CUDA; }
-    e = cudaFuncSetAttribute(sx::k_write_pieces<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(sx::WpTile));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sx::k_write_pieces<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(sx::WpTile));
+    e = cudaFuncSetAttribute(sx::k_write_pieces<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sx::kWpWarps * sizeof(sx::WarpTile)));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sx::k_write_pieces<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sx::kWpWarps * sizeof(sx::WarpTile)));
     if (e != cudaSuccess) { g_last_cuda = e; cudaFreeHost(c->h_pinned); free(c); return SX_E_CUDA; }
     *out = c;
     return SX_OK;
@@ -572,9 +568,9 @@ sx_status sx_write(sx_ctx* c, void* d_out_records, uint64_t cap_records, void* c
     SX_CUDA(cudaSetDevice(c->device));
     uint32_t n = c->P.n_tags;
     float4* out = static_cast<float4*>(d_out_records);
-    sx::k_write_pieces<false><<<c->sm_count * sx::kWpBlocksPerSM, sx::kWpThreads, sizeof(sx::WpTile), s>>>(
+    sx::k_write_pieces<false><<<c->sm_count * sx::kWpBlocksPerSM, sx::kWpThreads, sx::kWpWarps * sizeof(sx::WarpTile), s>>>(
         c->P, c->pieces, (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_side_stats(c), c->seg_off, out, cap_records, ctx_err(c));
-    sx::k_write_pieces<true><<<c->sm_count * sx::kWpBlocksPerSM, sx::kWpThreads, sizeof(sx::WpTile), s>>>(
+    sx::k_write_pieces<true><<<c->sm_count * sx::kWpBlocksPerSM, sx::kWpThreads, sx::kWpWarps * sizeof(sx::WarpTile), s>>>(
         c->P, c->pieces, (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_side_stats(c), c->seg_off, out, cap_records, ctx_err(c));
     sx::k_write_segments<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(c->P, c->seg_count, c->seg_off, out, cap_records,
                                                                                                (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_err(c));
