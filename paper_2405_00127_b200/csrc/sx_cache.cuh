@@ -49,6 +49,57 @@ SX_DEV void piece_load(const float4* slot, const PieceHead& hd, Piece& p, float*
     p.at0 = hd.at0; p.at1 = hd.at1;
 }
 
+// ---------------------------------------------------------------- the side plan as the writer keeps it in shared memory
+// 52 bytes instead of sizeof(SidePlan) = 100: range bounds are implied by the cusp parameter (range 0 = [0, tc],
+// range 1 = [tc, 1]; the super-critical range is range 0 iff sup0), counts fit 16 bits.
+struct PlanLite {
+    float eta, tc;
+    uint32_t seg, total;
+    uint16_t n0, n1, ne;
+    uint8_t flags;   // 0 two ranges, 1 sup0, 2 sup1, 3 uniform0, 4 uniform1, 5 uniform evolute
+    uint8_t pad;
+    float ua0, ub0, ua1, ub1, wa, wb, skp;
+};
+SX_DEV PlanLite plan_pack(const SidePlan& s) {
+    PlanLite q;
+    q.eta = s.eta; q.tc = s.off[0].tb; q.seg = s.seg; q.total = (uint32_t)s.total;
+    q.n0 = (uint16_t)s.off[0].n; q.n1 = (uint16_t)s.off[1].n; q.ne = (uint16_t)s.evo.n;
+    q.flags = (uint8_t)((s.nr == 2 ? 1u : 0u) | (s.sup[0] ? 2u : 0u) | (s.sup[1] ? 4u : 0u) | (s.off[0].uniform ? 8u : 0u) |
+                        (s.off[1].uniform ? 16u : 0u) | (s.evo.uniform ? 32u : 0u));
+    q.pad = 0;
+    q.ua0 = s.off[0].ua; q.ub0 = s.off[0].ub; q.ua1 = s.off[1].ua; q.ub1 = s.off[1].ub;
+    q.wa = s.evo.wa; q.wb = s.evo.wb; q.skp = s.evo.skp;
+    return q;
+}
+SX_DEV OffPlan plan_off(const PlanLite& q, bool second) {
+    OffPlan o;
+    o.n = second ? q.n1 : q.n0;
+    o.uniform = (q.flags & (second ? 16u : 8u)) != 0u;
+    o.ta = second ? q.tc : 0.0f; o.tb = second ? 1.0f : q.tc;
+    o.ua = second ? q.ua1 : q.ua0; o.ub = second ? q.ub1 : q.ub0;
+    return o;
+}
+SX_DEV EvoPlan plan_evo(const PlanLite& q);
+// the fields of the SidePlan that the part table is built from
+SX_DEV SidePlan plan_unpack(const PlanLite& q) {
+    SidePlan s;
+    s.eta = q.eta; s.seg = q.seg; s.total = (int)q.total;
+    s.nr = (q.flags & 1u) ? 2 : 1;
+    s.sup[0] = (q.flags & 2u) != 0u; s.sup[1] = (q.flags & 4u) != 0u;
+    s.off[0] = plan_off(q, false); s.off[1] = plan_off(q, true);
+    s.evo = plan_evo(q);
+    s.cusp_a = s.evo.ta != 0.0f; s.cusp_b = s.evo.tb != 1.0f;
+    return s;
+}
+SX_DEV EvoPlan plan_evo(const PlanLite& q) {
+    EvoPlan e;
+    const bool second = (q.flags & 1u) && !(q.flags & 2u);  // two ranges and the first one regular
+    e.n = q.ne; e.uniform = (q.flags & 32u) != 0u;
+    e.ta = second ? q.tc : 0.0f; e.tb = second ? 1.0f : q.tc;
+    e.wa = q.wa; e.wb = q.wb; e.skp = q.skp;
+    return e;
+}
+
 // ---------------------------------------------------------------- parts
 // The records of one side of one piece, in OUTPUT order, are a short list of PARTS (at most 8): chains of n
 // records over n+1 vertices.  Vertex m of a part is either one of the part's two END vertices -- a piece end

@@ -19,7 +19,7 @@ namespace sx {
 constexpr int kSegThreads = 128;           // thread-per-segment kernels (d2, d3)
 constexpr int kCntThreads = 32;            // count kernel: curves (and segments) per block
 constexpr int kWpThreads = 256;            // write kernel: threads per block
-constexpr int kWpBlocksPerSM = 3;
+constexpr int kWpBlocksPerSM = 4;
 constexpr int kShortSide = 2;               // records of a "short" side (scene statistic of the count kernel)
 constexpr int kDirectMax = 6;               // DIRECT variant: records of a side its own staging thread writes
 
@@ -137,15 +137,16 @@ k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__
 //           record k (lane 31 that of the next record, for lane 30); the END vertex comes from the next lane by
 //           shuffle, or is a part end (piece end point / cusp point: no integral).
 // Records go out as 16-byte (line) or 2 x 16-byte (arc) stores to consecutive addresses within a part.  A tile whose
-// sides have more than kWtParts parts in all (the worst case is 8 per side) is processed in two halves.
+// sides have more than kWtParts parts in all (the worst case is 8 per side) is processed in two halves or four
+// quarters of its sides.
 constexpr int kWtPieces = 16;
 constexpr int kWtSides = 32;
-constexpr int kWtParts = 128;
+constexpr int kWtParts = 96;
 constexpr int kWpWarps = kWpThreads / 32;
 struct WarpTile {
     Piece piece[kWtPieces];
     Spiral spiral[kWtPieces];
-    SidePlan plan[kWtSides];
+    PlanLite plan[kWtSides];
     float4 cusp[kWtSides];          // x, y, t of the side's cusp vertex
     Part part[kWtParts];
     uint32_t ppref[kWtParts + 1];
@@ -199,7 +200,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
             two_ranges = sp.nr == 2;
             tc = sp.off[0].tb;
             sp.seg = hd.seg;
-            S.plan[lane] = sp;
+            S.plan[lane] = plan_pack(sp);
             if (side == 0) S.piece[lane >> 1] = p;
         }
         {   // anchor table: each of the two lanes of a piece integrates one half, then they exchange totals
@@ -222,7 +223,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
         if (DIRECT && ndirect) {
             // vertices 0..n of the range in forward order, records stored mirrored for the +h side; the same vertex
             // functions as the table path, hence bit-identical records
-            const OffPlan o = S.plan[lane].off[0];
+            const OffPlan o = plan_off(S.plan[lane], false);
             const Spiral& z = S.spiral[lane >> 1];
             const float4 nocusp = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
             const uint32_t kind = side ? (uint32_t)(kOffset | kPlus) : (uint32_t)kOffset;
@@ -246,9 +247,12 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
         }
         // ---- table + write, in one pass, or in two halves of the warp's sides when the parts do not fit
         const uint32_t all_parts = __reduce_add_sync(0xffffffffu, nparts);
-        const int n_pass = all_parts > (uint32_t)kWtParts ? 2 : 1;
+        const uint32_t low_parts = __reduce_add_sync(0xffffffffu, lane < 16 ? nparts : 0u);
+        // 1 pass; or the two halves of the warp's sides; or its four quarters (8 sides x 8 parts always fit)
+        const int n_pass = all_parts <= (uint32_t)kWtParts ? 1 : ((low_parts <= (uint32_t)kWtParts && all_parts - low_parts <= (uint32_t)kWtParts) ? 2 : 4);
+        const int pass_shift = n_pass == 2 ? 4 : 3;
         for (int pass = 0; pass < n_pass; pass++) {
-            const bool mine = n_pass == 1 || (lane >> 4) == pass;
+            const bool mine = n_pass == 1 || (lane >> pass_shift) == pass;
             const uint32_t np_ = mine ? nparts : 0u, nr_ = mine ? nrec : 0u;
             uint32_t ip = np_, ir = nr_;
 #pragma unroll
@@ -257,7 +261,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
                 if (lane >= dd) { ip += a2; ir += b2; }
             }
             const uint32_t tparts = __shfl_sync(0xffffffffu, ip, 31), trecs = __shfl_sync(0xffffffffu, ir, 31);
-            if (np_) side_parts(S.plan[lane], (uint32_t)lane, side != 0, arc, base, ir - nr_, np_, &S.part[ip - np_], &S.ppref[ip - np_]);
+            if (np_) side_parts(plan_unpack(S.plan[lane]), (uint32_t)lane, side != 0, arc, base, ir - nr_, np_, &S.part[ip - np_], &S.ppref[ip - np_]);
             if (lane == 0) S.ppref[tparts] = trecs;
             __syncwarp();
             for (uint32_t q = 0; q * 31u < trecs; q++) {
@@ -280,7 +284,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
                     const uint32_t m = r - S.ppref[lo];
                     const uint32_t ss = pt.info & 127u;
                     pp = &S.piece[ss >> 1];
-                    const SidePlan& sp = S.plan[ss];
+                    const PlanLite& sp = S.plan[ss];
                     const float e2 = sp.eta;
                     const float4 cusp = S.cusp[ss];
                     rec = pt.base + m; kind = (pt.info >> 12) & 15u; sg = sp.seg; want_angle = (pt.info & 2048u) != 0u;
@@ -290,7 +294,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
                     } else {
                         const int idx = (pt.info & 128u) ? (int)pt.i0 - (int)m : (int)pt.i0 + (int)m;
                         const bool evo = ((pt.info >> 8) & 3u) == 2u;
-                        tA = evo ? evolute_t(*pp, sp.evo, idx) : offset_t(*pp, (pt.info & 1024u) ? sp.off[1] : sp.off[0], e2, idx);
+                        tA = evo ? evolute_t(*pp, plan_evo(sp), idx) : offset_t(*pp, plan_off(sp, (pt.info & 1024u) != 0u), e2, idx);
                         A = normal_point(*pp, S.spiral[ss >> 1], tA, evo ? es_radius(*pp, tA) : e2);
                     }
                     if (last) B = end_vertex(*pp, (pt.info >> 19) & 7u, e2, cusp, &tB);
