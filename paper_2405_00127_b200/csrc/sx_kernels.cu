@@ -18,7 +18,7 @@ namespace sx {
 
 constexpr int kSegThreads = 128;           // thread-per-segment kernels (d2, d3)
 constexpr int kCntThreads = 32;            // count kernel: curves (and segments) per block
-constexpr int kWpThreads = 256;            // write kernel: threads per block
+constexpr int kWpThreads = 224;            // write kernel: threads per block (7 independent warps)
 constexpr int kWpBlocksPerSM = 4;
 constexpr int kShortSide = 2;               // records of a "short" side (scene statistic of the count kernel)
 constexpr int kDirectMax = 6;               // DIRECT variant: records of a side its own staging thread writes
@@ -142,6 +142,7 @@ k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__
 constexpr int kWtPieces = 16;
 constexpr int kWtSides = 32;
 constexpr int kWtParts = 96;
+constexpr int kRing = 64;                  // >= 2 x 32: see the write loop
 constexpr int kWpWarps = kWpThreads / 32;
 struct WarpTile {
     Piece piece[kWtPieces];
@@ -151,6 +152,7 @@ struct WarpTile {
     Part part[kWtParts];
     uint32_t ppref[kWtParts + 1];
     uint32_t pad[3];
+    float4 ring[kRing];             // x, y, t of the interior vertices just ahead of the records being written
 };
 
 // Two variants, chosen on the DEVICE from the count kernel's scene statistic (both are launched, one exits at once):
@@ -264,52 +266,78 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
             if (np_) side_parts(plan_unpack(S.plan[lane]), (uint32_t)lane, side != 0, arc, base, ir - nr_, np_, &S.part[ip - np_], &S.ppref[ip - np_]);
             if (lane == 0) S.ppref[tparts] = trecs;
             __syncwarp();
-            for (uint32_t q = 0; q * 31u < trecs; q++) {
-                const uint32_t r = q * 31u + (uint32_t)lane;
+            // ---- write: 32 records per iteration.  Record r of part i (its m-th) starts at the part's vertex m and ends
+            // at vertex m + 1.  The INTERIOR vertices of all parts, in record order, have the running index
+            // v = r - i - 1 (start) / r - i (end): they are evaluated densely, 32 at a time by all lanes, into a ring of
+            // kRing entries just ahead of the records that use them (both neighbours read the same bits); part ends are
+            // piece end points or the cusp point and cost no integral.
+            const uint32_t tverts = trecs - tparts;
+            uint32_t v_done = 0;
+            for (uint32_t r0 = 0; r0 < trecs; r0 += 32u) {
+                const uint32_t r = r0 + (uint32_t)lane;
                 const bool act = r < trecs;
-                V2 A = v2(0.0f, 0.0f), B = A;
-                float tA = 0.0f, tB = 0.0f;
-                bool last = true, want_angle = false;
-                uint64_t rec = 0;
-                uint32_t kind = 0, sg = 0;
-                const Piece* pp = &S.piece[0];
+                uint32_t lo = 0;
+                Part pt;
+                pt.base = 0; pt.n = 1; pt.i0 = 0; pt.info = 0;
+                uint32_t m = 0;
                 if (act) {
-                    uint32_t lo = 0, hi = tparts;  // largest part with ppref <= r
+                    uint32_t hi = tparts;  // largest part with ppref <= r
 #pragma unroll 1
                     while (hi - lo > 1u) {
                         uint32_t mid = (lo + hi) >> 1;
                         if (S.ppref[mid] <= r) lo = mid; else hi = mid;
                     }
-                    const Part pt = S.part[lo];
-                    const uint32_t m = r - S.ppref[lo];
-                    const uint32_t ss = pt.info & 127u;
-                    pp = &S.piece[ss >> 1];
-                    const PlanLite& sp = S.plan[ss];
-                    const float e2 = sp.eta;
-                    const float4 cusp = S.cusp[ss];
-                    rec = pt.base + m; kind = (pt.info >> 12) & 15u; sg = sp.seg; want_angle = (pt.info & 2048u) != 0u;
-                    last = m + 1u == (uint32_t)pt.n;
-                    if (m == 0u) {
-                        A = end_vertex(*pp, (pt.info >> 16) & 7u, e2, cusp, &tA);
-                    } else {
-                        const int idx = (pt.info & 128u) ? (int)pt.i0 - (int)m : (int)pt.i0 + (int)m;
-                        const bool evo = ((pt.info >> 8) & 3u) == 2u;
-                        tA = evo ? evolute_t(*pp, plan_evo(sp), idx) : offset_t(*pp, plan_off(sp, (pt.info & 1024u) != 0u), e2, idx);
-                        A = normal_point(*pp, S.spiral[ss >> 1], tA, evo ? es_radius(*pp, tA) : e2);
-                    }
-                    if (last) B = end_vertex(*pp, (pt.info >> 19) & 7u, e2, cusp, &tB);
+                    pt = S.part[lo];
+                    m = r - S.ppref[lo];
                 }
-                const float nx = __shfl_down_sync(0xffffffffu, A.x, 1), ny = __shfl_down_sync(0xffffffffu, A.y, 1), nt = __shfl_down_sync(0xffffffffu, tA, 1);
-                if (!last) { B = v2(nx, ny); tB = nt; }
-                if (act && lane < 31) {
+                const bool s_int = act && m >= 1u, e_int = act && m + 1u < (uint32_t)pt.n;
+                const int v_end = (int)(r - lo);  // index of the record's end vertex if interior; the start vertex is v_end - 1
+                const int need = e_int ? v_end : (s_int ? v_end - 1 : -1);
+                const int need_max = __reduce_max_sync(0xffffffffu, need);
+                while ((int)v_done <= need_max) {
+                    const uint32_t v = v_done + (uint32_t)lane;
+                    if (v < tverts) {
+                        uint32_t l2 = 0, h2 = tparts;  // largest part j with ppref[j] - j <= v: the part that owns vertex v
+#pragma unroll 1
+                        while (h2 - l2 > 1u) {
+                            uint32_t mid = (l2 + h2) >> 1;
+                            if (S.ppref[mid] - mid <= v) l2 = mid; else h2 = mid;
+                        }
+                        const Part pj = S.part[l2];
+                        const uint32_t mm = v - (S.ppref[l2] - l2) + 1u;
+                        const uint32_t ss = pj.info & 127u;
+                        const Piece& pc = S.piece[ss >> 1];
+                        const PlanLite& sp = S.plan[ss];
+                        const int idx = (pj.info & 128u) ? (int)pj.i0 - (int)mm : (int)pj.i0 + (int)mm;
+                        const bool evo = ((pj.info >> 8) & 3u) == 2u;
+                        const float t = evo ? evolute_t(pc, plan_evo(sp), idx) : offset_t(pc, plan_off(sp, (pj.info & 1024u) != 0u), sp.eta, idx);
+                        const V2 g = normal_point(pc, S.spiral[ss >> 1], t, evo ? es_radius(pc, t) : sp.eta);
+                        S.ring[v & (uint32_t)(kRing - 1)] = make_float4(g.x, g.y, t, 0.0f);
+                    }
+                    v_done += 32u;
+                    __syncwarp();
+                }
+                if (act) {
+                    const uint32_t ss = pt.info & 127u;
+                    const Piece& pc = S.piece[ss >> 1];
+                    const PlanLite& sp = S.plan[ss];
+                    const float4 cusp = S.cusp[ss];
+                    V2 A, B;
+                    float tA, tB;
+                    if (s_int) { const float4 q = S.ring[(uint32_t)(v_end - 1) & (uint32_t)(kRing - 1)]; A = v2(q.x, q.y); tA = q.z; }
+                    else A = end_vertex(pc, (pt.info >> 16) & 7u, sp.eta, cusp, &tA);
+                    if (e_int) { const float4 q = S.ring[(uint32_t)v_end & (uint32_t)(kRing - 1)]; B = v2(q.x, q.y); tB = q.z; }
+                    else B = end_vertex(pc, (pt.info >> 19) & 7u, sp.eta, cusp, &tB);
+                    const uint64_t rec = pt.base + m;
                     if (!arc) {
                         out[rec] = make_float4(A.x, A.y, B.x, B.y);
                     } else {
                         out[2 * rec] = make_float4(A.x, A.y, B.x, B.y);
-                        out[2 * rec + 1] = make_float4(want_angle ? es_dphi(*pp, tA, tB) + 0.0f : 0.0f,  // + 0: no negative zero
-                                                     f_of_u(sg), f_of_u(kind), 0.0f);
+                        out[2 * rec + 1] = make_float4((pt.info & 2048u) ? es_dphi(pc, tA, tB) + 0.0f : 0.0f,  // + 0: no negative zero
+                                                     f_of_u(sp.seg), f_of_u((pt.info >> 12) & 15u), 0.0f);
                     }
                 }
+                __syncwarp();
             }
             __syncwarp();
         }
