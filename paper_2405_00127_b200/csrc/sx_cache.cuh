@@ -145,9 +145,8 @@ SX_DEV void side_parts(const SidePlan& s, uint32_t side_slot, bool mirror, bool 
         pref[pos] = tile_prefix + before;
         idx++; fwd += n;
     };
-#pragma unroll
-    for (int r = 0; r < 2; r++) {
-        if (r >= s.nr) break;
+#pragma unroll 1
+    for (int r = 0; r < s.nr; r++) {
         const OffPlan o = r == 0 ? s.off[0] : s.off[1];
         const bool sup = r == 0 ? s.sup[0] : s.sup[1];
         const uint32_t ca = end_code(o.ta), cb = end_code(o.tb);
@@ -155,13 +154,15 @@ SX_DEV void side_parts(const SidePlan& s, uint32_t side_slot, bool mirror, bool 
             push((uint32_t)o.n, 0, false, 1u, (uint32_t)r, true, kOffset, ca, cb);
         } else {
             // evolute patch (section 6): connectors x2, evolute x2, reversed offset, connectors x2;
-            // the evolute meets the offset curve at the cusp
+            // the evolute meets the offset curve at the cusp.  (Loops, not copies: code size.)
             const uint32_t ea = s.cusp_a ? (uint32_t)kEndCusp : (ca | kEndEvo), eb = s.cusp_b ? (uint32_t)kEndCusp : (cb | kEndEvo);
-            if (!s.cusp_a) { push(1u, 0, false, 0u, 0u, false, kConnector, ca, ea); push(1u, 0, false, 0u, 0u, false, kConnector, ca, ea); }
-            push((uint32_t)s.evo.n, 0, false, 2u, 0u, false, kEvolute, ea, eb);
-            push((uint32_t)s.evo.n, 0, false, 2u, 0u, false, kEvolute, ea, eb);
+#pragma unroll 1
+            for (int c = 0; c < (s.cusp_a ? 0 : 2); c++) push(1u, 0, false, 0u, 0u, false, kConnector, ca, ea);
+#pragma unroll 1
+            for (int c = 0; c < 2; c++) push((uint32_t)s.evo.n, 0, false, 2u, 0u, false, kEvolute, ea, eb);
             push((uint32_t)o.n, o.n, true, 1u, (uint32_t)r, true, kOffsetRev, cb, ca);  // L403, L191
-            if (!s.cusp_b) { push(1u, 0, false, 0u, 0u, false, kConnector, eb, cb); push(1u, 0, false, 0u, 0u, false, kConnector, eb, cb); }
+#pragma unroll 1
+            for (int c = 0; c < (s.cusp_b ? 0 : 2); c++) push(1u, 0, false, 0u, 0u, false, kConnector, eb, cb);
         }
     }
 }

@@ -219,7 +219,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
         // the side's cusp vertex: the parallel curve at the cusp parameter (L380-386), evaluated once and shared by the
         // parts that meet there (a side has a cusp iff it has two ranges)
         if (live && two_ranges) {
-            V2 c = normal_point(p, S.spiral[lane >> 1], tc, eta);
+            V2 c = normal_point(S.piece[lane >> 1], S.spiral[lane >> 1], tc, eta);
             S.cusp[lane] = make_float4(c.x, c.y, tc, 0.0f);
         }
         if (DIRECT && ndirect) {
@@ -234,7 +234,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
             for (uint32_t i = 1; i <= ndirect; i++) {
                 float t;
                 V2 cur;
-                if (i < ndirect) { t = offset_t(p, o, eta, (int)i); cur = normal_point(p, z, t, eta); }
+                if (i < ndirect) { t = offset_t(p, o, eta, (int)i); cur = normal_point(S.piece[lane >> 1], z, t, eta); }
                 else cur = end_vertex(p, kEndT1, eta, nocusp, &t);
                 const uint64_t rec = base + (side ? ndirect - i : i - 1u);
                 const V2 A = side ? cur : prev, B = side ? prev : cur;

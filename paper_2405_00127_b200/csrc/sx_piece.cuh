@@ -13,7 +13,8 @@ namespace sx {
 // cbrtf, because t is ill-conditioned in x on nearly circular pieces (dt/dx = L / (2 eta k1)): one ulp in f_approx
 // moves a vertex by up to ~5e-4 px along the curve, and the oracle evaluates this path in fp32 too.
 // f_approx (L149), odd extension (L157), middle piece sign-preserving (R-3b)
-SX_DEV float f_approx(float x) {
+// (not inlined: four call sites per side plan; the kernels' working set has to stay inside the instruction cache)
+__device__ __noinline__ float f_approx(float x) {
     // All four pieces are evaluated and one is selected: the threads of a warp sit on different pieces, and a
     // branch per piece would serialise them.  sin on [0, 0.88] by its Taylor series to y^11 (truncation 6e-9).
     const float a = fabsf(x);
@@ -104,15 +105,16 @@ SX_DEV void sx_sincos(float x, float* s, float* c) {
 }
 
 // int_{m-hd}^{m+hd} exp(i phi(u)) du by 3-point Gauss-Legendre (hd may be negative)
-SX_DEV void es_gl3(float a, float hk, float m, float hd, float* ix, float* iy) {
+// (not inlined: one copy of the three sincos for the anchor table, the vertices and the cusp point)
+__device__ __noinline__ float2 es_gl3(float a, float hk, float m, float hd) {
     const float d = hd * 0.77459666924148338f;
     const float u0 = m - d, u2 = m + d;
     float s0, c0, s1, c1, s2, c2;
     sx_sincos(u0 * fmaf(hk, u0, a), &s0, &c0);
     sx_sincos(m * fmaf(hk, m, a), &s1, &c1);
     sx_sincos(u2 * fmaf(hk, u2, a), &s2, &c2);
-    *ix = hd * fmaf(0.55555555555555556f, c0 + c2, 0.88888888888888889f * c1);
-    *iy = hd * fmaf(0.55555555555555556f, s0 + s2, 0.88888888888888889f * s1);
+    return make_float2(hd * fmaf(0.55555555555555556f, c0 + c2, 0.88888888888888889f * c1),
+                       hd * fmaf(0.55555555555555556f, s0 + s2, 0.88888888888888889f * s1));
 }
 
 // one half of the anchor table: half 0 integrates intervals [0, max(K/2,1)), half 1 intervals [K/2, K) (none when
@@ -126,9 +128,8 @@ SX_DEV int es_anchor_half(const Piece& p, int K, int half, float* hx, float* hy,
 #pragma unroll
     for (int k = 0; k < kAnchors / 2; k++) {
         if (k < count) {
-            float ix, iy;
-            es_gl3(a, hk, ((float)(first + k) + 0.5f) * w, 0.5f * w, &ix, &iy);
-            zx += ix; zy += iy;
+            const float2 in = es_gl3(a, hk, ((float)(first + k) + 0.5f) * w, 0.5f * w);
+            zx += in.x; zy += in.y;
         }
         hx[k] = zx; hy[k] = zy;
     }
@@ -173,9 +174,8 @@ SX_DEV void es_eval(const Piece& p, const Spiral& sp, float t, V2* pos, V2* tan)
     kf = kf < 0.0f ? 0.0f : (kf > K ? K : kf);
     const int k = (int)kf;
     const float t0 = kf / K, hd = 0.5f * (t - t0);  // K is a power of two: exact
-    float ix, iy;
-    es_gl3(a, hk, t0 + hd, hd, &ix, &iy);
-    const float zx = sp.zx[k] + ix, zy = sp.zy[k] + iy;
+    const float2 in = es_gl3(a, hk, t0 + hd, hd);
+    const float zx = sp.zx[k] + in.x, zy = sp.zy[k] + in.y;
     float wx = fmaf(zx, sp.wr, -zy * sp.wi), wy = fmaf(zx, sp.wi, zy * sp.wr);
     pos->x = fmaf(p.ch.x, wx, fmaf(-p.ch.y, wy, p.la.x));
     pos->y = fmaf(p.ch.x, wy, fmaf(p.ch.y, wx, p.la.y));
@@ -192,7 +192,8 @@ SX_DEV V2 offset_point(V2 V, V2 u, float eta) { return v2(fmaf(eta, -u.y, V.x), 
 // At t = 0 and t = 1 the cubic's own point and tangent are used, so that adjacent pieces (and the join of the
 // next segment) share bits.  The spiral is evaluated unconditionally and the end-point cases are selected
 // afterwards, so that a warp evaluating a mix of interior and end vertices stays converged.
-SX_DEV V2 normal_point(const Piece& p, const Spiral& sp, float t, float r) {
+// (not inlined: one copy for the ring, the cusp point and the direct writer)
+__device__ __noinline__ V2 normal_point(const Piece& p, const Spiral& sp, float t, float r) {
     V2 l, T;
     es_eval(p, sp, t, &l, &T);
     const bool e0 = t == 0.0f, e1 = t == 1.0f;
