@@ -117,46 +117,47 @@ struct Style { float width, miter_limit; int join, cap; };
 // tangent T1) -- R-10.  -h side runs forward A->B, +h side backward B'->A'.
 template <bool EMIT>
 SX_DEV uint32_t emit_join(const Params& P, const Style& st, V2 V, V2 T0, V2 W, V2 T1, float h, const Writer* w, uint32_t first) {
-    float cr = cross(T0, T1), dt = dot(T0, T1);
-    bool outer_minus = (cr > 0.0f) || (cr == 0.0f && dt < 0.0f);
-    float phi = fabsf(atan2f(cr, dt));
-    float opd = 1.0f + dt;
-    bool miter_ok = (opd > 1e-6f) && (2.0f / opd <= st.miter_limit * st.miter_limit);
+    // Written per ROLE (outer join, inner join), not per side: which side is the outer one depends on the turn, and
+    // a warp whose lanes turn both ways would otherwise run the outer and the inner code twice each.
+    const float cr = cross(T0, T1), dt = dot(T0, T1);
+    const bool outer_minus = (cr > 0.0f) || (cr == 0.0f && dt < 0.0f);
+    const float opd = 1.0f + dt;
+    const bool miter = st.join == kJoinMiter && (opd > 1e-6f) && (2.0f / opd <= st.miter_limit * st.miter_limit);
+    const bool round = st.join == kJoinRound;
     const bool arc = P.mode == kModeArc;
-    uint32_t idx = 0;
-#pragma unroll
-    for (int side = 0; side < 2; side++) {
-        bool outer = side == 0 ? outer_minus : !outer_minus;
-        uint32_t sb = side == 0 ? 0u : (uint32_t)kPlus;
-        V2 s0, s1;
-        if (EMIT) {
-            s0 = side == 0 ? offset_point(V, T0, -h) : offset_point(W, T1, h);
-            s1 = side == 0 ? offset_point(W, T1, -h) : offset_point(V, T0, h);
+    float phi = 0.0f;
+    uint32_t n_outer = miter ? 2u : 1u;
+    if (round) { phi = fabsf(atan2f(cr, dt)); n_outer = (uint32_t)round_count(phi, h, P.mode, P.tol_fl); }
+    if (EMIT) {
+        // side 0 (-h, forward V -> W) comes first, then side 1 (+h, backward W -> V)
+        const uint32_t first_outer = first + (outer_minus ? 0u : 2u), first_inner = first + (outer_minus ? n_outer : 0u);
+        {   // outer side
+            const bool plus = !outer_minus;
+            const float hh = plus ? h : -h;
+            const uint32_t kind = kJoinOuter | (plus ? (uint32_t)kPlus : 0u);
+            const V2 s0 = offset_point(plus ? W : V, plus ? T1 : T0, hh), s1 = offset_point(plus ? V : W, plus ? T0 : T1, hh);
+            if (round) {
+                const V2 r = plus ? v2(fmaf(h, -T1.y, W.x - V.x), fmaf(h, T1.x, W.y - V.y)) : v2(h * T0.y, -h * T0.x);
+                emit_round(w, first_outer, (int)n_outer, V, r, s0, s1, phi, kind, arc);
+            } else if (miter) {
+                const float k = hh / opd;  // tip = V -/+ h (N0+N1)/(1+dt)
+                const V2 tip = v2(fmaf(k, -T0.y - T1.y, V.x), fmaf(k, T0.x + T1.x, V.y));
+                w->put(first_outer, s0, tip, 0.0f, kind);
+                w->put(first_outer + 1u, tip, s1, 0.0f, kind);
+            } else {
+                w->put(first_outer, s0, s1, 0.0f, kind);
+            }
         }
-        if (!outer) {  // inner join: through the vertex (strong correctness, L35)
-            if (EMIT) { w->put(first + idx, s0, V, 0.0f, kJoinInner | sb); w->put(first + idx + 1, V, s1, 0.0f, kJoinInner | sb); }
-            idx += 2;
-        } else if (st.join == kJoinRound) {
-            int n = round_count(phi, h, P.mode, P.tol_fl);
-            if (EMIT) {
-                V2 r = side == 0 ? v2(h * T0.y, -h * T0.x) : v2(fmaf(h, -T1.y, W.x - V.x), fmaf(h, T1.x, W.y - V.y));
-                emit_round(w, first + idx, n, V, r, s0, s1, phi, kJoinOuter | sb, arc);
-            }
-            idx += (uint32_t)n;
-        } else if (st.join == kJoinMiter && miter_ok) {
-            if (EMIT) {
-                float k = (side == 0 ? -h : h) / opd;  // tip = V -/+ h (N0+N1)/(1+dt)
-                V2 tip = v2(fmaf(k, -T0.y - T1.y, V.x), fmaf(k, T0.x + T1.x, V.y));
-                w->put(first + idx, s0, tip, 0.0f, kJoinOuter | sb);
-                w->put(first + idx + 1, tip, s1, 0.0f, kJoinOuter | sb);
-            }
-            idx += 2;
-        } else {
-            if (EMIT) w->put(first + idx, s0, s1, 0.0f, kJoinOuter | sb);
-            idx += 1;
+        {   // inner side: through the vertex (strong correctness, L35)
+            const bool plus = outer_minus;
+            const float hh = plus ? h : -h;
+            const uint32_t kind = kJoinInner | (plus ? (uint32_t)kPlus : 0u);
+            const V2 s0 = offset_point(plus ? W : V, plus ? T1 : T0, hh), s1 = offset_point(plus ? V : W, plus ? T0 : T1, hh);
+            w->put(first_inner, s0, V, 0.0f, kind);
+            w->put(first_inner + 1u, V, s1, 0.0f, kind);
         }
     }
-    return idx;
+    return n_outer + 2u;
 }
 
 // cap at vertex V with outward direction T: from V - hN(T) counter-clockwise to V + hN(T) (R-11)
