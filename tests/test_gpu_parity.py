@@ -354,6 +354,23 @@ def _sampled_full_size(B, ctx, name, mode, n_sample, seed):
     del out
 
 
+def test_full_size_c4_every_path_is_watertight(B, ctx):
+    """A property that holds at any size: at the full CAD-scale config every one of the 100,000 outlines is watertight
+    (bitwise: the multiset of record start points equals the multiset of end points), and path offsets are monotone."""
+    sc = S.make("c4")
+    dev = "cuda:0"
+    tags, pts, sty = B.scene_to_torch(sc, device=dev)
+    rec, poff = B.stroke_expand(ctx, tags, pts, sty, sc.affine, sc.tolerance, 1)
+    torch.cuda.synchronize()
+    assert B.sx_last_error(ctx) == 0
+    xy = rec[:, :4].contiguous().cpu().numpy()
+    po = poff.cpu().numpy()
+    assert np.isfinite(xy).all() and po[0] == 0 and po[-1] == len(xy) and (np.diff(po) > 0).all()
+    assert ck.watertight_violations(xy, po) == 0
+    kinds = rec[:, 6].contiguous().view(torch.int32).cpu().numpy()
+    assert ((kinds & 7) <= ck.K_CAP).all()
+
+
 def test_full_size_c3_sampled(B, ctx):
     _sampled_full_size(B, ctx, "c3", 0, 400, 7)
 
