@@ -208,7 +208,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
         {   // anchor table: each of the two lanes of a piece integrates one half, then they exchange totals
             const int K = es_intervals(p.k0, p.k1);
             float hx[kAnchors / 2], hy[kAnchors / 2], tx, ty;
-            const int cnt = es_anchor_half(p, K, side, hx, hy, &tx, &ty);
+            const int cnt = es_anchor_half<DIRECT>(p, K, side, hx, hy, &tx, &ty);
             const float ox = __shfl_xor_sync(0xffffffffu, tx, 1), oy = __shfl_xor_sync(0xffffffffu, ty, 1);
             if (live) es_anchor_store(S.spiral[lane >> 1], K, side, cnt, hx, hy, tx, ty, ox, oy);
         }
@@ -219,7 +219,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
         // the side's cusp vertex: the parallel curve at the cusp parameter (L380-386), evaluated once and shared by the
         // parts that meet there (a side has a cusp iff it has two ranges)
         if (live && two_ranges) {
-            V2 c = normal_point(S.piece[lane >> 1], S.spiral[lane >> 1], tc, eta);
+            V2 c = normal_point_sel<DIRECT>(S.piece[lane >> 1], S.spiral[lane >> 1], tc, eta);
             S.cusp[lane] = make_float4(c.x, c.y, tc, 0.0f);
         }
         if (DIRECT && ndirect) {
@@ -234,7 +234,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
             for (uint32_t i = 1; i <= ndirect; i++) {
                 float t;
                 V2 cur;
-                if (i < ndirect) { t = offset_t(p, o, eta, (int)i); cur = normal_point(S.piece[lane >> 1], z, t, eta); }
+                if (i < ndirect) { t = offset_t(p, o, eta, (int)i); cur = normal_point_sel<DIRECT>(p, z, t, eta); }
                 else cur = end_vertex(p, kEndT1, eta, nocusp, &t);
                 const uint64_t rec = base + (side ? ndirect - i : i - 1u);
                 const V2 A = side ? cur : prev, B = side ? prev : cur;
@@ -311,7 +311,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
                         const int idx = (pj.info & 128u) ? (int)pj.i0 - (int)mm : (int)pj.i0 + (int)mm;
                         const bool evo = ((pj.info >> 8) & 3u) == 2u;
                         const float t = evo ? evolute_t(pc, plan_evo(sp), idx) : offset_t(pc, plan_off(sp, (pj.info & 1024u) != 0u), sp.eta, idx);
-                        const V2 g = normal_point(pc, S.spiral[ss >> 1], t, evo ? es_radius(pc, t) : sp.eta);
+                        const V2 g = normal_point_sel<DIRECT>(pc, S.spiral[ss >> 1], t, evo ? es_radius(pc, t) : sp.eta);
                         S.ring[v & (uint32_t)(kRing - 1)] = make_float4(g.x, g.y, t, 0.0f);
                     }
                     v_done += 32u;

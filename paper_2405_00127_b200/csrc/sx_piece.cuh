@@ -105,8 +105,7 @@ SX_DEV void sx_sincos(float x, float* s, float* c) {
 }
 
 // int_{m-hd}^{m+hd} exp(i phi(u)) du by 3-point Gauss-Legendre (hd may be negative)
-// (not inlined: one copy of the three sincos for the anchor table, the vertices and the cusp point)
-__device__ __noinline__ float2 es_gl3(float a, float hk, float m, float hd) {
+SX_DEV float2 es_gl3_body(float a, float hk, float m, float hd) {
     const float d = hd * 0.77459666924148338f;
     const float u0 = m - d, u2 = m + d;
     float s0, c0, s1, c1, s2, c2;
@@ -116,10 +115,17 @@ __device__ __noinline__ float2 es_gl3(float a, float hk, float m, float hd) {
     return make_float2(hd * fmaf(0.55555555555555556f, c0 + c2, 0.88888888888888889f * c1),
                        hd * fmaf(0.55555555555555556f, s0 + s2, 0.88888888888888889f * s1));
 }
+// One non-inlined copy for the kernels whose working set has to stay inside the instruction cache (the table
+// variant of the write kernel); INL = true inlines instead (the DIRECT variant is small enough, and calls cost
+// it register spills).  Same operations either way, hence the same bits.
+__device__ __noinline__ float2 es_gl3_call(float a, float hk, float m, float hd) { return es_gl3_body(a, hk, m, hd); }
+template <bool INL>
+SX_DEV float2 es_gl3(float a, float hk, float m, float hd) { return INL ? es_gl3_body(a, hk, m, hd) : es_gl3_call(a, hk, m, hd); }
 
 // one half of the anchor table: half 0 integrates intervals [0, max(K/2,1)), half 1 intervals [K/2, K) (none when
 // K = 1); cumulative sums relative to the half's start in hx/hy[0..count), the half's total in *tx, *ty.
 // es_prepare = both halves by one thread; the write kernel gives one half to each of two threads.
+template <bool INL = false>
 SX_DEV int es_anchor_half(const Piece& p, int K, int half, float* hx, float* hy, float* tx, float* ty) {
     const float a = p.k0 - 0.5f * p.k1, hk = 0.5f * p.k1;
     const float w = 1.0f / (float)K;
@@ -128,7 +134,7 @@ SX_DEV int es_anchor_half(const Piece& p, int K, int half, float* hx, float* hy,
 #pragma unroll
     for (int k = 0; k < kAnchors / 2; k++) {
         if (k < count) {
-            const float2 in = es_gl3(a, hk, ((float)(first + k) + 0.5f) * w, 0.5f * w);
+            const float2 in = es_gl3<INL>(a, hk, ((float)(first + k) + 0.5f) * w, 0.5f * w);
             zx += in.x; zy += in.y;
         }
         hx[k] = zx; hy[k] = zy;
@@ -167,6 +173,7 @@ SX_DEV float es_phi(const Piece& p, float t) { return t * fmaf(0.5f * p.k1, t, p
 SX_DEV float es_dphi(const Piece& p, float ta, float tb) { return (tb - ta) * fmaf(0.5f * p.k1, ta + tb, p.k0 - 0.5f * p.k1); }
 
 // local position and unit tangent at piece fraction t in [0,1]: la + ch (x) Z(t)/Z(1) (L632)
+template <bool INL = false>
 SX_DEV void es_eval(const Piece& p, const Spiral& sp, float t, V2* pos, V2* tan) {
     const float a = p.k0 - 0.5f * p.k1, hk = 0.5f * p.k1;
     const float K = sp.K;
@@ -174,7 +181,7 @@ SX_DEV void es_eval(const Piece& p, const Spiral& sp, float t, V2* pos, V2* tan)
     kf = kf < 0.0f ? 0.0f : (kf > K ? K : kf);
     const int k = (int)kf;
     const float t0 = kf / K, hd = 0.5f * (t - t0);  // K is a power of two: exact
-    const float2 in = es_gl3(a, hk, t0 + hd, hd);
+    const float2 in = es_gl3<INL>(a, hk, t0 + hd, hd);
     const float zx = sp.zx[k] + in.x, zy = sp.zy[k] + in.y;
     float wx = fmaf(zx, sp.wr, -zy * sp.wi), wy = fmaf(zx, sp.wi, zy * sp.wr);
     pos->x = fmaf(p.ch.x, wx, fmaf(-p.ch.y, wy, p.la.x));
@@ -192,10 +199,10 @@ SX_DEV V2 offset_point(V2 V, V2 u, float eta) { return v2(fmaf(eta, -u.y, V.x), 
 // At t = 0 and t = 1 the cubic's own point and tangent are used, so that adjacent pieces (and the join of the
 // next segment) share bits.  The spiral is evaluated unconditionally and the end-point cases are selected
 // afterwards, so that a warp evaluating a mix of interior and end vertices stays converged.
-// (not inlined: one copy for the ring, the cusp point and the direct writer)
-__device__ __noinline__ V2 normal_point(const Piece& p, const Spiral& sp, float t, float r) {
+template <bool INL>
+SX_DEV V2 normal_point_body(const Piece& p, const Spiral& sp, float t, float r) {
     V2 l, T;
-    es_eval(p, sp, t, &l, &T);
+    es_eval<INL>(p, sp, t, &l, &T);
     const bool e0 = t == 0.0f, e1 = t == 1.0f;
     if (e0) { l = p.la; T = p.ua; }
     if (e1) { l = p.lb; T = p.ub; }
@@ -205,6 +212,10 @@ __device__ __noinline__ V2 normal_point(const Piece& p, const Spiral& sp, float 
     if (e1 && p.at1) g = offset_point(p.P3, p.ub, r);
     return g;
 }
+// (one non-inlined copy for the ring, the cusp point and the reference walk; see es_gl3)
+__device__ __noinline__ V2 normal_point(const Piece& p, const Spiral& sp, float t, float r) { return normal_point_body<false>(p, sp, t, r); }
+template <bool INL>
+SX_DEV V2 normal_point_sel(const Piece& p, const Spiral& sp, float t, float r) { return INL ? normal_point_body<true>(p, sp, t, r) : normal_point(p, sp, t, r); }
 SX_DEV V2 es_offset(const Piece& p, const Spiral& sp, float t, float eta) { return normal_point(p, sp, t, eta); }
 SX_DEV V2 es_evolute(const Piece& p, const Spiral& sp, float t) { return normal_point(p, sp, t, es_radius(p, t)); }  // section 6
 
