@@ -175,6 +175,11 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
     const int side = lane & 1;
     for (uint32_t tile = blockIdx.x * (uint32_t)kWpWarps + (uint32_t)warp; (uint64_t)tile * kWtPieces < reserved; tile += n_warps) {
         // ---- stage
+        {   // pull the next tile's descriptors (16 x 80 B = ten 128-byte lines) into L2 while this tile is worked on
+            const uint64_t nslot = (uint64_t)(tile + n_warps) * kWtPieces;
+            if (lane < 10 && nslot < reserved)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(pieces + nslot * kDescQuads) + 128 * lane));
+        }
         const uint32_t slot = tile * (uint32_t)kWtPieces + (uint32_t)(lane >> 1);
         Piece p;
         p.k0 = 0.0f; p.k1 = 0.0f;
