@@ -1,8 +1,10 @@
 // sx_segment.cuh -- one input segment end to end (Alg. 1 L306-343 per thread, Alg. 2 L351-438 inside).
 //
-// process_segment<EMIT=false> returns the number of records the segment produces (count kernel);
-// process_segment<EMIT=true> writes them in the canonical order (write kernel).  Both instantiate the
-// same plan functions, so the counts agree by construction.
+// The pieces the kernels are made of: fit_next (Alg. 2 as a resumable generator: the count kernel), joins and caps
+// (segment_tail: the count kernel with EMIT = false, the segment writer with EMIT = true) and process_segment, the
+// thread-per-segment reference walk of everything a segment emits, in canonical order (the fallback writer, and the
+// definition the table-driven piece writer of sx_cache.cuh / sx_kernels.cu reproduces bit for bit).  Counting and
+// writing instantiate the same plan functions, so the counts agree by construction.
 #pragma once
 #include "sx_piece.cuh"
 
