@@ -120,12 +120,13 @@ SX_DEV V2 xform(const float* A, float x, float y) {
 
 // first control-polygon leg that is not (near) zero, else (1,0) (R-5): the limit tangent of the curve
 SX_DEV V2 pick_tangent(V2 a, V2 b, V2 c, bool* degenerate) {
-    *degenerate = false;
-    if (len2(a) >= kEpsQ2) return unit(a);
-    if (len2(b) >= kEpsQ2) return unit(b);
-    if (len2(c) >= kEpsQ2) return unit(c);
-    *degenerate = true;
-    return v2(1.0f, 0.0f);
+    // the leg is SELECTED first and normalised once (three normalisations behind three branches cost a third of the
+    // segment writer's instructions)
+    const bool ua = len2(a) >= kEpsQ2, ub = len2(b) >= kEpsQ2, uc = len2(c) >= kEpsQ2;
+    const V2 d = ua ? a : (ub ? b : c);
+    *degenerate = !(ua || ub || uc);
+    const V2 u = unit(d);
+    return *degenerate ? v2(1.0f, 0.0f) : u;
 }
 
 #ifdef __CUDA_ARCH__
@@ -176,9 +177,25 @@ SX_DEV Seg load_segment(const Params& P, uint32_t i, uint32_t tag) {
 
 // start point and start tangent only (join partner / start cap owner)
 SX_DEV void load_segment_start(const Params& P, uint32_t j, V2* P0, V2* ts) {
-    Seg s = load_segment(P, j, P.tags[j]);
-    *P0 = s.P0;
-    *ts = s.ts;
+    // = load_segment(P, j, tags[j]).{P0, ts} without the end tangent: the same legs in the same order
+    const uint32_t cnt = P.tags[j] & 3u;
+    const float* p = P.pts + 2 * (uint64_t)P.pt_off[j];
+    auto a0 = ldg2(p), a1 = ldg2(p + 2);
+    const V2 q0 = xform(P.A, a0.x, a0.y), q1 = xform(P.A, a1.x, a1.y);
+    V2 l1 = q1 - q0, l2 = l1, l3 = l1;  // line: d, d, d
+    if (cnt >= 2u) {
+        auto a2 = ldg2(p + 4);
+        const V2 q2 = xform(P.A, a2.x, a2.y);
+        l2 = q2 - q0; l3 = l2;              // quadratic: a, b, b
+        if (cnt == 3u) {
+            auto a3 = ldg2(p + 6);
+            const V2 q3 = xform(P.A, a3.x, a3.y);
+            l3 = q3 - q0;                   // cubic: c1, c2, c3
+        }
+    }
+    bool dg;
+    *P0 = q0;
+    *ts = pick_tangent(l1, l2, l3, &dg);
 }
 
 // ---------------------------------------------------------------- cubic evaluation (Alg. 2), Bernstein form
