@@ -356,22 +356,24 @@ k_write_segments(Params P, const uint32_t* __restrict__ seg_count, const uint64_
                  uint64_t cap_records, uint32_t piece_cap, const uint32_t* __restrict__ piece_ctr, uint32_t* err) {
     uint32_t i = blockIdx.x * (uint32_t)kSegThreads + threadIdx.x;
     if (i >= P.n_tags) return;
-    uint32_t n = seg_count[i];
+    // everything that can be loaded from i alone, in one batch (the kernel is bound by the latency of its dependent loads)
+    const uint32_t jn = i + 1u < P.n_tags ? i + 1u : i;
+    const uint32_t n = seg_count[i], tag = P.tags[i], path = P.path_idx[i], pt = P.pt_off[i], first_seg = P.sp_first[i];
+    const uint32_t tag_n = P.tags[jn], pt_n = P.pt_off[jn];
+    const uint64_t off = seg_off[i];
     if (n == 0u) return;
-    uint64_t off = seg_off[i];
     if (off + n > cap_records) { atomicOr(err, kErrCapacity); return; }
     Writer w;
     w.out = out; w.base = off; w.seg = i; w.mode = P.mode;
     if (*piece_ctr > piece_cap) return;  // cache overflow: k_write_fallback takes the whole call
-    uint32_t tag = P.tags[i];
     Style st;
     float h;
-    load_style(P, P.path_idx[i], &st, &h);
-    Seg s = load_segment(P, i, tag);
+    load_style(P, path, &st, &h);
+    Seg s = load_segment_at(P, pt, tag);
     uint32_t first;
     if (s.kind == 1 || s.degenerate) { emit_straight(s, h, &w); first = 2u; }
-    else first = n - segment_tail<false>(P, i, tag, s, st, h, nullptr, 0);
-    segment_tail<true>(P, i, tag, s, st, h, &w, first);
+    else first = n - segment_tail<false>(P, tag, s, st, h, first_seg, tag_n, pt_n, nullptr, 0);
+    segment_tail<true>(P, tag, s, st, h, first_seg, tag_n, pt_n, &w, first);
 }
 
 // (d3) thread-per-segment writer for a call whose pieces did not fit the cache (sx_set_piece_cache_limit, or

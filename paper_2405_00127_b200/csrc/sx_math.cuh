@@ -135,10 +135,11 @@ SX_DEV float2 ldg2(const float* p) { return __ldg(reinterpret_cast<const float2*
 SX_DEV V2 ldg2(const float* p) { return v2(p[0], p[1]); }
 #endif
 
-SX_DEV Seg load_segment(const Params& P, uint32_t i, uint32_t tag) {
+// pt = index of the segment's first point (pt_off[i] from the tag scan)
+SX_DEV Seg load_segment_at(const Params& P, uint32_t pt, uint32_t tag) {
     Seg s;
     int cnt = tag & 3;
-    const float* p = P.pts + 2 * (uint64_t)P.pt_off[i];
+    const float* p = P.pts + 2 * (uint64_t)pt;
     auto a0 = ldg2(p), a1 = ldg2(p + 2);
     V2 q0 = xform(P.A, a0.x, a0.y), q1 = xform(P.A, a1.x, a1.y);
     s.kind = cnt;
@@ -176,10 +177,12 @@ SX_DEV Seg load_segment(const Params& P, uint32_t i, uint32_t tag) {
 }
 
 // start point and start tangent only (join partner / start cap owner)
-SX_DEV void load_segment_start(const Params& P, uint32_t j, V2* P0, V2* ts) {
-    // = load_segment(P, j, tags[j]).{P0, ts} without the end tangent: the same legs in the same order
-    const uint32_t cnt = P.tags[j] & 3u;
-    const float* p = P.pts + 2 * (uint64_t)P.pt_off[j];
+SX_DEV Seg load_segment(const Params& P, uint32_t i, uint32_t tag) { return load_segment_at(P, P.pt_off[i], tag); }
+
+SX_DEV void load_segment_start_at(const Params& P, uint32_t pt, uint32_t tag, V2* P0, V2* ts) {
+    // = load_segment_at(P, pt, tag).{P0, ts} without the end tangent: the same legs in the same order
+    const uint32_t cnt = tag & 3u;
+    const float* p = P.pts + 2 * (uint64_t)pt;
     auto a0 = ldg2(p), a1 = ldg2(p + 2);
     const V2 q0 = xform(P.A, a0.x, a0.y), q1 = xform(P.A, a1.x, a1.y);
     V2 l1 = q1 - q0, l2 = l1, l3 = l1;  // line: d, d, d
@@ -197,6 +200,7 @@ SX_DEV void load_segment_start(const Params& P, uint32_t j, V2* P0, V2* ts) {
     *P0 = q0;
     *ts = pick_tangent(l1, l2, l3, &dg);
 }
+SX_DEV void load_segment_start(const Params& P, uint32_t j, V2* P0, V2* ts) { load_segment_start_at(P, P.pt_off[j], P.tags[j], P0, ts); }
 
 // ---------------------------------------------------------------- cubic evaluation (Alg. 2), Bernstein form
 SX_DEV V2 cubic_pos(const Seg& s, float t) {

@@ -264,23 +264,31 @@ SX_DEV bool load_style(const Params& P, uint32_t path, Style* st, float* h) {
 
 // what follows the offset curves of segment i (Alg. 1): the join with its partner, or, on the last
 // segment of an open subpath, [end cap][start cap]
+// tag_n, pt_n: tag and point offset of segment i + 1, first: sp_first[i] -- loaded by the caller together with the
+// segment's own scan results, so that the partner's points are one dependent load away, not two
 template <bool EMIT>
-SX_DEV uint32_t segment_tail(const Params& P, uint32_t i, uint32_t tag, const Seg& s, const Style& st, float h, const Writer* w, uint32_t first) {
+SX_DEV uint32_t segment_tail(const Params& P, uint32_t tag, const Seg& s, const Style& st, float h, uint32_t first_seg, uint32_t tag_n,
+                             uint32_t pt_n, const Writer* w, uint32_t first) {
     bool sp_end = ((tag >> 2) | (tag >> 4)) & 1u;
     bool closed = (tag >> 7) & 1u;
     uint32_t n = 0;
     if (!sp_end || closed) {
-        uint32_t j = sp_end ? P.sp_first[i] : i + 1;
         V2 W, T1;
-        load_segment_start(P, j, &W, &T1);
+        if (sp_end) load_segment_start(P, first_seg, &W, &T1);
+        else load_segment_start_at(P, pt_n, tag_n, &W, &T1);
         n += emit_join<EMIT>(P, st, s.P3, s.te, W, T1, h, w, first);
     } else {
         V2 F, Tf;
-        load_segment_start(P, P.sp_first[i], &F, &Tf);
+        load_segment_start(P, first_seg, &F, &Tf);
         n += emit_cap<EMIT>(P, st, s.P3, s.te, h, w, first);
         n += emit_cap<EMIT>(P, st, F, v2(-Tf.x, -Tf.y), h, w, first + n);
     }
     return n;
+}
+template <bool EMIT>
+SX_DEV uint32_t segment_tail(const Params& P, uint32_t i, uint32_t tag, const Seg& s, const Style& st, float h, const Writer* w, uint32_t first) {
+    const uint32_t jn = i + 1u < P.n_tags ? i + 1u : i;
+    return segment_tail<EMIT>(P, tag, s, st, h, P.sp_first[i], P.tags[jn], P.pt_off[jn], w, first);
 }
 
 // straight fast path (R-1b): the two offset lines of a line (or fully degenerate) segment are exact
