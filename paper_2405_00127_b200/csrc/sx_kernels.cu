@@ -417,6 +417,8 @@ struct sx_ctx {
     uint64_t piece_cap;
     uint64_t piece_limit; // 0 = no limit (sx_set_piece_cache_limit)
     int sm_count;
+    cudaStream_t side_stream;   // k_write_segments runs here, beside k_write_pieces on the caller's stream
+    cudaEvent_t ev_fork, ev_join;
     // last sx_count
     sx::Params P;
     uint64_t n_paths;
@@ -499,6 +501,10 @@ sx_status sx_create(sx_ctx** out, int32_t device) {
     e = cudaFuncSetAttribute(sx::k_write_pieces<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sx::kWpWarps * sizeof(sx::WarpTile)));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(sx::k_write_pieces<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sx::kWpWarps * sizeof(sx::WarpTile)));
     if (e != cudaSuccess) { g_last_cuda = e; cudaFreeHost(c->h_pinned); free(c); return SX_E_CUDA; }
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming);
+    if (e != cudaSuccess) { g_last_cuda = e; cudaFreeHost(c->h_pinned); free(c); return SX_E_CUDA; }
     *out = c;
     return SX_OK;
 }
@@ -507,6 +513,9 @@ sx_status sx_destroy(sx_ctx* c) {
     if (!c) return SX_E_INVALID_ARG;
     cudaSetDevice(c->device);
     cudaDeviceSynchronize();
+    cudaStreamDestroy(c->side_stream);
+    cudaEventDestroy(c->ev_fork);
+    cudaEventDestroy(c->ev_join);
     cudaFree(c->pt_off);
     cudaFree(c->pieces);
     cudaFree(c->sync_area);
@@ -607,12 +616,18 @@ sx_status sx_write(sx_ctx* c, void* d_out_records, uint64_t cap_records, void* c
     SX_CUDA(cudaSetDevice(c->device));
     uint32_t n = c->P.n_tags;
     float4* out = static_cast<float4*>(d_out_records);
+    // the segment writer is bound by the latency of its dependent loads, the piece writer by instruction issue: they
+    // run side by side (fork / join on events; everything stays ordered with respect to the caller's stream)
+    SX_CUDA(cudaEventRecord(c->ev_fork, s));
+    SX_CUDA(cudaStreamWaitEvent(c->side_stream, c->ev_fork, 0));
+    sx::k_write_segments<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, c->side_stream>>>(
+        c->P, c->seg_count, c->seg_off, out, cap_records, (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_err(c));
+    SX_CUDA(cudaEventRecord(c->ev_join, c->side_stream));
     sx::k_write_pieces<false><<<c->sm_count * sx::kWpBlocksPerSM, sx::kWpThreads, sx::kWpWarps * sizeof(sx::WarpTile), s>>>(
         c->P, c->pieces, (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_side_stats(c), c->seg_off, out, cap_records, ctx_err(c));
     sx::k_write_pieces<true><<<c->sm_count * sx::kWpBlocksPerSM, sx::kWpThreads, sx::kWpWarps * sizeof(sx::WarpTile), s>>>(
         c->P, c->pieces, (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_side_stats(c), c->seg_off, out, cap_records, ctx_err(c));
-    sx::k_write_segments<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(c->P, c->seg_count, c->seg_off, out, cap_records,
-                                                                                               (uint32_t)c->piece_cap, ctx_piece_ctr(c), ctx_err(c));
+    SX_CUDA(cudaStreamWaitEvent(s, c->ev_join, 0));
     c->launches += 3;
     if (!c->cache_fits) {
         sx::k_write_fallback<<<(n + sx::kSegThreads - 1) / sx::kSegThreads, sx::kSegThreads, 0, s>>>(c->P, c->seg_count, c->seg_off, out, cap_records,
