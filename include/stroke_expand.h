@@ -131,7 +131,8 @@ sx_status sx_count(sx_ctx* ctx, const uint8_t* d_tags, uint64_t n_tags, const fl
  * by mode, 16-byte aligned) of capacity cap_records.  SX_E_CAPACITY if the capacity is known to be
  * too small (the total is known on the host only when sx_count was given h_total; otherwise the
  * kernel itself refuses to write past the capacity and the error is reported by sx_last_error after
- * a stream sync). */
+ * a stream sync).  Part of the work runs on a stream owned by the context, forked from and joined to `cuda_stream`
+ * with events: for the caller everything is ordered on `cuda_stream` as usual (the pattern is CUDA-graph capturable). */
 sx_status sx_write(sx_ctx* ctx, void* d_out_records, uint64_t cap_records, void* cuda_stream);
 
 /* ------------------------------------------------------------------ one-shot, device buffers
