@@ -30,7 +30,7 @@ constexpr int kDirectMax = 6;               // DIRECT variant: records of a side
 // its next accepted piece (fit_next, Alg. 2); the round's pieces are compacted through shared memory and
 // their 2 x T side plans are spread over ALL threads of the block (a thread whose curve is finished still plans
 // for its neighbours); one atomic per round reserves exactly T descriptor slots of the piece cache.
-__global__ void __launch_bounds__(kCntThreads)
+__global__ void __launch_bounds__(kCntThreads, 32)
 k_count(Params P, uint32_t* __restrict__ seg_count, const uint32_t* __restrict__ curve_idx, const uint32_t* __restrict__ n_curves_p,
         float4* __restrict__ pieces, uint32_t piece_cap, uint32_t* piece_ctr, uint32_t* side_stats, const uint32_t* __restrict__ err) {
     __shared__ float4 s_q[kCntThreads];          // k0, k1, L, h of the round's pieces
