@@ -30,7 +30,7 @@ UNIT = "segments/s"
 MODE_OF = {"c3": 0, "c4": 1, "c5": 0, "c1": 0, "c2": 0}
 # dram__bytes_read.sum + dram__bytes_write.sum of the write pass per launch, from the committed ncu captures
 # (profiles/r1_final.md); None = not captured for that workload
-NCU_TRAFFIC = {"c4": 519.7e6, "c5": None}  # c4: 362.7 MB k_write_pieces + 157.0 MB k_write_segments (profiles/r1_final.md)
+NCU_TRAFFIC = {"c4": 519.2e6, "c5": None}  # c4: 362.7 MB k_write_pieces + 156.5 MB k_write_segments (profiles/r1_final.md)
 REF_SAMPLE_PATHS = {"c4": 20000, "c5": 1000, "c3": 20000, "c1": 256, "c2": 2000}
 
 
