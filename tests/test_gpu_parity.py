@@ -395,3 +395,14 @@ def test_long_chains_tight_tolerance(B, ctx):
         compare(sc, mode, g, r)
         assert ck.watertight_violations(g.xy, g.path_off) == 0
     assert g.seg_count.max() > 200
+
+
+def test_very_long_chains(B, ctx):
+    """Tolerance 2e-5 px on two paths: thousands of records per side (chains spanning many tiles and ring wrap-arounds)."""
+    sc = S.make("c1", n_paths=2)
+    sc["tolerance"] = 2e-5
+    g = gpu_run(B, ctx, sc, 0)
+    r = oracle_run(sc, 0)
+    compare(sc, 0, g, r)
+    assert ck.watertight_violations(g.xy, g.path_off) == 0
+    assert g.seg_count.max() > 5000
