@@ -30,8 +30,7 @@ SX_DEV void piece_store(float4* slot, const Piece& p, float h, uint32_t seg, uin
 }
 
 struct PieceHead { uint32_t seg, rel, n_minus, n_plus; bool at0, at1; };
-SX_DEV PieceHead piece_head(const float4* slot) {
-    float4 q = __ldg(slot + 4);
+SX_DEV PieceHead piece_head(float4 q) {  // q = quad 4 of the descriptor
     PieceHead hd;
     hd.seg = u_of_f(q.x);
     uint32_t r = u_of_f(q.y);

@@ -173,8 +173,23 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
     const bool arc = P.mode == kModeArc;
     const uint32_t n_warps = gridDim.x * (uint32_t)kWpWarps;
     const int side = lane & 1;
+    // The head of a descriptor (segment, relative offset, side totals) and the record offset of its segment are a chain
+    // of two dependent loads at the start of every tile: they are fetched one tile ahead, into registers.
+    float4 q4_next = make_float4(f_of_u(kInvalidSeg), 0.0f, 0.0f, 0.0f);
+    uint64_t off_next = 0;
+    {
+        const uint64_t slot0 = (uint64_t)(blockIdx.x * (uint32_t)kWpWarps + (uint32_t)warp) * kWtPieces + (uint64_t)(lane >> 1);
+        if (slot0 < reserved) { q4_next = __ldg(pieces + slot0 * kDescQuads + 4); off_next = seg_off[u_of_f(q4_next.x)]; }
+    }
     for (uint32_t tile = blockIdx.x * (uint32_t)kWpWarps + (uint32_t)warp; (uint64_t)tile * kWtPieces < reserved; tile += n_warps) {
         // ---- stage
+        const float4 q4 = q4_next;
+        const uint64_t seg_base = off_next;
+        {
+            const uint64_t nslot = (uint64_t)(tile + n_warps) * kWtPieces + (uint64_t)(lane >> 1);
+            q4_next = make_float4(f_of_u(kInvalidSeg), 0.0f, 0.0f, 0.0f);
+            if (nslot < reserved) q4_next = __ldg(pieces + nslot * kDescQuads + 4);  // an L2 hit (prefetched below, a tile ago)
+        }
         {   // pull the next tile's descriptors (16 x 80 B = ten 128-byte lines) into L2 while this tile is worked on
             const uint64_t nslot = (uint64_t)(tile + n_warps) * kWtPieces;
             if (lane < 10 && nslot < reserved)
@@ -188,7 +203,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
         hd.seg = kInvalidSeg;
         if (slot < reserved) {
             const float4* d = pieces + (uint64_t)slot * kDescQuads;
-            hd = piece_head(d);
+            hd = piece_head(q4);
             piece_load(d, hd, p, &h);
         }
         const bool live = hd.seg != kInvalidSeg;
@@ -200,7 +215,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
         if (live) {
             SidePlan sp = side_plan(p, eta, P.mode, P.tol_fl);
             nrec = (uint32_t)sp.total;
-            base = seg_off[hd.seg] + hd.rel + (side ? hd.n_minus : 0u);
+            base = seg_base + hd.rel + (side ? hd.n_minus : 0u);
             if (base + nrec > cap_records) { atomicOr(err, kErrCapacity); nrec = 0; }
             else nparts = side_part_count(sp);
             simple = DIRECT && nparts == 1u && !sp.sup[0] && nrec <= (uint32_t)kDirectMax;
@@ -252,6 +267,7 @@ k_write_pieces(Params P, const float4* __restrict__ pieces, uint32_t piece_cap, 
                 prev = cur; tp = t;
             }
         }
+        off_next = u_of_f(q4_next.x) != kInvalidSeg ? seg_off[u_of_f(q4_next.x)] : 0u;  // consumed by the next tile
         // ---- table + write, in one pass, or in two halves of the warp's sides when the parts do not fit
         const uint32_t all_parts = __reduce_add_sync(0xffffffffu, nparts);
         const uint32_t low_parts = __reduce_add_sync(0xffffffffu, lane < 16 ? nparts : 0u);
