@@ -3,4 +3,4 @@
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this
 package.  It never imports paper_2405_00127_b200's CUDA binding, and that package never imports this.
 """
-from .binding import build, expand, lib, OracleResult  # noqa: F401
+from .binding import build, expand, lib, piece_expand, OracleResult  # noqa: F401

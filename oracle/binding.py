@@ -49,6 +49,8 @@ def lib():
         L.so_f_approx_inv.argtypes = [C.c_float]
         L.so_ghi.argtypes = [C.c_float, C.c_float, C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.so_es_integral.argtypes = [C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.so_piece_expand.restype = C.c_int
+        L.so_piece_expand.argtypes = [C.c_float] * 8 + [C.c_int, C.POINTER(_Result)]
         L.so_fit_error_export.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_float, C.c_void_p]
         _lib = L
     return _lib
@@ -73,6 +75,26 @@ def _arr(ptr, n, dtype, width=1):
     return a.reshape(n, width) if width > 1 else a
 
 
+def _collect(r, n, p):
+    m = int(r.n_rec)
+    res = OracleResult(_arr(r.xy, m, np.float32, 4), _arr(r.angle, m, np.float32), _arr(r.kind, m, np.uint8),
+                       _arr(r.seg, m, np.uint32), _arr(r.seg_count, n, np.uint32), _arr(r.path_off, p + 1, np.uint64),
+                       _arr(r.pt_off, n, np.uint32), _arr(r.path_idx, n, np.uint32), _arr(r.sp_first, n, np.uint32),
+                       dict(zip(STAT_NAMES, [int(x) for x in r.stats[:len(STAT_NAMES)]])))
+    lib().so_free(C.byref(r))
+    return res
+
+
+def piece_expand(k0, k1, L, h, tol_fl, mode, x0=0.0, y0=0.0, dir0=0.0):
+    """Both sides of ONE Euler-spiral piece given by its parameters (so_piece_expand): for the pins that measure
+    the emitted arcs / evolute chords against the exact spiral."""
+    r = _Result()
+    rc = lib().so_piece_expand(k0, k1, L, x0, y0, dir0, h, tol_fl, int(mode), C.byref(r))
+    if rc != 0:
+        raise ValueError(f"oracle so_piece_expand failed: {rc}")
+    return _collect(r, 1, 1)
+
+
 def expand(tags, points, styles, affine, tolerance, mode):
     """Run the oracle on host numpy streams; returns OracleResult (copies; C buffers are freed)."""
     L = lib()
@@ -87,10 +109,4 @@ def expand(tags, points, styles, affine, tolerance, mode):
                      affine.ctypes.data, float(tolerance), int(mode), C.byref(r))
     if rc != 0:
         raise ValueError(f"oracle so_expand failed: {rc}")
-    m = int(r.n_rec)
-    res = OracleResult(_arr(r.xy, m, np.float32, 4), _arr(r.angle, m, np.float32), _arr(r.kind, m, np.uint8),
-                       _arr(r.seg, m, np.uint32), _arr(r.seg_count, n, np.uint32), _arr(r.path_off, p + 1, np.uint64),
-                       _arr(r.pt_off, n, np.uint32), _arr(r.path_idx, n, np.uint32), _arr(r.sp_first, n, np.uint32),
-                       dict(zip(STAT_NAMES, [int(x) for x in r.stats[:len(STAT_NAMES)]])))
-    L.so_free(C.byref(r))
-    return res
+    return _collect(r, n, p)

@@ -16,8 +16,9 @@
  * double from those fp32 parameters (Euler-spiral integral by 16-point Gauss-Legendre) and rounded
  * to fp32 once: this is the definition the fp32 kernels must reproduce within 1e-3 px.
  *
- * Parity pins live in tests/test_oracle_*.py.  "parity unpinned": the three-term
- * cubic->ES error estimate of section 7.1 against the paper's "mean ratio 1.656" claim (only pinned
+ * Parity pins live in tests/test_oracle_*.py (arc-mode counts of section 5 and evolute counts of section 6:
+ * tests/test_oracle_pins.py, measured against the exact spiral).  "parity unpinned": the
+ * three-term cubic->ES error estimate of section 7.1 against the paper's "mean ratio 1.656" claim (only pinned
  * through the tolerance invariant), and the constants EPS_Q, DELTA_T, DT_MIN, the |theta|>120deg
  * guard (exercised through invariants on degenerate inputs only).
  */
@@ -83,6 +84,10 @@ static float dotf(v2f a, v2f b) { return a.x * b.x + a.y * b.y; }
 static float crossf(v2f a, v2f b) { return a.x * b.y - a.y * b.x; }
 static float len2(v2f a) { return a.x * a.x + a.y * a.y; }
 static v2f unit(v2f a) { float l = sqrtf(len2(a)); return v2(a.x / l, a.y / l); }
+/* Angles (R-17): the fp32 value nearest to the angle of the vector (x, y), i.e. atan2 evaluated in
+ * double and rounded once.  This makes th0, th1 (hence k0, k1, L and everything derived from them) independent of
+ * any particular libm's single-precision atan2f rounding. */
+static float atan2_r(float y, float x) { return (float)atan2((double)y, (double)x); }
 
 /* ------------------------------------------------------------------ Gauss-Legendre nodes (double) */
 #define GLN 16
@@ -224,7 +229,7 @@ float so_fit_error(v2f u0, v2f u1, float q0mag, float q1mag, v2f ch, float dt, f
     v2f uc = v2(ch.x / chord, ch.y / chord);
     float s0 = crossf(u0, uc), c0 = dotf(u0, uc); /* sin, cos of th0 = angle from start tangent to chord */
     float s1 = crossf(uc, u1), c1 = dotf(uc, u1); /* th1 = angle from chord to end tangent */
-    float th0 = atan2f(s0, c0), th1 = atan2f(s1, c1);
+    float th0 = atan2_r(s0, c0), th1 = atan2_r(s1, c1); /* R-17 */
     *th0_out = th0;
     *th1_out = th1;
     if (c0 < -0.5f || c1 < -0.5f) return 2.0f * chord; /* outside the validated box: force a split (R-4) */
@@ -420,15 +425,19 @@ static int evolute_params(const ctx_t* c, const piece_t* p, float ta, float tb, 
  * ranges, super-critical ranges with evolute patch. */
 static void side_records(ctx_t* c, const piece_t* p, float eta, reclist* out) {
     float g0 = 1.0f - es_kappa(p, 0.0f) * eta, g1 = 1.0f - es_kappa(p, 1.0f) * eta; /* cusp0, cusp1 (L382-384) up to a positive factor */
-    float tc = (g0 * g1 >= 0.0f) ? 1.0f : g0 / (g0 - g1);                              /* L386 */
+    /* L386.  The cusp is inside the piece iff g0 and g1 have strictly opposite signs (decided from the signs, not
+     * from the product: g0 == 0 with g1 < 0 is a piece that is super-critical over its whole length). */
+    int has_cusp = (g0 > 0.0f && g1 < 0.0f) || (g0 < 0.0f && g1 > 0.0f);
+    float tc = has_cusp ? g0 / (g0 - g1) : 1.0f;
+    int first_sup = g0 < 0.0f || (g0 == 0.0f && g1 < 0.0f);
     float ranges[2][2];
     int sup[2], nr = 0;
-    if (g0 >= 0.0f) { ranges[nr][0] = 0.0f; ranges[nr][1] = tc; sup[nr] = 0; nr++; }      /* L388-392: regular on [0,t] */
-    if (g0 < 0.0f || tc < 1.0f) {                                                          /* L397-403: evolute patch */
-        if (g0 >= 0.0f) { ranges[nr][0] = tc; ranges[nr][1] = 1.0f; } else { ranges[nr][0] = 0.0f; ranges[nr][1] = tc; }
+    if (!first_sup) { ranges[nr][0] = 0.0f; ranges[nr][1] = tc; sup[nr] = 0; nr++; }      /* L388-392: regular on [0,t] */
+    if (first_sup || tc < 1.0f) {                                                          /* L397-403: evolute patch */
+        if (!first_sup) { ranges[nr][0] = tc; ranges[nr][1] = 1.0f; } else { ranges[nr][0] = 0.0f; ranges[nr][1] = tc; }
         sup[nr] = 1; nr++;
     }
-    if (g0 < 0.0f && tc < 1.0f) { ranges[nr][0] = tc; ranges[nr][1] = 1.0f; sup[nr] = 0; nr++; } /* L407-411: regular on [t,1] */
+    if (first_sup && tc < 1.0f) { ranges[nr][0] = tc; ranges[nr][1] = 1.0f; sup[nr] = 0; nr++; } /* L407-411: regular on [t,1] */
     for (int r = 0; r < nr; r++) {
         float ta = ranges[r][0], tb = ranges[r][1];
         float* ts;
@@ -461,13 +470,8 @@ static void side_records(ctx_t* c, const piece_t* p, float eta, reclist* out) {
     }
 }
 
-static int emit_piece(ctx_t* c, piece_t* p, float h) {
-    float cc;
-    so_ghi(p->th0, p->th1, &p->k1, &cc);
-    p->k0 = p->th0 + p->th1;
-    if (!(cc > 0.05f)) cc = 0.05f; /* far outside the polynomial's range (|theta| near pi): keep L finite */
-    p->L = p->chord / cc;
-    if (!(p->L > 1e-12f)) p->L = 1e-12f; /* zero-length piece accepted at DT_MIN */
+/* both sides of a piece whose k0, k1, L are set */
+static int piece_records(ctx_t* c, piece_t* p, float h) {
     so_es_integral(p->k0, p->k1, 1.0, &p->z1x, &p->z1y);
     c->out->stats[ST_PIECES]++;
     reclist l = {0, 0, 0};
@@ -482,6 +486,16 @@ static int emit_piece(ctx_t* c, piece_t* p, float h) {
         if (push_rec(c, l.r[i - 1].b, l.r[i - 1].a, c->mode == MODE_ARC ? -l.r[i - 1].angle : 0.0, l.r[i - 1].kind | K_PLUS)) return -1;
     free(l.r);
     return 0;
+}
+
+static int emit_piece(ctx_t* c, piece_t* p, float h) {
+    float cc;
+    so_ghi(p->th0, p->th1, &p->k1, &cc);
+    p->k0 = p->th0 + p->th1;
+    if (!(cc > 0.05f)) cc = 0.05f; /* far outside the polynomial's range (|theta| near pi): keep L finite */
+    p->L = p->chord / cc;
+    if (!(p->L > 1e-12f)) p->L = 1e-12f; /* zero-length piece accepted at DT_MIN */
+    return piece_records(c, p, h);
 }
 
 /* ================================================================== segments */
@@ -643,7 +657,7 @@ static int emit_join(ctx_t* c, const so_style* st, v2f Vf, v2f T0, v2f Wf, v2f T
     int outer_minus = (cr > 0.0f) || (cr == 0.0f && dt < 0.0f);
     v2d A = offset_point(V, T0, -h), B = offset_point(W, T1, -h);
     v2d Bp = offset_point(W, T1, h), Ap = offset_point(V, T0, h);
-    float phi = fabsf(atan2f(cr, dt));
+    float phi = fabsf(atan2_r(cr, dt));
     float opd = 1.0f + dt;
     int miter_ok = (opd > 1e-6f) && (2.0f / opd <= st->miter_limit * st->miter_limit); /* 1/sin(beta/2) <= limit */
     for (int side = 0; side < 2; side++) {
@@ -769,4 +783,36 @@ void so_fit_error_export(const float* u0, const float* u1, float q0mag, float q1
     float th0, th1, chord;
     float e = so_fit_error(v2(u0[0], u0[1]), v2(u1[0], u1[1]), q0mag, q1mag, v2(ch[0], ch[1]), dt, &th0, &th1, &chord);
     out4[0] = th0; out4[1] = th1; out4[2] = chord; out4[3] = e;
+}
+
+/* One Euler-spiral piece given directly by its parameters (for the pins of sections 5 and 6, which measure the
+ * emitted arcs / evolute chords against the exact spiral): unit-arc curvature kappa(s) = k0 + k1 s on [-1/2,1/2]
+ * (R-1), arc length L px, starting at (x0, y0) with tangent angle dir0; both sides at half-width h, flatten
+ * tolerance tol_fl (the TOL_FL of R-13, given directly), in canonical order.  Same code path as a piece accepted by
+ * Alg. 2 from here on (piece_records). */
+int so_piece_expand(float k0, float k1, float L, float x0, float y0, float dir0, float h, float tol_fl, int mode, so_result* out) {
+    memset(out, 0, sizeof(*out));
+    out->seg_count = (uint32_t*)calloc(2, sizeof(uint32_t));
+    out->path_off = (uint64_t*)calloc(2, sizeof(uint64_t));
+    out->pt_off = (uint32_t*)calloc(2, sizeof(uint32_t));
+    out->path_idx = (uint32_t*)calloc(2, sizeof(uint32_t));
+    out->sp_first = (uint32_t*)calloc(2, sizeof(uint32_t));
+    ctx_t c;
+    c.out = out; c.mode = mode; c.tol_es = 0; c.tol_fl = tol_fl; c.cur_seg = 0;
+    piece_t p;
+    memset(&p, 0, sizeof(p));
+    p.k0 = k0; p.k1 = k1; p.L = L;
+    double zx, zy;
+    so_es_integral(k0, k1, 1.0, &zx, &zy);
+    double cd = cos((double)dir0), sd = sin((double)dir0);
+    p.ua = v2((float)cd, (float)sd);
+    p.ub = v2((float)cos((double)dir0 + (double)k0), (float)sin((double)dir0 + (double)k0)); /* phi(1) = k0 */
+    p.ch = v2((float)((double)L * (cd * zx - sd * zy)), (float)((double)L * (sd * zx + cd * zy)));
+    p.pa.x = x0; p.pa.y = y0;
+    p.pb.x = (double)x0 + (double)p.ch.x; p.pb.y = (double)y0 + (double)p.ch.y;
+    p.chord = sqrtf(len2(p.ch));
+    if (piece_records(&c, &p, h)) { so_free(out); return -1; }
+    out->seg_count[0] = (uint32_t)out->n_rec;
+    out->path_off[1] = out->n_rec;
+    return 0;
 }

@@ -1,0 +1,158 @@
+"""Pins for the oracle's arc-mode subdivision (section 5) and evolute flattening (section 6,
+L185-197): the records of ONE Euler-spiral piece (oracle.piece_expand) are measured against the exact spiral,
+its exact parallel curve and its exact evolute, all built here by double-precision quadrature -- geometry the
+oracle does not compute.  A wrong constant in either count formula (120, the (1 + 0.4 |h s kappa'|) factor,
+8 TOL_FL) moves the measured deviation out of the bands below.  Also the cusp-split boundary case kappa(0) eta == 1.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import checkers as ck
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "es_arc_and_evolute_counts.txt")
+K_OFFSET, K_OFFSET_REV, K_EVOLUTE, K_CONNECTOR, K_PLUS = 0, 1, 2, 3, 8
+
+
+def exact_spiral(k0, k1, L, n=40001):
+    """The spiral kappa(t) = (k0 + k1 (t - 1/2)) / L from the origin along +x: parameter, position (complex),
+    tangent angle, curvature.  Cumulative Simpson on a fine grid (error ~1e-13 of L)."""
+    t = np.linspace(0.0, 1.0, n)
+    th = (k0 - 0.5 * k1) * t + 0.5 * k1 * t * t
+    e = np.exp(1j * th)
+    tm = 0.5 * (t[1:] + t[:-1])
+    em = np.exp(1j * ((k0 - 0.5 * k1) * tm + 0.5 * k1 * tm * tm))
+    z = np.concatenate([[0.0], np.cumsum((e[:-1] + 4.0 * em + e[1:]) * (t[1] - t[0]) / 6.0)])
+    return t, L * z, th, (k0 + k1 * (t - 0.5)) / L
+
+
+def golden(kind):
+    for line in open(GOLD):
+        f = line.split()
+        if f and f[0] == kind:
+            return [float(v) for v in f[1:]]
+    raise KeyError(kind)
+
+
+def arc_deviation(k0, k1, L, h, tol_fl, plus):
+    """(records, max distance from points ON the emitted arcs to the exact parallel curve) of one side."""
+    r = oracle.piece_expand(k0, k1, L, h, tol_fl, 1)
+    t, P, th, kap = exact_spiral(k0, k1, L)
+    O = P + (h if plus else -h) * 1j * np.exp(1j * th)
+    m = r.kind == (K_OFFSET | (K_PLUS if plus else 0))
+    on_arcs = ck.arcs_to_lines(r.xy[m].astype(np.float64), r.angle[m].astype(np.float64), n=24)[:, 0:2]
+    return int(m.sum()), float(ck.dist_points_to_polyline(on_arcs, np.stack([O.real, O.imag], 1)[::4]).max())
+
+
+def evolute_deviation(k0, k1, L, h, tol_fl):
+    """[(records per copy, max distance from the exact evolute to the emitted evolute polyline)] per side with a
+    super-critical range.  Exact evolute E = P + N / kappa (L193) over the part of the piece where kappa eta > 1."""
+    r = oracle.piece_expand(k0, k1, L, h, tol_fl, 0)
+    t, P, th, kap = exact_spiral(k0, k1, L)
+    out = []
+    for plus in (False, True):
+        m = ((r.kind & 7) == K_EVOLUTE) & (((r.kind & K_PLUS) != 0) == plus)
+        if not m.any():
+            continue
+        sup = kap * (h if plus else -h) > 1.0
+        E = P[sup] + 1j * np.exp(1j * th[sup]) / kap[sup]
+        ev = r.xy[m].astype(np.float64)
+        half = len(ev) // 2
+        assert np.array_equal(ev[:half], ev[half:])                       # "output twice" (L197)
+        assert np.array_equal(ev[1:half, 0:2], ev[:half - 1, 2:4])        # a connected polyline
+        chain = np.concatenate([ev[:half, 0:2], ev[half - 1:half, 2:4]])
+        out.append((half, float(ck.dist_points_to_polyline(np.stack([E.real, E.imag], 1)[::4], chain).max())))
+    return out
+
+
+# ---------------------------------------------------------------- section 5: parallel curve -> arcs (L171-177)
+def test_arc_count_and_error_of_the_survey_row():
+    k0, k1, L, h, d, n_real, n, err = golden("arc")
+    for plus in (False, True):
+        got_n, dev = arc_deviation(k0, k1, L, h, d, plus)
+        assert got_n == int(n)
+        assert 0.8 * err <= dev <= 1.02 * err, dev      # measured 0.128 / 0.133 px against 0.1432 px predicted (L173: O(1/n^3))
+
+
+def _regular_sides(seed, count):
+    """random pieces in the range Alg. 2 accepts (|k0| <= 2.5, |k1| <= 8) with a side that stays sub-critical"""
+    rng = np.random.default_rng(seed)
+    out = []
+    while len(out) < count:
+        k0, k1, L, h = rng.uniform(-2.5, 2.5), rng.uniform(-8, 8), rng.uniform(10, 200), rng.uniform(1, 60)
+        for plus in (False, True):
+            eta = h if plus else -h
+            if max((k0 - 0.5 * k1) / L * eta, (k0 + 0.5 * k1) / L * eta) < 0.97:
+                out.append((k0, k1, L, h, plus))
+    return out[:count]
+
+
+def test_arc_deviation_uses_the_tolerance_and_keeps_it():
+    """L171-177: n = s cbrt(|kappa'| (1 + 0.4 |h s kappa'|) / (120 d)).  Measured on 160 random regular sides: the arcs
+    stay within 1.15 d of the exact parallel curve (99 % within d) -- which fails without the (1 + 0.4 |h s kappa'|)
+    factor (measured up to 1.57 d) or with a larger constant than 120 -- and they USE the budget: median deviation
+    above 0.35 d, which fails with a smaller constant (120 -> 12 gives 0.06 d)."""
+    d = 0.2
+    ratio = np.array([arc_deviation(k0, k1, L, h, d, plus)[1] / d for k0, k1, L, h, plus in _regular_sides(1, 160)])
+    assert ratio.max() <= 1.15, ratio.max()
+    assert np.quantile(ratio, 0.97) <= 1.0
+    assert 0.35 <= np.median(ratio) <= 0.8, np.median(ratio)
+
+
+def test_arc_h_factor_matters_on_strongly_offset_sides():
+    """The sides where |h s kappa'| is large are exactly those that break the bound without the factor of L177."""
+    d = 0.2
+    sides = [s for s in _regular_sides(2, 600) if 0.4 * abs(s[3] * s[1]) / s[2] > 0.8]
+    assert len(sides) >= 40
+    ratio = np.array([arc_deviation(k0, k1, L, h, d, plus)[1] / d for k0, k1, L, h, plus in sides[:60]])
+    assert ratio.max() <= 1.15 and np.median(ratio) >= 0.25, (ratio.max(), np.median(ratio))
+
+
+# ---------------------------------------------------------------- section 6: evolute -> lines (L195)
+def test_evolute_count_and_error_of_the_survey_row():
+    k0, k1, L, h, d, n_real, n, err = golden("evolute")
+    (got_n, dev), = evolute_deviation(k0, k1, L, h, d)
+    assert got_n == int(n)
+    assert abs(dev - err) <= 0.02 * err, dev            # d (n_real / n)^2: the density constant of L195 is exactly 1
+
+
+def test_evolute_chords_use_the_tolerance_and_keep_it():
+    """L195 + L77-83: evolute chords deviate by d (n_real / n)^2 <= d.  On random pieces with a super-critical range:
+    never above 1.05 d (8 TOL_FL -> 80 TOL_FL gives up to 10 d), and the median above 0.45 d (8 -> 0.8 gives 0.07 d)."""
+    rng = np.random.default_rng(3)
+    d, ratio = 0.2, []
+    while len(ratio) < 60:
+        k0, k1, L, h = rng.uniform(-2.5, 2.5), rng.uniform(-8, 8), rng.uniform(20, 200), rng.uniform(20, 100)
+        if abs(k1) < 0.5:
+            continue
+        ratio += [dev / d for n, dev in evolute_deviation(k0, k1, L, h, d) if n >= 2]
+    ratio = np.array(ratio)
+    assert ratio.max() <= 1.05, ratio.max()
+    assert 0.45 <= np.median(ratio) <= 0.95, np.median(ratio)
+
+
+# ---------------------------------------------------------------- section 7.3.1: cusp split at the boundary
+def test_piece_that_starts_exactly_at_the_cusp_is_supercritical_throughout():
+    """kappa(0) eta == 1 exactly (k0 = 1, k1 = 1, L = 4: kappa(0) = 0.125; eta = 8) and kappa(1) eta = 3: the +h side
+    runs backwards over the whole piece (L267: at most one cusp, here at t = 0) -> reversed offset + evolute patch,
+    no forward offset record; the -h side is regular."""
+    r = oracle.piece_expand(1.0, 1.0, 4.0, 8.0, 0.2, 0)
+    plus = (r.kind & K_PLUS) != 0
+    k3 = r.kind & 7
+    assert not (plus & (k3 == K_OFFSET)).any()
+    assert (plus & (k3 == K_OFFSET_REV)).sum() >= 1 and (plus & (k3 == K_EVOLUTE)).sum() >= 2
+    assert ((~plus) & (k3 == K_OFFSET)).sum() >= 1 and ((~plus) & (k3 != K_OFFSET)).sum() == 0
+    # the patch is closed: the side's records chain from the offset point at t = 1 back to the one at t = 0
+    assert ck.watertight_violations(np.concatenate([r.xy[plus], [[*r.xy[plus][-1, 2:4], *r.xy[plus][0, 0:2]]]]),
+                                    np.array([0, plus.sum() + 1])) == 0
+
+
+def test_evolute_of_a_nearly_circular_piece():
+    """The small-curvature-variation branch of the evolute count (constant density, R-7 applied to L195):
+    k1 / k0 = 1 % and a tolerance small enough that the count is not 1."""
+    d = 1e-4
+    (n, dev), = evolute_deviation(2.0, 0.02, 50.0, 40.0, d)
+    assert n >= 20
+    assert 0.4 * d <= dev <= 1.05 * d, (n, dev)
