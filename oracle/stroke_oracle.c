@@ -339,6 +339,10 @@ static v2d es_evolute(const piece_t* p, float t) {
     return r;
 }
 
+/* v -> sgn(v) |v|^1.5 and its inverse: the integral of sqrt|v| and the s ~ i^(2/3) rule of section 2.2 (L97) */
+static float pow15(float v) { float a = fabsf(v), w = a * sqrtf(a); return v < 0 ? -w : w; }
+static float pow15_inv(float w) { float c = cbrtf(fabsf(w)); c = c * c; return w < 0 ? -c : c; }
+enum { RULE_UNIFORM = 0, RULE_F_APPROX = 1, RULE_INFLECTION = 2, RULE_CUSP = 3 };
 static float clampf(float x, float lo, float hi) { return x < lo ? lo : (x > hi ? hi : x); }
 static float count_clamp(float n) { if (!(n >= 1.0f)) return 1.0f; return n > N_MAX ? N_MAX : n; }
 
@@ -347,7 +351,7 @@ static float count_clamp(float n) { if (!(n >= 1.0f)) return 1.0f; return n > N_
 static int offset_params(const ctx_t* c, const piece_t* p, float eta, float ta, float tb, float** ts_out) {
     float n_f;
     float ua = 0, ub = 0;
-    int uniform = 1;
+    int rule = RULE_UNIFORM;
     float ah = fabsf(eta);
     if (c->mode == MODE_ARC) {
         /* L177: n = s cbrt(|k'|(1+0.4|h s k'|)/(120 d)), s=L, k'=k1/L^2; scaled by the range fraction (R-12) */
@@ -357,16 +361,34 @@ static int offset_params(const ctx_t* c, const piece_t* p, float eta, float ta, 
         float ka = es_kappa(p, ta), kb = es_kappa(p, tb);
         float xa = 2.0f * eta * ka - 1.0f, xb = 2.0f * eta * kb - 1.0f; /* L125: inflection -> -1, cusp -> +1 */
         float xm = 0.5f * (xa + xb);
+        float kp = fabsf(p->k1) / (p->L * p->L);
         if (fabsf(xb - xa) < 0.015625f * fmaxf(1.0f, fabsf(xm))) {
-            /* small curvature variation: constant density sqrt|k(1-k eta)| (R-7; limit is L73) */
-            float km = 0.5f * (ka + kb);
-            n_f = ceilf((tb - ta) * p->L * sqrtf(fabsf(km * (1.0f - km * eta)) / (8.0f * c->tol_fl)));
+            /* x varies too little over the range for the difference of two f_approx values in fp32 (R-7): the density
+             * sqrt|k (1 - k eta)| (L77-83, L131) is integrated locally instead.  km, gm: curvature and cusp factor at the
+             * middle of the range; m_infl, m_cusp: how far km is from the inflection (k = 0) and from the cusp (k = 1/eta). */
+            float km = 0.5f * (ka + kb), dk = fabsf(kb - ka);
+            float gm = 1.0f - km * eta;
+            float m_infl = fabsf(km), m_cusp = fabsf(gm) / ah;
+            if (dk <= 0.125f * fminf(m_infl, m_cusp)) {
+                /* neither zero of the density is near: constant density (limit: the circular arc, L73) */
+                n_f = ceilf((tb - ta) * p->L * sqrtf(fabsf(km * gm) / (8.0f * c->tol_fl)));
+            } else if (m_infl <= m_cusp) {
+                /* an inflection in or next to the range: int sqrt|k| ds = 2/3 |k|^1.5 / k' (section 2.2: the
+                 * subdivision points follow s_i ~ i^(2/3) from the inflection), the factor sqrt|1 - k eta| at the middle */
+                ua = pow15(ka); ub = pow15(kb);
+                n_f = ceilf((2.0f / 3.0f) * fabsf(ub - ua) * sqrtf(fabsf(gm)) / (kp * sqrtf(8.0f * c->tol_fl)));
+                rule = RULE_INFLECTION;
+            } else {
+                /* the range ends next to the cusp: the same with g = 1 - k eta (ds = dg / (eta k')), sqrt|k| at the middle */
+                ua = pow15(1.0f - ka * eta); ub = pow15(1.0f - kb * eta);
+                n_f = ceilf((2.0f / 3.0f) * fabsf(ub - ua) * sqrtf(fabsf(km)) / (ah * kp * sqrtf(8.0f * c->tol_fl)));
+                rule = RULE_CUSP;
+            }
         } else {
             ua = so_f_approx(xa);
             ub = so_f_approx(xb);
-            float kp = fabsf(p->k1) / (p->L * p->L);
             n_f = ceilf(fabsf(ub - ua) / (4.0f * kp * ah * sqrtf(ah) * sqrtf(8.0f * c->tol_fl))); /* L83 with density sqrt|1-x^2|/(2 sqrt|h|) */
-            uniform = 0;
+            rule = RULE_F_APPROX;
         }
     }
     int n = (int)count_clamp(n_f);
@@ -376,11 +398,12 @@ static int offset_params(const ctx_t* c, const piece_t* p, float eta, float ta, 
     for (int i = 1; i < n; i++) {
         float fr = (float)i / (float)n;
         float t;
-        if (uniform) t = ta + fr * (tb - ta);
+        if (rule == RULE_UNIFORM) t = ta + fr * (tb - ta);
         else {
-            float u = ua + fr * (ub - ua);
-            float x = so_f_approx_inv(u);
-            float kap = (x + 1.0f) / (2.0f * eta);
+            float u = ua + fr * (ub - ua), kap;
+            if (rule == RULE_F_APPROX) kap = (so_f_approx_inv(u) + 1.0f) / (2.0f * eta);
+            else if (rule == RULE_INFLECTION) kap = pow15_inv(u);
+            else kap = (1.0f - pow15_inv(u)) / eta;
             t = 0.5f + (kap * p->L - p->k0) / p->k1;
         }
         ts[i] = clampf(t, ta, tb);
