@@ -1,20 +1,27 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the stroke-expansion hot path on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c5|c3] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c5|c3|c2|c1] [--mode line|arc] [--impl ours|reference]
 
-A step is one pass of the whole hot path (tag scan -> count -> allocation scan -> write) over one synthetic scene
-(default: config 4, the CAD-scale scene BASELINE.json's target is quoted on: 1,000,000 segments, arc output,
-tolerance 0.1).  `value` is input segments per second with the streams resident in HBM, device-timed with CUDA
-events on the launching stream (L2 flushed between steps); `e2e` is the same metric through the host-buffer C-ABI
-call with the H2D / D2H copies inside the timed region.  `--impl reference` times the CPU oracle instead.
-Prints ONE JSON line (rank 0).
+A step is one pass of the whole hot path -- kernel (a) tag scan, then the expansion kernel: (b) count, (c) allocation scan,
+(d) write, fused -- over one synthetic scene (default: config 4, the CAD-scale scene BASELINE.json's target is quoted on:
+1,000,000 segments, arc output, tolerance 0.1), through the C-ABI call `stroke_expand_into`.  `value` is input segments
+per second with the streams resident in HBM, device-timed with CUDA events on the launching stream (L2 flushed between
+steps); `e2e` is the same metric through the host-buffer C-ABI call with the H2D / D2H copies inside the timed region.
+`roofline` is the dominant kernel (the expansion kernel, timed by the library's own events on the launching stream)
+against the measured HBM peak; `roofline.whole_step` is T_roof / T_step with the three ceilings of SURVEY 8(d)
+(algorithmic bytes / measured HBM bandwidth, FP32 lane-operations / measured FFMA issue rate, MUFU operations / measured
+MUFU rate), the unit counts taken from the instrumented oracle on a sample of the scene.  `--impl reference` times the CPU
+oracle instead.  Prints ONE JSON line (rank 0).  With --gpus N > 1 and no torchrun environment, bench.py starts the N
+replicas itself (torch.distributed.run, one process per GPU).
 """
 from __future__ import annotations
 
 import argparse
 import json
+import multiprocessing as mp
 import os
+import subprocess
 import sys
 import threading
 import time
@@ -28,10 +35,15 @@ if ROOT not in sys.path:
 METRIC = "input path segments/sec expanded (device-timed)"
 UNIT = "segments/s"
 MODE_OF = {"c3": 0, "c4": 1, "c5": 0, "c1": 0, "c2": 0}
-# dram__bytes_read.sum + dram__bytes_write.sum of the write pass per launch, from the committed ncu captures
-# (profiles/r1_final.md); None = not captured for that workload
-NCU_TRAFFIC = {"c4": 519.2e6, "c5": None}  # c4: 362.7 MB k_write_pieces + 156.5 MB k_write_segments (profiles/r1_final.md)
+# whole-step dram__bytes_read.sum + dram__bytes_write.sum per step from the committed `ncu --set full` captures
+# (profiles/r2_counters.md names the command and the commit of each); None = not captured for that workload / mode
+NCU_TRAFFIC = {}
+NCU_TRAFFIC_SOURCE = "profiles/r2_counters.md"
 REF_SAMPLE_PATHS = {"c4": 20000, "c5": 1000, "c3": 20000, "c1": 256, "c2": 2000}
+# issue slots (FMA = 1) and special-function operations per unit of the method's own work
+SLOTS = {"fit_iter": (110, 7), "piece": (60, 2), "range_line": (30, 5), "range_arc": (12, 2), "vertex_line": (65, 4),
+         "record_arc": (55, 3), "vertex_evolute": (60, 4), "join": (40, 4), "round_vertex": (6, 0), "cap": (20, 2)}
+FP32_THEORETICAL = 148 * 128 * 1.965e9
 
 
 def load_peaks():
@@ -43,11 +55,12 @@ def load_peaks():
 
 
 class ClockSampler(threading.Thread):
-    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+    """Samples SM clock and throttle reasons through NVML; start() returns once the first sample is in."""
 
     def __init__(self, index):
         super().__init__(daemon=True)
-        self.index, self.samples, self.reasons, self.max_mhz, self._stop_evt = index, [], set(), None, threading.Event()
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt, self._ready, self._mark = threading.Event(), threading.Event(), None
 
     def run(self):
         try:
@@ -58,17 +71,30 @@ class ClockSampler(threading.Thread):
             names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
                      "hw_power_brake_slowdown": 0x80, "sync_boost": 0x10, "applications_clocks_setting": 0x2}
             while not self._stop_evt.is_set():
-                self.samples.append(int(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                mhz = int(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
                 try:
                     r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(h))
                 except Exception:
                     r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(h))
-                for k, bit in names.items():
-                    if r & bit:
-                        self.reasons.add(k)
-                time.sleep(0.002)
+                if self._mark is not None:
+                    self.samples.append(mhz)
+                    for k, bit in names.items():
+                        if r & bit:
+                            self.reasons.add(k)
+                self._ready.set()
+                time.sleep(0.001)
         except Exception as e:  # no NVML: report that, never fake numbers
             self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+            self._ready.set()
+
+    def begin(self):
+        """Start the thread (before the warm-up) and wait for NVML to answer."""
+        self.start()
+        self._ready.wait(timeout=10)
+
+    def mark(self):
+        """Samples taken from now on belong to the timed region."""
+        self._mark = time.perf_counter()
 
     def stop(self):
         self._stop_evt.set()
@@ -98,40 +124,99 @@ def make_scene(workload, n_paths=None):
     return S.make(workload, n_paths=n_paths)
 
 
-def time_oracle(sc, mode, reps=1):
+# ---------------------------------------------------------------- the oracle on the host cores
+def _oracle_chunk(job):
     import oracle
-    best, r = None, None
+    tags, points, styles, affine, tol, mode = job
+    t0 = time.perf_counter()
+    r = oracle.expand(tags, points, styles, affine, tol, mode)
+    return time.perf_counter() - t0, r.n_rec, r.stats
+
+
+def oracle_jobs(sc, mode, n_chunks):
+    """The scene cut into n_chunks runs of whole paths (paths are independent units)."""
+    from paper_2405_00127_b200 import scenes as S
+    bounds = np.linspace(0, sc.n_paths, n_chunks + 1).astype(int)
+    jobs = []
+    for a, b in zip(bounds[:-1], bounds[1:]):
+        if b > a:
+            sub, _ = S.subset_paths(sc, np.arange(a, b))
+            jobs.append((sub.tags, sub.points, sub.styles, sub.affine, float(sub.tolerance), mode))
+    return jobs
+
+
+def time_oracle(jobs, pool=None, reps=1):
+    """Wall-clock seconds of the oracle over the jobs (oracle_jobs: the scene cut into runs of whole paths, one per
+    process of the pool), best of reps; records; summed unit counts."""
+    best, out = None, None
     for _ in range(reps):
         t0 = time.perf_counter()
-        r = oracle.expand(sc.tags, sc.points, sc.styles, sc.affine, sc.tolerance, mode)
+        res = [_oracle_chunk(j) for j in jobs] if pool is None else pool.map(_oracle_chunk, jobs)
         dt = time.perf_counter() - t0
-        best = dt if best is None else min(best, dt)
-    return best, r
+        if best is None or dt < best:
+            best, out = dt, res
+    stats = {}
+    for _, _, st in out:
+        for k, v in st.items():
+            stats[k] = stats.get(k, 0) + v
+    return best, sum(r[1] for r in out), stats
+
+
+def make_pool(cores):
+    if cores <= 1:
+        return None
+    pool = mp.get_context("fork").Pool(cores)
+    pool.map(abs, range(cores))  # the workers are up before anything is timed
+    return pool
 
 
 def run_reference(args):
-    """The oracle, as it stands, on the host cores (single thread), each step a bounded sample of the workload."""
+    """The oracle, as it stands, on all host cores (one process per core over runs of whole paths); each step a bounded
+    sample of the workload."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
+    import oracle
+    oracle.build()
     mode = MODE_OF[args.workload] if args.mode is None else int(args.mode == "arc")
-    npaths = REF_SAMPLE_PATHS[args.workload]
+    cores = os.cpu_count() or 1
+    npaths = REF_SAMPLE_PATHS[args.workload] * (4 if cores >= 8 else 1)
     sc = make_scene(args.workload, n_paths=npaths)
-    for _ in range(args.warmup):
-        time_oracle(sc, mode)
+    pool = make_pool(cores)
+    jobs = oracle_jobs(sc, mode, cores)
+    for _ in range(max(args.warmup, 1)):
+        time_oracle(jobs, pool)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        _, r = time_oracle(sc, mode)
+        _, n_rec, _ = time_oracle(jobs, pool)
     dt = time.perf_counter() - t0
+    if pool is not None:
+        pool.close()
     value = sc.n_segments * args.steps / dt
-    sample = f"first {npaths} paths of {args.workload} ({sc.n_segments} segments -> {r.n_rec} records) per step"
+    sample = f"first {sc.n_paths} paths of {args.workload} ({sc.n_segments} segments -> {n_rec} records) per step, {cores} processes over runs of whole paths"
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": args.workload, "mode": "arc" if mode else "line", "tolerance": float(sc.tolerance), "sample": sample},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
+
+
+def unit_work(stats, kinds, mode, scale):
+    """I_fp32, I_mufu of SURVEY 8(d) from the instrumented oracle's unit counts (scaled from the sample to the scene)."""
+    k3 = kinds & 7
+    n_join_outer, n_cap = int((k3 == 4).sum()), int((k3 == 6).sum())
+    joins = stats["joins"] // 2
+    units = {"fit_iter": stats["fit_iters"], "piece": stats["pieces"],
+             "range_arc" if mode else "range_line": stats["ranges_reg"] + stats["ranges_sup"],
+             "record_arc" if mode else "vertex_line": stats["rec_offset"],
+             "vertex_evolute": stats["rec_evolute"] // 2 + stats["rec_connector"] // 2,
+             "join": joins, "cap": stats["caps"],
+             "round_vertex": max(0, n_join_outer - joins) + max(0, n_cap - stats["caps"])}
+    i_fp32 = sum(SLOTS[k][0] * v for k, v in units.items()) * scale
+    i_mufu = sum(SLOTS[k][1] * v for k, v in units.items()) * scale
+    return i_fp32, i_mufu, {k: int(v * scale) for k, v in units.items()}
 
 
 def run_ours(args):
@@ -153,6 +238,9 @@ def run_ours(args):
     n_seg, n_paths = sc.n_segments, sc.n_paths
     tags, pts, sty = B.scene_to_torch(sc, device=dev)
     width = 8 if mode else 4
+    sampler = ClockSampler(local)
+    sampler.begin()
+    issue = B.sx_measure_issue_peaks(local)
     ctx = B.sx_create(local)
     stream = torch.cuda.current_stream()
     poff = torch.empty(n_paths + 1, dtype=torch.int64, device=dev)
@@ -160,21 +248,17 @@ def run_ours(args):
     out = torch.empty((total, width), dtype=torch.float32, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
 
-    def step(ev=None):
-        if ev:
-            ev[0].record(stream)
-        B.sx_count(ctx, tags, pts, sty, sc.affine, sc.tolerance, mode, poff, want_total=False)
-        if ev:
-            ev[1].record(stream)
-        B.sx_write(ctx, out, total)
-        if ev:
-            ev[2].record(stream)
+    def step():
+        # the call a user makes when the capacity is known: one pass, asynchronous, no host round trip
+        B.stroke_expand_into(ctx, tags, pts, sty, sc.affine, sc.tolerance, mode, out, poff, want_total=False)
 
-    for _ in range(max(args.warmup, 3)):
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
         flush.fill_(1)
         step()
     torch.cuda.synchronize()
     assert B.sx_last_error(ctx) == 0
+    assert int(poff[-1].item()) == total
 
     def barrier():
         torch.cuda.synchronize()
@@ -182,28 +266,60 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(args.steps)]
     launches0 = B.sx_launch_count(ctx)
-    sampler = ClockSampler(local)
     barrier()
-    sampler.start()
+    sampler.mark()
     for k in range(args.steps):
         flush.fill_(k & 0xff)  # L2 flush between timed steps (outside the event brackets)
-        step(evs[k])
+        evs[k][0].record(stream)
+        step()
+        evs[k][1].record(stream)
     barrier()
-    clocks = sampler.stop()
     launches = B.sx_launch_count(ctx) - launches0
     assert B.sx_last_error(ctx) == 0
-    t_count = sum(e[0].elapsed_time(e[1]) for e in evs) * 1e-3
-    t_write = sum(e[1].elapsed_time(e[2]) for e in evs) * 1e-3
-    t_total = sum(e[0].elapsed_time(e[2]) for e in evs) * 1e-3
+    t_total = sum(e[0].elapsed_time(e[1]) for e in evs) * 1e-3
     t_total = max_over_ranks(t_total, world, dev)
+    # keep the GPU under the same load until the sampler has seen it (short workloads finish between two NVML polls)
+    t_end = time.perf_counter() + 0.25
+    while len(sampler.samples) < 3 and time.perf_counter() < t_end:
+        step()
+        torch.cuda.synchronize()
+    clocks = sampler.stop()
+    stats = B.sx_call_stats(ctx)
+
+    # ---- per-kernel durations: the library's own events on the launching stream, one query (sync) per step
+    B.sx_set_option(ctx, B.SX_OPT_TIME_KERNELS, 1)
+    k_steps = max(3, min(args.steps, 10))
+    t_scan = t_expand = 0.0
+    for k in range(k_steps):
+        flush.fill_(k & 0xff)
+        step()
+        a, b = B.sx_kernel_times(ctx)
+        t_scan += a * 1e-3
+        t_expand += b * 1e-3
+    B.sx_set_option(ctx, B.SX_OPT_TIME_KERNELS, 0)
+    t_scan /= k_steps
+    t_expand /= k_steps
+
+    # ---- the one-shot call with an unknown record count: count pass, host read of the total, allocation, write pass
+    o_steps = max(3, min(args.steps, 5))
+    B.stroke_expand(ctx, tags, pts, sty, sc.affine, sc.tolerance, mode)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(o_steps):
+        rec1, _ = B.stroke_expand(ctx, tags, pts, sty, sc.affine, sc.tolerance, mode)
+    torch.cuda.synchronize()
+    t_one = (time.perf_counter() - t0) / o_steps
+    assert rec1.shape[0] == total
+    del rec1
 
     # ---- end to end through the host-buffer entry point (pinned host memory, copies inside the timed region)
     htags, hpts, hsty = B.scene_to_torch(sc, pin=True)
     hout = torch.empty((total, width), dtype=torch.float32).pin_memory()
     hpoff = torch.empty(n_paths + 1, dtype=torch.int64).pin_memory()
     e2e_steps = max(3, min(args.steps, 10))
+    B.stroke_expand_host(ctx, htags, hpts, hsty, sc.affine, sc.tolerance, mode, hout, hpoff)
     B.stroke_expand_host(ctx, htags, hpts, hsty, sc.affine, sc.tolerance, mode, hout, hpoff)
     barrier()
     t0 = time.perf_counter()
@@ -218,36 +334,55 @@ def run_ours(args):
 
     if rank == 0:
         peak, peak_src = load_peaks()
-        # algorithmic bytes of the dominant kernel (write): the streams it must read + the records it must write
-        alg_bytes = tags.numel() + pts.numel() * 4 + sty.numel() + total * width * 4
-        ach = alg_bytes / (t_write / args.steps) / 1e9
-        alg_step = alg_bytes + (n_paths + 1) * 8  # + the per-path offsets written by the allocation scan
+        t_step = t_total / args.steps
+        # algorithmic bytes: the streams read once, the records and the path offsets written once
+        alg_bytes = tags.numel() + pts.numel() * 4 + sty.numel() + total * width * 4 + (n_paths + 1) * 8
+        ach = alg_bytes / t_expand / 1e9
+        key = f"{args.workload}-{'arc' if mode else 'line'}"
         line = {"metric": METRIC, "value": job_throughput(n_seg, args.steps, world, t_total), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True, "scaling": "weak",
+                "warmup": warm, "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": args.workload, "segments": n_seg, "paths": n_paths, "records": int(total),
                            "mode": "arc" if mode else "line", "tolerance": float(sc.tolerance), "l2": "flushed between steps (256 MiB fill)",
+                           "call": "stroke_expand_into (one pass: tag scan + fused count / allocation scan / write)",
                            "parallelism": "replicas only" if world > 1 else "single GPU"},
                 "output_records_per_s": job_throughput(total, args.steps, world, t_total),
-                "kernel_ms": {"scan+count+alloc_scan": 1e3 * t_count / args.steps, "write": 1e3 * t_write / args.steps},
+                "kernel_ms": {"k_tag_scan": 1e3 * t_scan, "k_expand": 1e3 * t_expand, "timed_by": "library events on the launching stream, mean of %d steps" % k_steps},
+                "tiles": stats,
                 "gpu_launches": int(launches), "clocks": clocks,
+                "one_shot": {"call": "stroke_expand (count pass, host read of the total, allocation callback, write pass)",
+                             "ms_per_call_wall": 1e3 * t_one, "value": n_seg / t_one, "unit": UNIT},
                 "e2e": {"value": job_throughput(n_seg, e2e_steps, world, t_e2e), "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                         "ms_per_step": 1e3 * t_e2e / e2e_steps},
-                "roofline": {"kernel": "write pass (d): k_write_pieces + k_write_segments, timed together around sx_write",
+                "roofline": {"kernel": "k_expand (count + allocation scan + write in one pass): %.1f %% of the step" % (100 * t_expand / (t_scan + t_expand)),
                              "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                             "traffic": NCU_TRAFFIC.get(args.workload) if args.paths is None else None,
+                             "traffic": NCU_TRAFFIC.get(key) if args.paths is None else None, "traffic_source": NCU_TRAFFIC_SOURCE,
                              "peak_source": peak_src, "algorithmic_bytes_per_launch": int(alg_bytes),
-                             "whole_step": {"achieved": alg_step / (t_total / args.steps) / 1e9, "frac": alg_step / (t_total / args.steps) / 1e9 / peak,
-                                            "algorithmic_bytes": int(alg_step)},
-                             "fp32_issue_peak_lane_ops_per_s": 148 * 128 * 1.965e9,
-                             "note": "measured regime is FP32/ALU issue, not HBM (DESIGN.md section 8, profiles/)"}}
-        # ---- the oracle timed beside it on this box's host cores (single thread), bounded sample
+                             "bytes_per_segment": alg_bytes / n_seg}}
+        # ---- the oracle timed beside it on this box's host cores: one core and all cores, bounded sample; its unit
+        # counts give the FP32 / MUFU ceilings of the whole step
         if world == 1 and not args.no_cpu_baseline:
-            npaths = REF_SAMPLE_PATHS[args.workload] * 5
-            sub = make_scene(args.workload, n_paths=min(npaths, n_paths))
-            dt, r = time_oracle(sub, mode, reps=3)
-            line["cpu_baseline"] = {"value": sub.n_segments / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                    "sample": f"first {sub.n_paths} paths of {args.workload} ({sub.n_segments} segments -> {r.n_rec} records), best of 3"}
+            cores = os.cpu_count() or 1
+            npaths = min(REF_SAMPLE_PATHS[args.workload] * 5, n_paths)
+            sub = make_scene(args.workload, n_paths=npaths)
+            dt1, n_rec, st = time_oracle(oracle_jobs(sub, mode, 1), None, reps=2)
+            pool = make_pool(cores)
+            dtn, _, _ = time_oracle(oracle_jobs(sub, mode, cores), pool, reps=3)
+            if pool is not None:
+                pool.close()
+            sample = f"first {sub.n_paths} paths of {args.workload} ({sub.n_segments} segments -> {n_rec} records), best of 2 (one core) / 3 (all cores)"
+            line["cpu_baseline"] = {"value": sub.n_segments / dtn, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                                    "one_core": {"value": sub.n_segments / dt1, "cores": 1}}
+            import oracle
+            r = oracle.expand(sub.tags, sub.points, sub.styles, sub.affine, sub.tolerance, mode)
+            i_fp32, i_mufu, units = unit_work(r.stats, r.kind, mode, n_seg / sub.n_segments)
+            ceil = {"hbm_ms": 1e3 * alg_bytes / (peak * 1e9), "fp32_ms": 1e3 * i_fp32 / issue["fp32_ffma"], "mufu_ms": 1e3 * i_mufu / issue["mufu"]}
+            bound = max(ceil, key=ceil.get)
+            line["roofline"]["whole_step"] = {
+                "t_roof_ms": ceil[bound], "t_step_ms": 1e3 * t_step, "frac": ceil[bound] / (1e3 * t_step), "bound": bound.split("_")[0],
+                "ceilings_ms": ceil, "i_fp32_lane_ops": i_fp32, "i_mufu_ops": i_mufu, "units": units,
+                "r_fp32_measured": issue["fp32_ffma"], "r_fp32_mix_measured": issue["fp32_mix"], "r_fp32_theoretical": FP32_THEORETICAL,
+                "r_mufu_measured": issue["mufu"], "slot_table": "SURVEY 8(d)", "units_from": sample}
         print(json.dumps(line), flush=True)
     B.sx_destroy(ctx)
     if world > 1:
@@ -265,6 +400,11 @@ def main():
     ap.add_argument("--mode", default=None, choices=["line", "arc"], help="override the workload's output mode")
     ap.add_argument("--paths", type=int, default=None, help="profiling only: shrink the workload to this many paths")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started by hand: become the launcher of N replicas, one process per GPU
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(29500 + os.getpid() % 1000), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
     if args.impl == "reference":
         run_reference(args)
     else:

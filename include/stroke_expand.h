@@ -8,8 +8,9 @@
  * through an Euler-spiral intermediate (section 7, Alg. 2), evolute patches where curvature
  * exceeds 1/half-width (section 6), joins and caps (Alg. 1).
  *
- * Pipeline behind these calls: (a) tag-stream scan  (b) per-segment count
- * (c) allocation scan  (d) write.  All of it runs in hand-written CUDA kernels; there is no CPU path.
+ * Pipeline behind these calls: (a) tag-stream scan, then ONE kernel that runs (b) the
+ * per-segment count, (c) the allocation scan and (d) the write with every intermediate result in shared memory.
+ * All of it runs in hand-written CUDA kernels; there is no CPU path.
  *
  * Conventions
  *  - Every function returns an sx_status (0 = OK, < 0 = error).  No exception crosses the boundary.
@@ -36,7 +37,7 @@ enum {
     SX_E_BAD_STREAM = -2,  /* malformed tag stream, detected on the device (see sx_count)              */
     SX_E_CAPACITY = -3,    /* output buffer smaller than the record count                              */
     SX_E_CUDA = -4,        /* a CUDA runtime call failed; sx_strerror gives cudaGetErrorString text    */
-    SX_E_STATE = -5        /* sx_write without a preceding successful sx_count                         */
+    SX_E_STATE = -5        /* sx_write without a preceding successful sx_count; sx_segment_info with nothing kept */
 };
 
 /* ------------------------------------------------------------------ input encoding (PAPER.md 8.2, L460-489)
@@ -107,9 +108,12 @@ sx_status sx_create(sx_ctx** out, int32_t device);
 sx_status sx_destroy(sx_ctx* ctx);
 
 /* ------------------------------------------------------------------ phase 1: scan + count + scan
- * Runs kernels (a) tag-stream scan, (b) per-segment count (Alg. 1/2 without the
- * writes) and (c) the allocation scan.
- *   d_tags[n_tags], d_points_xy[2*n_points], d_styles[n_paths]   device, read-only
+ * Runs kernels (a) tag-stream scan and the count-only instance of the expansion kernel:
+ * (b) per-segment count (Alg. 1/2 without the writes) and (c) the allocation scan.  Use this pair of calls when the
+ * output buffer can only be allocated once the record count is known; stroke_expand_into below needs one pass.
+ *   d_tags[n_tags], d_points_xy[2*n_points], d_styles[n_paths]   device, read-only.  ALIGNMENT: d_tags and d_styles
+ *                 16 bytes, d_points_xy and d_path_offsets 8 bytes (the kernels use vector loads); a pointer that
+ *                 is not aligned so is rejected with SX_E_INVALID_ARG (a contiguous but offset tensor view can be)
  *   h_affine[6]   HOST, row-major a b c d e f:  x' = a x + c y + e,  y' = b x + d y + f (L462);
  *                 must be finite and non-singular
  *   tolerance     > 0, device px (L37).  Internally split 0.1 / 0.8 between the cubic->Euler-spiral
@@ -127,13 +131,27 @@ sx_status sx_count(sx_ctx* ctx, const uint8_t* d_tags, uint64_t n_tags, const fl
                    uint64_t* d_path_offsets, uint64_t* h_total, void* cuda_stream);
 
 /* ------------------------------------------------------------------ phase 2: write
- * Kernel (d): writes the records of the preceding sx_count into d_out_records (sx_line[] or sx_arc[]
- * by mode, 16-byte aligned) of capacity cap_records.  SX_E_CAPACITY if the capacity is known to be
- * too small (the total is known on the host only when sx_count was given h_total; otherwise the
- * kernel itself refuses to write past the capacity and the error is reported by sx_last_error after
- * a stream sync).  Part of the work runs on a stream owned by the context, forked from and joined to `cuda_stream`
- * with events: for the caller everything is ordered on `cuda_stream` as usual (the pattern is CUDA-graph capturable). */
+ * Writes the records of the preceding sx_count into d_out_records (sx_line[] or sx_arc[] by mode, 16-byte
+ * aligned) of capacity cap_records: the expansion kernel again, on the same inputs, with the stores on (nothing
+ * is cached between the phases: the count pass is the same code and takes the same decisions).  SX_E_CAPACITY
+ * if the capacity is known to be too small (the total is known on the host only when sx_count was given
+ * h_total; otherwise the kernel itself refuses to write past the capacity and the error is reported by
+ * sx_last_error after a stream sync). */
 sx_status sx_write(sx_ctx* ctx, void* d_out_records, uint64_t cap_records, void* cuda_stream);
+
+/* ------------------------------------------------------------------ one pass into a caller-provided buffer
+ * The whole path in ONE pass: kernel (a), then the expansion kernel with count (b), allocation scan (c) and write
+ * (d) fused -- Alg. 1 / Alg. 2 run once per segment, nothing between the input streams and the records goes
+ * through device memory.  Inputs as for sx_count.  d_out_records (16-byte aligned) has room for cap_records
+ * records.  The count is always computed in full: a tile of segments whose records would pass the capacity is not
+ * written, the device-side capacity flag is raised (sx_last_error) and the total is still exact, so the caller can
+ * retry with a buffer of that size.  h_total (HOST, optional): when non-NULL the call synchronises the stream,
+ * writes the record count and returns SX_E_BAD_STREAM / SX_E_CAPACITY (count > cap_records) accordingly; when NULL
+ * the call stays asynchronous (the count is d_path_offsets[n_paths]). */
+sx_status stroke_expand_into(sx_ctx* ctx, const uint8_t* d_tags, uint64_t n_tags, const float* d_points_xy, uint64_t n_points,
+                             const sx_style* d_styles, uint64_t n_paths, const float* h_affine, float tolerance, int32_t mode,
+                             void* d_out_records, uint64_t cap_records, uint64_t* d_path_offsets, uint64_t* h_total,
+                             void* cuda_stream);
 
 /* ------------------------------------------------------------------ one-shot, device buffers
  * sx_count + allocate + sx_write.  `alloc` is called once (host side, after the count is known) and
@@ -148,7 +166,8 @@ sx_status stroke_expand(sx_ctx* ctx, const uint8_t* d_tags, uint64_t n_tags, con
 
 /* ------------------------------------------------------------------ one-shot, HOST buffers (end to end)
  * Same computation with every buffer on the host (pinned memory gives asynchronous copies): copies
- * the streams to the device, runs the four kernels, copies records and path offsets back.
+ * the streams to the device, runs the one-pass path (stroke_expand_into on a staging buffer owned by the
+ * context; a second pass only when that buffer had to grow), copies records and path offsets back.
  * h_out_records has room for cap_records records; *h_n_records receives the count even when
  * SX_E_CAPACITY is returned (so the caller can retry).  Returns after the results are in host memory. */
 sx_status stroke_expand_host(sx_ctx* ctx, const uint8_t* h_tags, uint64_t n_tags, const float* h_points_xy, uint64_t n_points,
@@ -159,7 +178,8 @@ sx_status stroke_expand_host(sx_ctx* ctx, const uint8_t* h_tags, uint64_t n_tags
 /* ------------------------------------------------------------------ introspection
  * Device pointers into the context's scratch of the last sx_count (valid until the next call on the
  * context): the tag-scan results and the per-segment record counts / offsets.  Any out pointer may
- * be NULL.  Used by the parity tests and the bench report. */
+ * be NULL.  Used by the parity tests and the bench report.  stroke_expand_into keeps the per-segment counts /
+ * offsets only under SX_OPT_KEEP_SEGMENT_INFO (12 bytes per segment of extra stores); SX_E_STATE otherwise. */
 sx_status sx_segment_info(sx_ctx* ctx, const uint32_t** d_pt_off, const uint32_t** d_path_idx, const uint32_t** d_sp_first,
                           const uint32_t** d_seg_count, const uint64_t** d_seg_offset);
 
@@ -167,12 +187,32 @@ sx_status sx_segment_info(sx_ctx* ctx, const uint32_t** d_pt_off, const uint32_t
  * SX_OK, SX_E_BAD_STREAM or SX_E_CAPACITY and clears the state. */
 sx_status sx_last_error(sx_ctx* ctx, void* cuda_stream);
 
-/* Memory knob for the piece cache: sx_count stores every accepted Euler-spiral piece
- * (80 bytes) so that sx_write need not repeat the cubic -> spiral fit.  The cache grows on demand; this call
- * caps it at max_pieces descriptors (0 = no cap, the default).  A call whose pieces do not fit is still
- * computed correctly, by the slower thread-per-segment writer.  Host-synchronous; invalidates a pending
- * sx_count. */
-sx_status sx_set_piece_cache_limit(sx_ctx* ctx, uint64_t max_pieces);
+/* Options of a context. */
+enum {
+    SX_OPT_KEEP_SEGMENT_INFO = 1, /* value != 0: stroke_expand_into also stores the per-segment counts / offsets        */
+    SX_OPT_TIME_KERNELS = 3,      /* value != 0: the library records CUDA events around its kernels (sx_kernel_times)          */
+    SX_OPT_TILES_PER_RANGE = 2    /* test knob for the expansion kernel, which works on ranges of 128 segments as 1, 2 or
+                                     4 tiles (adapted on the device to what fits its shared-memory tables): 0 adaptive
+                                     (default), 1 / 2 / 4 fixed, 8 = every tile takes the thread-per-segment reference
+                                     walk.  The records do not depend on it (tests/test_gpu_parity.py).               */
+};
+sx_status sx_set_option(sx_ctx* ctx, int32_t option, uint64_t value);
+
+/* Statistics of the last expansion kernel on the context (synchronises `cuda_stream`): h_out4[0] tiles that ran
+ * from shared memory, [1] tiles that took the thread-per-segment walk, [2] tiles per range now in use, [3] segments
+ * per range. */
+sx_status sx_call_stats(sx_ctx* ctx, uint64_t* h_out4, void* cuda_stream);
+
+/* Device durations of the two kernels of the last one-pass / count / write call made under SX_OPT_TIME_KERNELS, from
+ * CUDA events recorded on the call's own stream: h_ms2[0] tag scan (a), h_ms2[1] expansion kernel (b + c + d).
+ * Waits for the call to finish.  SX_E_STATE when nothing was timed. */
+sx_status sx_kernel_times(sx_ctx* ctx, float* h_ms2);
+
+/* Issue-rate microbenchmarks on `device` (host-synchronous, ~20 ms): h_out3[0] FP32 FMA lane-operations per second
+ * (independent FFMA chains on all SMs), [1] issued lane-operations per second of an FFMA + integer-ALU mix, [2]
+ * special-function (MUFU) lane-operations per second.  bench.py uses them as the measured R_fp32 / R_mufu of the
+ * roofline. */
+sx_status sx_measure_issue_peaks(int32_t device, double* h_out3);
 
 /* Number of kernel launches the library has issued on this context so far. */
 uint64_t sx_launch_count(const sx_ctx* ctx);

@@ -21,8 +21,11 @@ RECORD_BYTES = {SX_MODE_LINE: 16, SX_MODE_ARC: 32}
 ARC_DTYPE = np.dtype([("x0", "<f4"), ("y0", "<f4"), ("x1", "<f4"), ("y1", "<f4"), ("angle", "<f4"), ("seg", "<u4"),
                       ("kind", "<u4"), ("pad", "<u4")])
 
-EXPORTS = ["sx_create", "sx_destroy", "sx_count", "sx_write", "stroke_expand", "stroke_expand_host", "sx_segment_info",
-           "sx_last_error", "sx_set_piece_cache_limit", "sx_launch_count", "sx_strerror"]
+SX_OPT_KEEP_SEGMENT_INFO, SX_OPT_TILES_PER_RANGE, SX_OPT_TIME_KERNELS = 1, 2, 3
+
+EXPORTS = ["sx_create", "sx_destroy", "sx_count", "sx_write", "stroke_expand", "stroke_expand_into", "stroke_expand_host",
+           "sx_segment_info", "sx_last_error", "sx_set_option", "sx_call_stats", "sx_kernel_times", "sx_measure_issue_peaks", "sx_launch_count",
+           "sx_strerror"]
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
 _lib = None
@@ -49,10 +52,14 @@ def lib():
         L.sx_count.argtypes = [vp] + stream_args + [vp, C.POINTER(u64), vp]
         L.sx_write.argtypes = [vp, vp, u64, vp]
         L.stroke_expand.argtypes = [vp] + stream_args + [ALLOC_FN, vp, C.POINTER(vp), C.POINTER(u64), vp, vp]
+        L.stroke_expand_into.argtypes = [vp] + stream_args + [vp, u64, vp, C.POINTER(u64), vp]
         L.stroke_expand_host.argtypes = [vp] + stream_args + [vp, u64, C.POINTER(u64), vp, vp]
         L.sx_segment_info.argtypes = [vp] + [C.POINTER(vp)] * 5
         L.sx_last_error.argtypes = [vp, vp]
-        L.sx_set_piece_cache_limit.argtypes = [vp, u64]
+        L.sx_set_option.argtypes = [vp, i32, u64]
+        L.sx_call_stats.argtypes = [vp, C.POINTER(u64), vp]
+        L.sx_kernel_times.argtypes = [vp, C.POINTER(C.c_float)]
+        L.sx_measure_issue_peaks.argtypes = [i32, C.POINTER(C.c_double)]
         L.sx_launch_count.argtypes = [vp]
         L.sx_launch_count.restype = u64
         L.sx_strerror.argtypes = [i32]
@@ -85,7 +92,8 @@ def _affine(affine):
 
 
 def _dev_streams(tags, points, styles):
-    """tags u8[N], points f32[Npts,2], styles u8[P,16] (or any 16-byte rows) as contiguous CUDA tensors."""
+    """tags u8[N], points f32[Npts,2], styles u8[P,16] (or any 16-byte rows) as contiguous CUDA tensors.  The
+    library wants tags / styles 16-byte and points 8-byte aligned (it answers SX_E_INVALID_ARG otherwise)."""
     assert tags.is_cuda and points.is_cuda and styles.is_cuda, "device tensors expected (use stroke_expand_host for host data)"
     assert tags.dtype == torch.uint8 and points.dtype == torch.float32 and styles.dtype == torch.uint8
     assert tags.is_contiguous() and points.is_contiguous() and styles.is_contiguous()
@@ -109,7 +117,7 @@ def sx_count(ctx, tags, points, styles, affine, tolerance, mode, path_offsets, w
     when want_total is False: the call then stays asynchronous)."""
     args = _dev_streams(tags, points, styles)
     a, ap = _affine(affine)
-    assert path_offsets.is_cuda and path_offsets.element_size() == 8 and path_offsets.numel() >= args[5] + 1
+    assert path_offsets.is_cuda and path_offsets.is_contiguous() and path_offsets.element_size() == 8 and path_offsets.numel() >= args[5] + 1
     total = C.c_uint64(0)
     st = lib().sx_count(ctx, *args, ap, float(tolerance), int(mode), C.c_void_p(path_offsets.data_ptr()),
                         C.byref(total) if want_total else None, _stream_ptr(stream))
@@ -117,10 +125,34 @@ def sx_count(ctx, tags, points, styles, affine, tolerance, mode, path_offsets, w
     return int(total.value) if want_total else None
 
 
-def sx_write(ctx, out_records, cap_records, stream=None):
-    """Phase 2.  out_records: CUDA tensor with room for cap_records records (16 B line / 32 B arc)."""
+def sx_write(ctx, out_records, cap_records, mode=None, stream=None):
+    """Phase 2.  out_records: CUDA tensor with room for cap_records records (16 B line / 32 B arc; pass the mode of
+    the count to have the tensor's size checked against cap_records)."""
     assert out_records.is_cuda and out_records.is_contiguous()
+    if mode is not None:
+        assert out_records.numel() * out_records.element_size() >= int(cap_records) * RECORD_BYTES[int(mode)]
     _check(lib().sx_write(ctx, C.c_void_p(out_records.data_ptr()), int(cap_records), _stream_ptr(stream)), "sx_write")
+
+
+def stroke_expand_into(ctx, tags, points, styles, affine, tolerance, mode, out_records, path_offsets, want_total=True, stream=None):
+    """The whole path in one pass into a caller-provided CUDA tensor (float32 [cap,4] line / [cap,8] arc).  Returns
+    the record count (None when want_total is False: the call stays asynchronous).  Raises SX_E_CAPACITY with the
+    needed count in .needed when the records do not fit."""
+    args = _dev_streams(tags, points, styles)
+    a, ap = _affine(affine)
+    width = 4 if mode == SX_MODE_LINE else 8
+    assert out_records.is_cuda and out_records.is_contiguous() and out_records.dtype == torch.float32
+    cap = out_records.numel() // width
+    assert path_offsets.is_cuda and path_offsets.is_contiguous() and path_offsets.element_size() == 8 and path_offsets.numel() >= args[5] + 1
+    total = C.c_uint64(0)
+    st = lib().stroke_expand_into(ctx, *args, ap, float(tolerance), int(mode), C.c_void_p(out_records.data_ptr()), cap,
+                                  C.c_void_p(path_offsets.data_ptr()), C.byref(total) if want_total else None, _stream_ptr(stream))
+    if st == SX_E_CAPACITY:
+        e = StrokeExpandError(st, "stroke_expand_into")
+        e.needed = int(total.value)
+        raise e
+    _check(st, "stroke_expand_into")
+    return int(total.value) if want_total else None
 
 
 def stroke_expand(ctx, tags, points, styles, affine, tolerance, mode, stream=None):
@@ -205,8 +237,29 @@ def sx_last_error(ctx, stream=None):
     return int(lib().sx_last_error(ctx, _stream_ptr(stream)))
 
 
-def sx_set_piece_cache_limit(ctx, max_pieces):
-    _check(lib().sx_set_piece_cache_limit(ctx, int(max_pieces)), "sx_set_piece_cache_limit")
+def sx_set_option(ctx, option, value):
+    _check(lib().sx_set_option(ctx, int(option), int(value)), "sx_set_option")
+
+
+def sx_call_stats(ctx, stream=None):
+    """dict(fast_tiles, slow_tiles, tiles_per_range, range_segments) of the last expansion kernel on the context."""
+    out = (C.c_uint64 * 4)()
+    _check(lib().sx_call_stats(ctx, out, _stream_ptr(stream)), "sx_call_stats")
+    return dict(fast_tiles=int(out[0]), slow_tiles=int(out[1]), tiles_per_range=int(out[2]), range_segments=int(out[3]))
+
+
+def sx_kernel_times(ctx):
+    """(tag scan ms, expansion kernel ms) of the last call made under SX_OPT_TIME_KERNELS (waits for it)."""
+    out = (C.c_float * 2)()
+    _check(lib().sx_kernel_times(ctx, out), "sx_kernel_times")
+    return float(out[0]), float(out[1])
+
+
+def sx_measure_issue_peaks(device=0):
+    """dict(fp32_ffma, fp32_mix, mufu): measured lane-operations per second (issue-rate microbenchmarks)."""
+    out = (C.c_double * 3)()
+    _check(lib().sx_measure_issue_peaks(int(device), out), "sx_measure_issue_peaks")
+    return dict(fp32_ffma=float(out[0]), fp32_mix=float(out[1]), mufu=float(out[2]))
 
 
 def sx_launch_count(ctx):

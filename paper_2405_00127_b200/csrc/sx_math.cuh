@@ -14,7 +14,6 @@
 #pragma once
 #include <stdint.h>
 #include <math.h>
-#include <string.h>
 
 #ifndef SX_DEV
 #define SX_DEV __device__ __forceinline__
@@ -54,40 +53,11 @@ SX_DEV float len2(V2 a) { return a.x * a.x + a.y * a.y; }
 SX_DEV float div_fast(float a, float b) { return __fdividef(a, b); }
 SX_DEV float sqrt_fast(float a) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
 SX_DEV float cbrt_fast(float a) { return a > 0.0f ? __powf(a, 0.33333333333333333f) : 0.0f; }
-// atan2 for the end-tangent angles of a piece: one approximate division, odd minimax polynomial on [0,1]
-// (max error ~1e-7 rad), quadrant fix-up by selects
-SX_DEV float atan2_fast(float y, float x) {
-    const float ax = fabsf(x), ay = fabsf(y);
-    const float mx = fmaxf(ax, ay), mn = fminf(ax, ay);
-    const float a = mx > 0.0f ? __fdividef(mn, mx) : 0.0f;
-    const float s = a * a;
-    float r = fmaf(s, 0.00282363896258175373077393f, -0.0159569028764963150024414f);
-    r = fmaf(r, s, 0.0425049886107444763183594f);
-    r = fmaf(r, s, -0.0748900920152664184570312f);
-    r = fmaf(r, s, 0.106347933411598205566406f);
-    r = fmaf(r, s, -0.142027363181114196777344f);
-    r = fmaf(r, s, 0.199926957488059997558594f);
-    r = fmaf(r, s, -0.333331018686294555664062f);
-    r = fmaf(r * s, a, a);
-    if (ay > ax) r = 1.57079637050628662109375f - r;
-    if (x < 0.0f) r = 3.14159274101257324218750f - r;
-    return y < 0.0f ? -r : r;
-}
-SX_DEV V2 unit(V2 a) { float l = sqrtf(len2(a)); return v2(a.x / l, a.y / l); }
+// (not inlined: IEEE square root and two divisions, a dozen call sites)
+__device__ __noinline__ V2 unit(V2 a) { float l = sqrtf(len2(a)); return v2(a.x / l, a.y / l); }
 
-#ifdef __CUDA_ARCH__
 SX_DEV float u2f(uint32_t u) { return __uint_as_float(u); }
-#else
-SX_DEV float u2f(uint32_t u) { float f; memcpy(&f, &u, 4); return f; }
-#endif
-
-SX_DEV int ctz32(uint32_t x) {
-#ifdef __CUDA_ARCH__
-    return __ffs((int)x) - 1;
-#else
-    return __builtin_ctz(x);
-#endif
-}
+SX_DEV int ctz32(uint32_t x) { return __ffs((int)x) - 1; }
 
 // ---------------------------------------------------------------- per-call parameters (kernel argument, by value)
 struct Params {
@@ -129,11 +99,7 @@ SX_DEV V2 pick_tangent(V2 a, V2 b, V2 c, bool* degenerate) {
     return *degenerate ? v2(1.0f, 0.0f) : u;
 }
 
-#ifdef __CUDA_ARCH__
 SX_DEV float2 ldg2(const float* p) { return __ldg(reinterpret_cast<const float2*>(p)); }
-#else
-SX_DEV V2 ldg2(const float* p) { return v2(p[0], p[1]); }
-#endif
 
 // pt = index of the segment's first point (pt_off[i] from the tag scan)
 SX_DEV Seg load_segment_at(const Params& P, uint32_t pt, uint32_t tag) {
@@ -228,30 +194,70 @@ SX_DEV void eval_cubic(const Seg& s, float t, float dt, V2* pos, float* qmag, V2
 
 // ---------------------------------------------------------------- section 7.1: cubic -> Euler spiral error estimate
 // L215 unit-chord normalisation; L217 d-bar; L221 e1; L225 area; L227 e2; L229 e3; guards R-4.
-SX_DEV float fit_error(V2 u0, V2 u1, float q0mag, float q1mag, V2 ch, float dt, float* th0_out, float* th1_out, float* chord_out) {
-    float chord2 = len2(ch);
-    float chord = sqrtf(chord2);
-    *chord_out = chord;
-    if (chord2 < kEpsQ2) { *th0_out = 0.0f; *th1_out = 0.0f; return INFINITY; }
-    V2 uc = v2(ch.x / chord, ch.y / chord);
-    float s0 = cross(u0, uc), c0 = dot(u0, uc);
-    float s1 = cross(uc, u1), c1 = dot(uc, u1);
-    float th0 = atan2f(s0, c0), th1 = atan2f(s1, c1);  // accurate: the angles fix k0, k1 and hence every subdivision parameter
-    *th0_out = th0;
-    *th1_out = th1;
+//
+// Angles (reading R-17): th = the fp32 value nearest to the angle of (x, y): atan2 in double, rounded once.  The
+// oracle computes the same number with its own libm; the two agree unless the double result falls within an
+// ulp(double) of a rounding boundary of fp32 (probability ~1e-8 per call).  th0, th1 fix k0, k1, L and hence every
+// subdivision parameter and every evolute radius of the piece.
+__device__ __noinline__ float atan2_r(float y, float x) { return (float)atan2((double)y, (double)x); }
+
+// atan2 for the accept/split DECISION of Alg. 2 only (the error estimate of section 7.1 is compared with a tolerance):
+// IEEE division, odd minimax polynomial on [0, 1] (max error ~1e-7 rad).  The angles a piece is built from come
+// from atan2_r.
+SX_DEV float atan2_dec(float y, float x) {
+    const float ax = fabsf(x), ay = fabsf(y);
+    const float mx = fmaxf(ax, ay), mn = fminf(ax, ay);
+    const float a = mx > 0.0f ? mn / mx : 0.0f;
+    const float s = a * a;
+    float r = fmaf(s, 0.00282363896258175373077393f, -0.0159569028764963150024414f);
+    r = fmaf(r, s, 0.0425049886107444763183594f);
+    r = fmaf(r, s, -0.0748900920152664184570312f);
+    r = fmaf(r, s, 0.106347933411598205566406f);
+    r = fmaf(r, s, -0.142027363181114196777344f);
+    r = fmaf(r, s, 0.199926957488059997558594f);
+    r = fmaf(r, s, -0.333331018686294555664062f);
+    r = fmaf(r * s, a, a);
+    if (ay > ax) r = 1.57079637050628662109375f - r;
+    if (x < 0.0f) r = 3.14159274101257324218750f - r;
+    return y < 0.0f ? -r : r;
+}
+
+// section 7.1 with the decision-grade angles: the estimated error of the node (u0, q0mag) -> (u1, q1mag) over chord ch
+SX_DEV float node_error(V2 u0, V2 u1, float q0mag, float q1mag, V2 ch, float dt) {
+    const float chord2 = len2(ch);
+    const float chord = sqrtf(chord2);
+    if (chord2 < kEpsQ2) return INFINITY;
+    const V2 uc = v2(ch.x / chord, ch.y / chord);
+    const float s0 = cross(u0, uc), c0 = dot(u0, uc);
+    const float s1 = cross(uc, u1), c1 = dot(uc, u1);
     if (c0 < -0.5f || c1 < -0.5f) return 2.0f * chord;
-    float d0 = div_fast(q0mag * dt, chord), d1 = div_fast(q1mag * dt, chord);
-    float db0 = div_fast(2.0f, 3.0f * (1.0f + c0)), db1 = div_fast(2.0f, 3.0f * (1.0f + c1));
-    float s01 = s0 * c1 + c0 * s1;
-    float area = 0.15f * (2.0f * d0 * s0 + 2.0f * d1 * s1 - d0 * d1 * s01);
-    float areb = 0.15f * (2.0f * db0 * s0 + 2.0f * db1 * s1 - db0 * db1 * s01);
-    float ksum = fabsf(th0 + th1), kdif = fabsf(th0 - th1);
-    float k2 = ksum * ksum;
-    float e1 = 4.6255e-6f * k2 * k2 * ksum + 7.5e-3f * k2 * kdif;
-    float e2 = 1.55f * fabsf(area - areb);
-    float dd0 = db0 - d0, dd1 = db1 - d1;
-    float e3 = (0.005f * ksum + 0.07f * kdif) * sqrt_fast(dd0 * dd0 + dd1 * dd1);
+    const float th0 = atan2_dec(s0, c0), th1 = atan2_dec(s1, c1);
+    const float d0 = div_fast(q0mag * dt, chord), d1 = div_fast(q1mag * dt, chord);
+    const float db0 = div_fast(2.0f, 3.0f * (1.0f + c0)), db1 = div_fast(2.0f, 3.0f * (1.0f + c1));
+    const float s01 = s0 * c1 + c0 * s1;
+    const float area = 0.15f * (2.0f * d0 * s0 + 2.0f * d1 * s1 - d0 * d1 * s01);
+    const float areb = 0.15f * (2.0f * db0 * s0 + 2.0f * db1 * s1 - db0 * db1 * s01);
+    const float ksum = fabsf(th0 + th1), kdif = fabsf(th0 - th1);
+    const float k2 = ksum * ksum;
+    const float e1 = 4.6255e-6f * k2 * k2 * ksum + 7.5e-3f * k2 * kdif;
+    const float e2 = 1.55f * fabsf(area - areb);
+    const float dd0 = db0 - d0, dd1 = db1 - d1;
+    const float e3 = (0.005f * ksum + 0.07f * kdif) * sqrt_fast(dd0 * dd0 + dd1 * dd1);
     return chord * (e1 + e2 + e3);
+}
+
+
+// the end-tangent angles of an ACCEPTED piece (L211-213: th0 from the start tangent to the chord, th1 from the chord to
+// the end tangent) and its chord length; a zero chord (accepted at the deepest level only) has th0 = th1 = 0
+SX_DEV void piece_angles(V2 u0, V2 u1, V2 ch, float* th0, float* th1, float* chord_out) {
+    const float chord2 = len2(ch);
+    const float chord = sqrtf(chord2);
+    *chord_out = chord;
+    *th0 = 0.0f; *th1 = 0.0f;
+    if (chord2 < kEpsQ2) return;
+    const V2 uc = v2(ch.x / chord, ch.y / chord);
+    *th0 = atan2_r(cross(u0, uc), dot(u0, uc));
+    *th1 = atan2_r(cross(uc, u1), dot(uc, u1));
 }
 
 // ---------------------------------------------------------------- Appendix A: geometric Hermite interpolation

@@ -42,6 +42,11 @@ SX_DEV float f_approx_inv(float u) {
     return u < 0.0f ? -r : r;
 }
 
+// v -> sgn(v) |v|^1.5 and its inverse: the integral of sqrt|v| and the s ~ i^(2/3) rule of section 2.2 (L97)
+SX_DEV float pow15(float v) { const float a = fabsf(v), w = a * sqrtf(a); return v < 0.0f ? -w : w; }
+SX_DEV float pow15_inv(float w) { float c = cbrtf(fabsf(w)); c = c * c; return w < 0.0f ? -c : c; }
+enum : int { kRuleUniform = 0, kRuleFApprox = 1, kRuleInflection = 2, kRuleCusp = 3 };
+
 SX_DEV float clampf(float x, float lo, float hi) { return x < lo ? lo : (x > hi ? hi : x); }
 SX_DEV int count_clamp(float n) { if (!(n >= 1.0f)) return 1; return (int)(n > kNMax ? kNMax : n); }
 
@@ -220,13 +225,13 @@ SX_DEV V2 es_offset(const Piece& p, const Spiral& sp, float t, float eta) { retu
 SX_DEV V2 es_evolute(const Piece& p, const Spiral& sp, float t) { return normal_point(p, sp, t, es_radius(p, t)); }  // section 6
 
 // ---------------------------------------------------------------- subdivision plans
-struct OffPlan { int n; bool uniform; float ta, tb, ua, ub; };
+struct OffPlan { int n; int rule; float ta, tb, ua, ub; };   // rule: how the interior parameters are spaced (kRule*)
 struct EvoPlan { int n; bool uniform; float ta, tb, wa, wb, skp; };
 
 // offset range [ta,tb] of side eta (sections 4, 5): number of records and what the parameters need
 SX_DEV OffPlan offset_plan(const Piece& p, float eta, float ta, float tb, int mode, float tol_fl) {
     OffPlan o;
-    o.ta = ta; o.tb = tb; o.ua = 0.0f; o.ub = 0.0f; o.uniform = true;
+    o.ta = ta; o.tb = tb; o.ua = 0.0f; o.ub = 0.0f; o.rule = kRuleUniform;
     float n_f, ah = fabsf(eta);
     if (mode == kModeArc) {
         // L177 with s = L, kappa' = k1/L^2, scaled by the range fraction (R-12)
@@ -236,15 +241,32 @@ SX_DEV OffPlan offset_plan(const Piece& p, float eta, float ta, float tb, int mo
         float ka = es_kappa(p, ta), kb = es_kappa(p, tb);
         float xa = 2.0f * eta * ka - 1.0f, xb = 2.0f * eta * kb - 1.0f;  // L125: inflection -> -1, cusp -> +1
         float xm = 0.5f * (xa + xb);
+        float kp = div_fast(fabsf(p.k1), p.L * p.L);
         if (fabsf(xb - xa) < 0.015625f * fmaxf(1.0f, fabsf(xm))) {
-            float km = 0.5f * (ka + kb);  // constant density sqrt|k(1-k eta)| (R-7; limit is L73)
-            n_f = ceilf((tb - ta) * p.L * sqrt_fast(div_fast(fabsf(km * (1.0f - km * eta)), 8.0f * tol_fl)));
+            // x varies too little for a difference of two f_approx values in fp32 (R-7): the density sqrt|k (1 - k eta)|
+            // is integrated locally.  km, gm: curvature and cusp factor at the middle of the range; m_infl, m_cusp: how far
+            // km is from the inflection (k = 0) and from the cusp (k = 1/eta)
+            float km = 0.5f * (ka + kb), dk = fabsf(kb - ka);
+            float gm = 1.0f - km * eta;
+            float m_infl = fabsf(km), m_cusp = fabsf(gm) / ah;
+            if (dk <= 0.125f * fminf(m_infl, m_cusp)) {
+                n_f = ceilf((tb - ta) * p.L * sqrt_fast(div_fast(fabsf(km * gm), 8.0f * tol_fl)));  // constant density (limit: L73)
+            } else if (m_infl <= m_cusp) {
+                // an inflection in or next to the range: int sqrt|k| ds = 2/3 |k|^1.5 / k' (section 2.2)
+                o.ua = pow15(ka); o.ub = pow15(kb);
+                n_f = ceilf(div_fast((2.0f / 3.0f) * fabsf(o.ub - o.ua) * sqrt_fast(fabsf(gm)), kp * sqrt_fast(8.0f * tol_fl)));
+                o.rule = kRuleInflection;
+            } else {
+                // the range ends next to the cusp: the same with g = 1 - k eta
+                o.ua = pow15(1.0f - ka * eta); o.ub = pow15(1.0f - kb * eta);
+                n_f = ceilf(div_fast((2.0f / 3.0f) * fabsf(o.ub - o.ua) * sqrt_fast(fabsf(km)), ah * kp * sqrt_fast(8.0f * tol_fl)));
+                o.rule = kRuleCusp;
+            }
         } else {
             o.ua = f_approx(xa);
             o.ub = f_approx(xb);
-            float kp = div_fast(fabsf(p.k1), p.L * p.L);
             n_f = ceilf(div_fast(fabsf(o.ub - o.ua), 4.0f * kp * ah * sqrt_fast(ah) * sqrt_fast(8.0f * tol_fl)));  // L83
-            o.uniform = false;
+            o.rule = kRuleFApprox;
         }
     }
     o.n = count_clamp(n_f);
@@ -253,11 +275,12 @@ SX_DEV OffPlan offset_plan(const Piece& p, float eta, float ta, float tb, int mo
 // parameter of interior subdivision point i (0 < i < n)
 SX_DEV float offset_t(const Piece& p, const OffPlan& o, float eta, int i) {
     float fr = (float)i / (float)o.n, t;
-    if (o.uniform) t = o.ta + fr * (o.tb - o.ta);
+    if (o.rule == kRuleUniform) t = o.ta + fr * (o.tb - o.ta);
     else {
-        float u = o.ua + fr * (o.ub - o.ua);
-        float x = f_approx_inv(u);
-        float kap = (x + 1.0f) / (2.0f * eta);
+        float u = o.ua + fr * (o.ub - o.ua), kap;
+        if (o.rule == kRuleFApprox) kap = (f_approx_inv(u) + 1.0f) / (2.0f * eta);
+        else if (o.rule == kRuleInflection) kap = pow15_inv(u);
+        else kap = (1.0f - pow15_inv(u)) / eta;
         t = 0.5f + (kap * p.L - p.k0) / (p.k1);
     }
     return clampf(t, o.ta, o.tb);
@@ -306,14 +329,17 @@ struct SidePlan {
     uint32_t seg;    // source segment (filled by the write kernel)
 };
 
-SX_DEV SidePlan side_plan(const Piece& p, float eta, int mode, float tol_fl) {
+__device__ __noinline__ SidePlan side_plan(const Piece& p, float eta, int mode, float tol_fl) {
     SidePlan s;
     s.eta = eta; s.seg = 0u;
     float g0 = 1.0f - es_kappa(p, 0.0f) * eta, g1 = 1.0f - es_kappa(p, 1.0f) * eta;  // cusp0, cusp1 (L382-384)
-    float tc = (g0 * g1 >= 0.0f) ? 1.0f : g0 / (g0 - g1);                            // L386
-    // g0 >= 0: regular on [0,tc], then super-critical on [tc,1] if there is a cusp; g0 < 0: super-critical on
-    // [0,tc], then regular on [tc,1] if there is a cusp (L388-411)
-    const bool first_sup = g0 < 0.0f;
+    // L386.  The cusp is inside the piece iff g0 and g1 have strictly opposite signs (decided from the signs, not from the
+    // product: g0 == 0 with g1 < 0 is a piece that is super-critical over its whole length)
+    const bool has_cusp = (g0 > 0.0f && g1 < 0.0f) || (g0 < 0.0f && g1 > 0.0f);
+    float tc = has_cusp ? g0 / (g0 - g1) : 1.0f;
+    // regular on [0,tc], then super-critical on [tc,1] if there is a cusp; or super-critical on [0,tc], then regular on
+    // [tc,1] if there is a cusp (L388-411)
+    const bool first_sup = g0 < 0.0f || (g0 == 0.0f && g1 < 0.0f);
     s.nr = tc < 1.0f ? 2 : 1;
     s.sup[0] = first_sup;
     s.sup[1] = !first_sup;

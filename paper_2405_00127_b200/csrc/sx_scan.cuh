@@ -1,18 +1,15 @@
-// sx_scan.cuh -- the two single-pass prefix scans of the pipeline (decoupled look-back).
+// sx_scan.cuh -- (a) k_tag_scan, the single-pass prefix scan over the tag stream (decoupled look-back).
 //
-// (a) k_tag_scan: PAPER.md L464-466 + Table 1 (L468-481): every tag carries stream-offset increments and
-//     the offsets are prefix sums over the "tag monoid".  Ours is (points, paths, first) with
-//     points += count + subpath_end (L470), paths += path_end, first = max(index+1 of subpath ends):
-//     the exclusive prefix gives segment i its first point, its path and the first segment of its
-//     subpath (which replaces the paper's stroke-cap-marker segment, L483-489).  A fourth component counts the
-//     curve segments (quadratics and cubics) and yields their compact index list for the count kernel.
-// (c) k_alloc_scan: exclusive prefix sum of the per-segment record counts -> record offsets (replaces
-//     the paper's atomic bump allocation, L448), the per-path offsets and the total.
+// PAPER.md L464-466 + Table 1 (L468-481): every tag carries stream-offset increments and the offsets are prefix
+// sums over the "tag monoid".  Ours is (points, paths, first) with points += count + subpath_end (L470),
+// paths += path_end, first = max(index+1 of subpath ends): the exclusive prefix gives segment i its first point,
+// its path and the first segment of its subpath (which replaces the paper's stroke-cap-marker segment, L483-489).
 //
-// Both: one pass over the data, thread-sequential -> warp-shuffle -> cross-warp in shared memory ->
-// tile prefix by decoupled look-back (a tile publishes its aggregate, then looks back over its
-// predecessors' aggregates / inclusive prefixes, one warp inspecting 32 predecessors at a time).
-// Tile ids come from an atomic ticket, so a tile only ever waits for tiles that already started.
+// One pass over the data, thread-sequential -> warp-shuffle -> cross-warp in shared memory -> tile prefix by
+// decoupled look-back (a tile publishes its aggregate, then looks back over its predecessors' aggregates /
+// inclusive prefixes, one warp inspecting 32 predecessors at a time).  Tile ids come from an atomic ticket, so a
+// tile only ever waits for tiles that already started.  The allocation scan over the record counts (replacing the
+// atomic bump allocation of L448) uses the same protocol inside k_expand (sx_expand.cuh).
 #pragma once
 #include <stdint.h>
 #include <cuda_runtime.h>
@@ -22,23 +19,21 @@ namespace sx {
 constexpr int kScanThreads = 256;
 constexpr int kTagItems = 16;                         // tags per thread: one 16-byte load
 constexpr int kTagTile = kScanThreads * kTagItems;    // 4096
-constexpr int kCntItems = 8;                          // counts per thread: two 16-byte loads
-constexpr int kCntTile = kScanThreads * kCntItems;    // 2048
 
 enum : uint32_t { kErrBadStream = 1u, kErrCapacity = 2u };
 
-struct TagAgg { uint32_t pt, path, first, curve; };
-__device__ __forceinline__ TagAgg tag_identity() { TagAgg a; a.pt = 0; a.path = 0; a.first = 0; a.curve = 0; return a; }
+struct TagAgg { uint32_t pt, path, first; };
+__device__ __forceinline__ TagAgg tag_identity() { TagAgg a; a.pt = 0; a.path = 0; a.first = 0; return a; }
 __device__ __forceinline__ TagAgg tag_combine(TagAgg a, TagAgg b) {
-    TagAgg r; r.pt = a.pt + b.pt; r.path = a.path + b.path; r.first = a.first > b.first ? a.first : b.first; r.curve = a.curve + b.curve; return r;
+    TagAgg r; r.pt = a.pt + b.pt; r.path = a.path + b.path; r.first = a.first > b.first ? a.first : b.first; return r;
 }
 __device__ __forceinline__ TagAgg tag_shfl_up(TagAgg a, int d) {
     TagAgg r; r.pt = __shfl_up_sync(0xffffffffu, a.pt, d); r.path = __shfl_up_sync(0xffffffffu, a.path, d);
-    r.first = __shfl_up_sync(0xffffffffu, a.first, d); r.curve = __shfl_up_sync(0xffffffffu, a.curve, d); return r;
+    r.first = __shfl_up_sync(0xffffffffu, a.first, d); return r;
 }
 __device__ __forceinline__ TagAgg tag_shfl_xor(TagAgg a, int d) {
     TagAgg r; r.pt = __shfl_xor_sync(0xffffffffu, a.pt, d); r.path = __shfl_xor_sync(0xffffffffu, a.path, d);
-    r.first = __shfl_xor_sync(0xffffffffu, a.first, d); r.curve = __shfl_xor_sync(0xffffffffu, a.curve, d); return r;
+    r.first = __shfl_xor_sync(0xffffffffu, a.first, d); return r;
 }
 
 // look-back descriptor of one tag tile: status 0 = nothing yet, 1 = aggregate valid, 2 = inclusive valid
@@ -49,8 +44,7 @@ __device__ __forceinline__ uint64_t ld_volatile_u64(const uint64_t* p) { return 
 
 __global__ void __launch_bounds__(kScanThreads)
 k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint32_t n_paths, uint32_t* __restrict__ pt_off,
-           uint32_t* __restrict__ path_idx, uint32_t* __restrict__ sp_first, uint32_t* __restrict__ curve_idx, uint32_t* n_curves,
-           TagTileState* states, uint32_t* ticket, uint32_t* err) {
+           uint32_t* __restrict__ path_idx, uint32_t* __restrict__ sp_first, TagTileState* states, uint32_t* ticket, uint32_t* err) {
     __shared__ uint32_t s_tile;
     __shared__ TagAgg s_warp[kScanThreads / 32];
     __shared__ TagAgg s_prefix;
@@ -80,7 +74,6 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
         bad |= valid && (cnt == 0u || (tag & 8u));
         mine.pt += cnt + end;
         mine.path += (tag >> 4) & 1u;
-        mine.curve += (valid && cnt >= 2u) ? 1u : 0u;
         if (end) mine.first = base + k + 1u;
     }
     if (bad) atomicOr(err, kErrBadStream);
@@ -103,7 +96,7 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
     if (warp == 0) {
         TagTileState* me = states + tile;
         if (lane == 0 && tile > 0) {
-            me->agg = make_uint4(tile_agg.pt, tile_agg.path, tile_agg.first, tile_agg.curve);
+            me->agg = make_uint4(tile_agg.pt, tile_agg.path, tile_agg.first, 0u);
             __threadfence();
             *reinterpret_cast<volatile uint32_t*>(&me->status) = 1u;
         }
@@ -117,7 +110,7 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
             TagAgg v = tag_identity();
             if (j >= 0) {
                 const volatile uint4* src = st == 2u ? &states[j].inc : &states[j].agg;
-                v.pt = src->x; v.path = src->y; v.first = src->z; v.curve = src->w;
+                v.pt = src->x; v.path = src->y; v.first = src->z;
             }
             uint32_t m = __ballot_sync(0xffffffffu, st == 2u);
             int stop = __ffs((int)m) - 1;  // nearest predecessor with an inclusive prefix (lanes with j < 0 report 2)
@@ -131,7 +124,7 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
         if (lane == 0) {
             s_prefix = excl;
             TagAgg inc = tag_combine(excl, tile_agg);
-            me->inc = make_uint4(inc.pt, inc.path, inc.first, inc.curve);
+            me->inc = make_uint4(inc.pt, inc.path, inc.first, 0u);
             __threadfence();
             *reinterpret_cast<volatile uint32_t*>(&me->status) = 2u;
         }
@@ -147,7 +140,6 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
         uint32_t tag = (w[k >> 2] >> (8 * (k & 3))) & 0xffu;
         uint32_t cnt = tag & 3u, end = ((tag >> 2) | (tag >> 4)) & 1u;
         o_pt[k] = run.pt; o_path[k] = run.path; o_first[k] = run.first;
-        if (base + k < n && cnt >= 2u) curve_idx[run.curve++] = base + k;  // compact list of the curve segments, in order
         run.pt += cnt + end;
         run.path += (tag >> 4) & 1u;
         if (end) run.first = base + k + 1u;
@@ -169,89 +161,10 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
         uint32_t k = n - 1u - base;
         uint32_t last = (w[k >> 2] >> (8 * (k & 3))) & 0xffu;
         if (!(last & 16u) || run.pt != n_points || run.path != n_paths) atomicOr(err, kErrBadStream);
-        *n_curves = run.curve;
     }
 }
 
-// ---------------------------------------------------------------- (c) allocation scan
-// state word: status in bits 62-63 (0 nothing, 1 aggregate, 2 inclusive), value in bits 0-61
+// state word of the allocation look-back (k_expand): status in bits 62-63 (0 nothing, 1 aggregate, 2 inclusive), value in bits 0-61
 constexpr uint64_t kValMask = (1ull << 62) - 1ull;
-
-__global__ void __launch_bounds__(kScanThreads)
-k_alloc_scan(const uint32_t* __restrict__ count, uint32_t n, const uint8_t* __restrict__ tags, const uint32_t* __restrict__ path_idx,
-             uint32_t n_paths, uint64_t* __restrict__ seg_off, uint64_t* __restrict__ path_off, uint64_t* d_total, uint64_t* states,
-             uint32_t* ticket, const uint32_t* err) {
-    __shared__ uint32_t s_tile;
-    __shared__ uint64_t s_warp[kScanThreads / 32];
-    __shared__ uint64_t s_prefix;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
-    __syncthreads();
-    const uint32_t tile = s_tile;
-    const uint32_t base = tile * (uint32_t)kCntTile + (uint32_t)tid * kCntItems;
-    uint32_t c[kCntItems];
-    if (base + kCntItems <= n) {
-        uint4 a = __ldg(reinterpret_cast<const uint4*>(count + base)), b = __ldg(reinterpret_cast<const uint4*>(count + base + 4));
-        c[0] = a.x; c[1] = a.y; c[2] = a.z; c[3] = a.w; c[4] = b.x; c[5] = b.y; c[6] = b.z; c[7] = b.w;
-    } else {
-#pragma unroll
-        for (int k = 0; k < kCntItems; k++) c[k] = base + k < n ? count[base + k] : 0u;
-    }
-    uint64_t mine = 0;
-#pragma unroll
-    for (int k = 0; k < kCntItems; k++) mine += c[k];
-    uint64_t incl = mine;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        uint64_t o = __shfl_up_sync(0xffffffffu, incl, d);
-        if (lane >= d) incl += o;
-    }
-    if (lane == 31) s_warp[warp] = incl;
-    __syncthreads();
-    uint64_t tile_agg = 0, warp_excl = 0;
-#pragma unroll
-    for (int k = 0; k < kScanThreads / 32; k++) {
-        if (k == warp) warp_excl = tile_agg;
-        tile_agg += s_warp[k];
-    }
-    if (warp == 0) {
-        if (lane == 0 && tile > 0) *reinterpret_cast<volatile uint64_t*>(states + tile) = (1ull << 62) | tile_agg;
-        uint64_t excl = 0;
-        int idx = (int)tile - 1;
-        while (idx >= 0) {
-            int j = idx - lane;
-            uint64_t word = 2ull << 62;
-            if (j >= 0) { do { word = ld_volatile_u64(states + j); } while ((word >> 62) == 0ull); }
-            uint32_t m = __ballot_sync(0xffffffffu, (word >> 62) == 2ull);
-            int stop = __ffs((int)m) - 1;
-            uint64_t v = (lane > stop && m) ? 0ull : (word & kValMask);
-#pragma unroll
-            for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-            excl += v;
-            if (m) break;
-            idx -= 32;
-        }
-        if (lane == 0) {
-            s_prefix = excl;
-            *reinterpret_cast<volatile uint64_t*>(states + tile) = (2ull << 62) | (excl + tile_agg);
-        }
-    }
-    __syncthreads();
-    uint64_t up = __shfl_up_sync(0xffffffffu, incl, 1);
-    if (lane == 0) up = 0;
-    uint64_t run = s_prefix + warp_excl + up;
-    const bool ok = *err == 0u;
-#pragma unroll
-    for (int k = 0; k < kCntItems; k++) {
-        uint32_t i = base + k;
-        if (i < n) {
-            seg_off[i] = run;
-            // first segment of a path: the previous tag carries the path-end bit (Table 1)
-            if (ok && (i == 0u || (tags[i - 1] & 16u))) { uint32_t p = path_idx[i]; if (p < n_paths) path_off[p] = run; }
-            run += c[k];
-            if (i == n - 1u) { path_off[n_paths] = run; *d_total = run; }
-        }
-    }
-}
 
 }  // namespace sx

@@ -90,7 +90,7 @@ SX_DEV uint32_t piece_side(const Piece& p, const Spiral& z, float eta, bool mirr
 }
 
 // ---------------------------------------------------------------- round joins / caps (L65-69 exact arc metric; R-10)
-SX_DEV int round_count(float phi, float h, int mode, float tol_fl) {
+__device__ __noinline__ int round_count(float phi, float h, int mode, float tol_fl) {
     if (mode == kModeArc) return (phi <= 0.5f * kPi) ? 1 : 2;
     float n_f = 1.0f;
     if (tol_fl < h) n_f = ceilf(phi / (2.0f * acosf(1.0f - tol_fl / h)));
@@ -129,7 +129,7 @@ SX_DEV uint32_t emit_join(const Params& P, const Style& st, V2 V, V2 T0, V2 W, V
     const bool arc = P.mode == kModeArc;
     float phi = 0.0f;
     uint32_t n_outer = miter ? 2u : 1u;
-    if (round) { phi = fabsf(atan2f(cr, dt)); n_outer = (uint32_t)round_count(phi, h, P.mode, P.tol_fl); }
+    if (round) { phi = fabsf(atan2_r(cr, dt)); n_outer = (uint32_t)round_count(phi, h, P.mode, P.tol_fl); }
     if (EMIT) {
         // side 0 (-h, forward V -> W) comes first, then side 1 (+h, backward W -> V)
         const uint32_t first_outer = first + (outer_minus ? 0u : 2u), first_inner = first + (outer_minus ? n_outer : 0u);
@@ -213,8 +213,9 @@ SX_DEV bool fit_next(const Params& P, const Seg& s, FitState& f, Piece& p) {
         float next_qmag, th0, th1, chord;
         eval_cubic(s, t1, f.dt, &next_p, &next_qmag, &next_u);
         V2 ch = next_p - f.last_p;
-        float err = fit_error(f.last_u, next_u, f.last_qmag, next_qmag, ch, f.dt, &th0, &th1, &chord);
+        float err = node_error(f.last_u, next_u, f.last_qmag, next_qmag, ch, f.dt);
         if (err <= P.tol_es || f.dt <= kDtMin) {
+            piece_angles(f.last_u, next_u, ch, &th0, &th1, &chord);
             p.base = s.P0; p.P3 = s.P3;
             p.la = f.last_p; p.lb = next_p;
             p.ua = f.last_u; p.ub = next_u;
@@ -249,11 +250,7 @@ SX_DEV uint32_t flatten_cubic(const Params& P, const Seg& s, float h, const Writ
 
 // ---------------------------------------------------------------- Alg. 1: the whole segment
 SX_DEV bool load_style(const Params& P, uint32_t path, Style* st, float* h) {
-#ifdef __CUDA_ARCH__
     uint4 raw = __ldg(reinterpret_cast<const uint4*>(P.styles) + path);
-#else
-    uint4 raw = reinterpret_cast<const uint4*>(P.styles)[path];
-#endif
     st->width = u2f(raw.x);
     st->miter_limit = u2f(raw.y);
     st->join = (int)(raw.z & 0xffu);
