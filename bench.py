@@ -291,16 +291,14 @@ def run_ours(args):
     # ---- per-kernel durations: the library's own events on the launching stream, one query (sync) per step
     B.sx_set_option(ctx, B.SX_OPT_TIME_KERNELS, 1)
     k_steps = max(3, min(args.steps, 10))
-    t_scan = t_expand = 0.0
+    t_k = np.zeros(4)
     for k in range(k_steps):
         flush.fill_(k & 0xff)
         step()
-        a, b = B.sx_kernel_times(ctx)
-        t_scan += a * 1e-3
-        t_expand += b * 1e-3
+        t_k += np.array(B.sx_kernel_times(ctx)) * 1e-3
     B.sx_set_option(ctx, B.SX_OPT_TIME_KERNELS, 0)
-    t_scan /= k_steps
-    t_expand /= k_steps
+    t_k /= k_steps
+    t_scan, t_count, t_alloc, t_write = (float(x) for x in t_k)
 
     # ---- the one-shot call with an unknown record count: count pass, host read of the total, allocation, write pass
     o_steps = max(3, min(args.steps, 5))
@@ -337,24 +335,26 @@ def run_ours(args):
         t_step = t_total / args.steps
         # algorithmic bytes: the streams read once, the records and the path offsets written once
         alg_bytes = tags.numel() + pts.numel() * 4 + sty.numel() + total * width * 4 + (n_paths + 1) * 8
-        ach = alg_bytes / t_expand / 1e9
+        dominant, t_dom = max((("k_count (count pass: fit, counts, leaf records)", t_count), ("writers (k_write_segments, k_write_simple, k_write_general, k_write_walk)", t_write)), key=lambda kv: kv[1])
+        ach = alg_bytes / t_dom / 1e9
         key = f"{args.workload}-{'arc' if mode else 'line'}"
         line = {"metric": METRIC, "value": job_throughput(n_seg, args.steps, world, t_total), "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": warm, "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": args.workload, "segments": n_seg, "paths": n_paths, "records": int(total),
                            "mode": "arc" if mode else "line", "tolerance": float(sc.tolerance), "l2": "flushed between steps (256 MiB fill)",
-                           "call": "stroke_expand_into (one pass: tag scan + fused count / allocation scan / write)",
+                           "call": "stroke_expand_into (tag scan, count pass, allocation scan, writers; asynchronous, no host round trip)",
                            "parallelism": "replicas only" if world > 1 else "single GPU"},
                 "output_records_per_s": job_throughput(total, args.steps, world, t_total),
-                "kernel_ms": {"k_tag_scan": 1e3 * t_scan, "k_expand": 1e3 * t_expand, "timed_by": "library events on the launching stream, mean of %d steps" % k_steps},
+                "kernel_ms": {"k_tag_scan": 1e3 * t_scan, "k_count": 1e3 * t_count, "k_alloc_scan": 1e3 * t_alloc, "writers": 1e3 * t_write,
+                              "timed_by": "library events on the launching stream, mean of %d steps" % k_steps},
                 "tiles": stats,
                 "gpu_launches": int(launches), "clocks": clocks,
                 "one_shot": {"call": "stroke_expand (count pass, host read of the total, allocation callback, write pass)",
                              "ms_per_call_wall": 1e3 * t_one, "value": n_seg / t_one, "unit": UNIT},
                 "e2e": {"value": job_throughput(n_seg, e2e_steps, world, t_e2e), "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                         "ms_per_step": 1e3 * t_e2e / e2e_steps},
-                "roofline": {"kernel": "k_expand (count + allocation scan + write in one pass): %.1f %% of the step" % (100 * t_expand / (t_scan + t_expand)),
+                "roofline": {"kernel": "%s: %.1f %% of the step" % (dominant, 100 * t_dom / float(t_k.sum())),
                              "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                              "traffic": NCU_TRAFFIC.get(key) if args.paths is None else None, "traffic_source": NCU_TRAFFIC_SOURCE,
                              "peak_source": peak_src, "algorithmic_bytes_per_launch": int(alg_bytes),

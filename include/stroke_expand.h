@@ -108,9 +108,11 @@ sx_status sx_create(sx_ctx** out, int32_t device);
 sx_status sx_destroy(sx_ctx* ctx);
 
 /* ------------------------------------------------------------------ phase 1: scan + count + scan
- * Runs kernels (a) tag-stream scan and the count-only instance of the expansion kernel:
- * (b) per-segment count (Alg. 1/2 without the writes) and (c) the allocation scan.  Use this pair of calls when the
- * output buffer can only be allocated once the record count is known; stroke_expand_into below needs one pass.
+ * Runs kernels (a) tag-stream scan, (b) the count pass -- the cubic -> Euler-spiral fit of Alg. 2
+ * (L351-438) and the per-side subdivision counts (sections 4-6), which also leaves one 32-byte record per
+ * Euler-spiral piece in the context's scratch -- and (c) the allocation scan over the per-segment counts (replaces the
+ * atomic bump allocation of L448).  Use this pair of calls when the output buffer can only be allocated once the record
+ * count is known; stroke_expand_into below issues both phases in one asynchronous call.
  *   d_tags[n_tags], d_points_xy[2*n_points], d_styles[n_paths]   device, read-only.  ALIGNMENT: d_tags and d_styles
  *                 16 bytes, d_points_xy and d_path_offsets 8 bytes (the kernels use vector loads); a pointer that
  *                 is not aligned so is rejected with SX_E_INVALID_ARG (a contiguous but offset tensor view can be)
@@ -132,18 +134,16 @@ sx_status sx_count(sx_ctx* ctx, const uint8_t* d_tags, uint64_t n_tags, const fl
 
 /* ------------------------------------------------------------------ phase 2: write
  * Writes the records of the preceding sx_count into d_out_records (sx_line[] or sx_arc[] by mode, 16-byte
- * aligned) of capacity cap_records: the expansion kernel again, on the same inputs, with the stores on (nothing
- * is cached between the phases: the count pass is the same code and takes the same decisions).  SX_E_CAPACITY
- * if the capacity is known to be too small (the total is known on the host only when sx_count was given
- * h_total; otherwise the kernel itself refuses to write past the capacity and the error is reported by
- * sx_last_error after a stream sync). */
+ * aligned) of capacity cap_records: kernels (d), the writers, which read the per-segment offsets and the piece
+ * records phase 1 left (the fit is not repeated).  SX_E_CAPACITY if the capacity is known to be too small (the total
+ * is known on the host only when sx_count was given h_total; otherwise the kernels themselves refuse to write past
+ * the capacity and the error is reported by sx_last_error after a stream sync). */
 sx_status sx_write(sx_ctx* ctx, void* d_out_records, uint64_t cap_records, void* cuda_stream);
 
-/* ------------------------------------------------------------------ one pass into a caller-provided buffer
- * The whole path in ONE pass: kernel (a), then the expansion kernel with count (b), allocation scan (c) and write
- * (d) fused -- Alg. 1 / Alg. 2 run once per segment, nothing between the input streams and the records goes
- * through device memory.  Inputs as for sx_count.  d_out_records (16-byte aligned) has room for cap_records
- * records.  The count is always computed in full: a tile of segments whose records would pass the capacity is not
+/* ------------------------------------------------------------------ one call into a caller-provided buffer
+ * The whole path -- kernels (a), (b), (c), (d) -- in one asynchronous call without a host round trip: Alg. 1 / Alg. 2
+ * run once per segment.  Inputs as for sx_count.  d_out_records (16-byte aligned) has room for cap_records
+ * records.  The count is always computed in full: a segment whose records would pass the capacity is not
  * written, the device-side capacity flag is raised (sx_last_error) and the total is still exact, so the caller can
  * retry with a buffer of that size.  h_total (HOST, optional): when non-NULL the call synchronises the stream,
  * writes the record count and returns SX_E_BAD_STREAM / SX_E_CAPACITY (count > cap_records) accordingly; when NULL
@@ -166,8 +166,8 @@ sx_status stroke_expand(sx_ctx* ctx, const uint8_t* d_tags, uint64_t n_tags, con
 
 /* ------------------------------------------------------------------ one-shot, HOST buffers (end to end)
  * Same computation with every buffer on the host (pinned memory gives asynchronous copies): copies
- * the streams to the device, runs the one-pass path (stroke_expand_into on a staging buffer owned by the
- * context; a second pass only when that buffer had to grow), copies records and path offsets back.
+ * the streams to the device, runs stroke_expand_into on a staging buffer owned by the context (a second time only
+ * when that buffer had to grow), copies records and path offsets back.
  * h_out_records has room for cap_records records; *h_n_records receives the count even when
  * SX_E_CAPACITY is returned (so the caller can retry).  Returns after the results are in host memory. */
 sx_status stroke_expand_host(sx_ctx* ctx, const uint8_t* h_tags, uint64_t n_tags, const float* h_points_xy, uint64_t n_points,
@@ -178,8 +178,7 @@ sx_status stroke_expand_host(sx_ctx* ctx, const uint8_t* h_tags, uint64_t n_tags
 /* ------------------------------------------------------------------ introspection
  * Device pointers into the context's scratch of the last sx_count (valid until the next call on the
  * context): the tag-scan results and the per-segment record counts / offsets.  Any out pointer may
- * be NULL.  Used by the parity tests and the bench report.  stroke_expand_into keeps the per-segment counts /
- * offsets only under SX_OPT_KEEP_SEGMENT_INFO (12 bytes per segment of extra stores); SX_E_STATE otherwise. */
+ * be NULL.  Used by the parity tests and the bench report.  SX_E_STATE before the first count. */
 sx_status sx_segment_info(sx_ctx* ctx, const uint32_t** d_pt_off, const uint32_t** d_path_idx, const uint32_t** d_sp_first,
                           const uint32_t** d_seg_count, const uint64_t** d_seg_offset);
 
@@ -189,24 +188,25 @@ sx_status sx_last_error(sx_ctx* ctx, void* cuda_stream);
 
 /* Options of a context. */
 enum {
-    SX_OPT_KEEP_SEGMENT_INFO = 1, /* value != 0: stroke_expand_into also stores the per-segment counts / offsets        */
+    SX_OPT_KEEP_SEGMENT_INFO = 1, /* accepted and ignored: the per-segment counts / offsets are always kept              */
     SX_OPT_TIME_KERNELS = 3,      /* value != 0: the library records CUDA events around its kernels (sx_kernel_times)          */
-    SX_OPT_TILES_PER_RANGE = 2    /* test knob for the expansion kernel, which works on ranges of 128 segments as 1, 2 or
-                                     4 tiles (adapted on the device to what fits its shared-memory tables): 0 adaptive
-                                     (default), 1 / 2 / 4 fixed, 8 = every tile takes the thread-per-segment reference
-                                     walk.  The records do not depend on it (tests/test_gpu_parity.py).               */
+    SX_OPT_TILE_SEGMENTS = 2      /* test knob for the count pass, whose warps work on tiles of 32, 16 or 8 segments
+                                     (adapted on the device to what fits a warp's shared-memory tables): 0 adaptive
+                                     (default); 8 / 16 / 32 fixed; 2 = every tile is redone in sub-tiles of 8 segments
+                                     (the path of a tile that overflowed); 1 = every tile takes the thread-per-segment
+                                     reference walk.  The records do not depend on it (tests/test_gpu_parity.py).      */
 };
 sx_status sx_set_option(sx_ctx* ctx, int32_t option, uint64_t value);
 
-/* Statistics of the last expansion kernel on the context (synchronises `cuda_stream`): h_out4[0] tiles that ran
- * from shared memory, [1] tiles that took the thread-per-segment walk, [2] tiles per range now in use, [3] segments
- * per range. */
+/* Statistics of the last count pass on the context (synchronises `cuda_stream`): h_out4[0] tiles done in one
+ * go from shared memory, [1] tiles redone in sub-tiles, [2] segments that took the thread-per-segment walk, [3] the
+ * tile size (segments) of the call. */
 sx_status sx_call_stats(sx_ctx* ctx, uint64_t* h_out4, void* cuda_stream);
 
-/* Device durations of the two kernels of the last one-pass / count / write call made under SX_OPT_TIME_KERNELS, from
- * CUDA events recorded on the call's own stream: h_ms2[0] tag scan (a), h_ms2[1] expansion kernel (b + c + d).
- * Waits for the call to finish.  SX_E_STATE when nothing was timed. */
-sx_status sx_kernel_times(sx_ctx* ctx, float* h_ms2);
+/* Device durations of the kernels of the last stroke_expand_into call made under SX_OPT_TIME_KERNELS, from CUDA events
+ * recorded on the call's own stream: h_ms4[0] tag scan (a), [1] count pass (b), [2] allocation scan (c), [3] the
+ * writers (d).  Waits for the call to finish.  SX_E_STATE when nothing was timed. */
+sx_status sx_kernel_times(sx_ctx* ctx, float* h_ms4);
 
 /* Issue-rate microbenchmarks on `device` (host-synchronous, ~20 ms): h_out3[0] FP32 FMA lane-operations per second
  * (independent FFMA chains on all SMs), [1] issued lane-operations per second of an FFMA + integer-ALU mix, [2]

@@ -21,7 +21,7 @@ RECORD_BYTES = {SX_MODE_LINE: 16, SX_MODE_ARC: 32}
 ARC_DTYPE = np.dtype([("x0", "<f4"), ("y0", "<f4"), ("x1", "<f4"), ("y1", "<f4"), ("angle", "<f4"), ("seg", "<u4"),
                       ("kind", "<u4"), ("pad", "<u4")])
 
-SX_OPT_KEEP_SEGMENT_INFO, SX_OPT_TILES_PER_RANGE, SX_OPT_TIME_KERNELS = 1, 2, 3
+SX_OPT_KEEP_SEGMENT_INFO, SX_OPT_TILE_SEGMENTS, SX_OPT_TIME_KERNELS = 1, 2, 3
 
 EXPORTS = ["sx_create", "sx_destroy", "sx_count", "sx_write", "stroke_expand", "stroke_expand_into", "stroke_expand_host",
            "sx_segment_info", "sx_last_error", "sx_set_option", "sx_call_stats", "sx_kernel_times", "sx_measure_issue_peaks", "sx_launch_count",
@@ -242,17 +242,17 @@ def sx_set_option(ctx, option, value):
 
 
 def sx_call_stats(ctx, stream=None):
-    """dict(fast_tiles, slow_tiles, tiles_per_range, range_segments) of the last expansion kernel on the context."""
+    """dict(direct_tiles, sub_tiled_tiles, walk_segments, tile_segments) of the last expansion kernel on the context."""
     out = (C.c_uint64 * 4)()
     _check(lib().sx_call_stats(ctx, out, _stream_ptr(stream)), "sx_call_stats")
-    return dict(fast_tiles=int(out[0]), slow_tiles=int(out[1]), tiles_per_range=int(out[2]), range_segments=int(out[3]))
+    return dict(direct_tiles=int(out[0]), sub_tiled_tiles=int(out[1]), walk_segments=int(out[2]), tile_segments=int(out[3]))
 
 
 def sx_kernel_times(ctx):
-    """(tag scan ms, expansion kernel ms) of the last call made under SX_OPT_TIME_KERNELS (waits for it)."""
-    out = (C.c_float * 2)()
+    """(tag scan, count pass, allocation scan, writers) in ms of the last call made under SX_OPT_TIME_KERNELS (waits for it)."""
+    out = (C.c_float * 4)()
     _check(lib().sx_kernel_times(ctx, out), "sx_kernel_times")
-    return float(out[0]), float(out[1])
+    return tuple(float(x) for x in out)
 
 
 def sx_measure_issue_peaks(device=0):

@@ -1,8 +1,9 @@
 // sx_kernels.cu -- the C-ABI of include/stroke_expand.h and the host side of the pipeline.
 //
-// Kernels: (a) k_tag_scan (sx_scan.cuh), then k_expand (sx_expand.cuh): count (b), allocation scan (c) and write (d)
-// in one pass.  The curve mathematics is in sx_math.cuh / sx_piece.cuh, the thread-per-segment reference walk in
-// sx_segment.cuh, the part tables of the record-parallel writer in sx_cache.cuh.  sx_peaks.cuh: issue-rate microbenchmarks.
+// Kernels, all on the caller's stream: (a) k_tag_scan, (b) k_count (fit + counts + leaf records), (c) k_alloc_scan
+// (sx_scan.cuh, sx_count.cuh); (d) the four writers of sx_write.cuh.  The curve mathematics is in sx_math.cuh /
+// sx_piece.cuh, the thread-per-segment reference walk in sx_segment.cuh, the part tables of the record-parallel writer in
+// sx_cache.cuh.  sx_peaks.cuh: issue-rate microbenchmarks.
 //
 // Build: nvcc -gencode arch=compute_100a,code=sm_100a -fmad=false -lineinfo -shared (see ../build.py).
 // -fmad=false is part of the design: see the arithmetic discipline note in sx_math.cuh.
@@ -13,7 +14,7 @@
 #include <math.h>
 
 #include "../../include/stroke_expand.h"
-#include "sx_expand.cuh"
+#include "sx_write.cuh"
 #include "sx_peaks.cuh"
 
 // ====================================================================== host side
@@ -25,25 +26,31 @@ static thread_local cudaError_t g_last_cuda = cudaSuccess;
         if (e_ != cudaSuccess) { g_last_cuda = e_; return SX_E_CUDA; } \
     } while (0)
 
+constexpr int kEvents = 5;   // SX_OPT_TIME_KERNELS: before the tag scan, after it, after the count, after the allocation scan, after the writers
+
 struct sx_ctx {
     int device;
     // scratch of the call in flight
-    uint32_t *pt_off, *path_idx, *sp_first, *seg_count;
+    uint32_t *pt_off, *path_idx, *sp_first, *seg_count, *seg_tail, *walk_list;
     uint64_t* seg_off;
     uint64_t cap_segs;
-    uint8_t* sync_area;   // [flags, tickets, stats: 64 B][d_total 64 B][look-back words of k_expand][tag tile states]
+    sx::LeafRec* leaves;  // the Euler-spiral pieces between the count pass and the writers (32 B each)
+    uint64_t leaf_cap;
+    double leaves_per_seg;  // the most a call on this context has needed so far (learned whenever a call reads its total)
+    uint8_t* sync_area;   // [flags, tickets, statistics, counters: 128 B][d_total 128 B][look-back words of the allocation scan][tag tile states]
     uint64_t sync_bytes;
-    uint32_t* d_hint;     // tiles per range the blocks of k_expand start with (adapted on the device, kept across calls)
-    uint64_t* h_pinned;   // pinned: [0] total, [1] flags, [2] stats
+    uint32_t* d_hint;     // [0] tile size of the call in flight, [1] the one the last count pass proposed (adapted on the device, kept across calls)
+    uint64_t* h_pinned;   // pinned: [0] total, [1] flags, [2..3] stats, [4] leaf counter
     int sm_count;
-    cudaEvent_t ev[3];    // SX_OPT_TIME_KERNELS: before the tag scan, between the kernels, after the expansion kernel
+    int count_blocks, simple_blocks, general_blocks;   // persistent grids: resident blocks on the device
+    cudaEvent_t ev[kEvents];
     bool time_kernels, timed;
     // options
-    bool keep_info;       // SX_OPT_KEEP_SEGMENT_INFO
-    uint32_t force_tiles; // SX_OPT_TILES_PER_RANGE
+    uint32_t force_tiles; // SX_OPT_TILE_SEGMENTS
     // last sx_count / stroke_expand_into
-    sx::ExArgs A;
-    bool counted, total_known, info_valid;
+    sx::CountArgs C;
+    sx::WriteArgs W;
+    bool counted, total_known;
     uint64_t total;
     uint64_t launches;
     // staging for stroke_expand_host
@@ -52,19 +59,23 @@ struct sx_ctx {
     uint64_t* st_path; uint64_t st_path_n;
 };
 
-static uint32_t* ctx_err(sx_ctx* c) { return reinterpret_cast<uint32_t*>(c->sync_area); }
-static uint32_t* ctx_ticket(sx_ctx* c, int k) { return reinterpret_cast<uint32_t*>(c->sync_area) + 4 + 4 * k; }
-static uint32_t* ctx_stats(sx_ctx* c) { return reinterpret_cast<uint32_t*>(c->sync_area) + 12; }
-static uint64_t* ctx_total(sx_ctx* c) { return reinterpret_cast<uint64_t*>(c->sync_area + 64); }
-static uint64_t* ctx_states(sx_ctx* c) { return reinterpret_cast<uint64_t*>(c->sync_area + 128); }
+constexpr uint64_t kHeadBytes = 256;
+static uint32_t* ctx_word(sx_ctx* c, int k) { return reinterpret_cast<uint32_t*>(c->sync_area) + k; }
+static uint32_t* ctx_err(sx_ctx* c) { return ctx_word(c, 0); }
+static uint32_t* ctx_ticket(sx_ctx* c, int k) { return ctx_word(c, 4 + 4 * k); }   // 0 tag scan, 1 count, 2 allocation scan
+static uint32_t* ctx_stats(sx_ctx* c) { return ctx_word(c, 16); }                   // sx::kStWords words
+static unsigned long long* ctx_leaf_counter(sx_ctx* c) { return reinterpret_cast<unsigned long long*>(ctx_word(c, 24)); }
+static uint32_t* ctx_leaf_end_inv(sx_ctx* c) { return ctx_word(c, 26); }
+static uint32_t* ctx_walk_count(sx_ctx* c) { return ctx_word(c, 28); }
+static uint64_t* ctx_total(sx_ctx* c) { return reinterpret_cast<uint64_t*>(c->sync_area + 128); }
+static uint64_t* ctx_states(sx_ctx* c) { return reinterpret_cast<uint64_t*>(c->sync_area + kHeadBytes); }
 
 static uint64_t round_up(uint64_t x, uint64_t m) { return (x + m - 1) / m * m; }
-static uint64_t n_ranges(uint64_t n) { return (n + sx::kExRange - 1) / sx::kExRange; }
-static uint64_t states_bytes(uint64_t n) { return round_up((n_ranges(n) * sx::kExSlotsPerRange + 1) * 8, 64); }
+static uint64_t states_bytes(uint64_t n) { return round_up(((n + sx::kCntTile - 1) / sx::kCntTile + 1) * 8, 64); }
 
 static sx_status ensure_scratch(sx_ctx* c, uint64_t n) {
     uint64_t n_tag_tiles = (n + sx::kTagTile - 1) / sx::kTagTile + 1;
-    uint64_t need_sync = 128 + states_bytes(n) + n_tag_tiles * sizeof(sx::TagTileState);
+    uint64_t need_sync = kHeadBytes + states_bytes(n) + n_tag_tiles * sizeof(sx::TagTileState);
     if (need_sync > c->sync_bytes) {
         if (c->sync_area) SX_CUDA(cudaFree(c->sync_area));
         c->sync_area = nullptr; c->sync_bytes = 0;
@@ -76,15 +87,28 @@ static sx_status ensure_scratch(sx_ctx* c, uint64_t n) {
         if (c->pt_off) SX_CUDA(cudaFree(c->pt_off));
         c->pt_off = nullptr; c->cap_segs = 0;
         uint64_t cap = round_up(n + n / 8 + 64, 64);
-        // one allocation: 4 u32 arrays then the u64 offsets (all 256-byte aligned since cap % 64 == 0)
+        // one allocation: 6 u32 arrays then the u64 offsets (all 256-byte aligned since cap % 64 == 0)
         uint8_t* p;
-        SX_CUDA(cudaMalloc(&p, cap * (4 * 4 + 8)));
+        SX_CUDA(cudaMalloc(&p, cap * (6 * 4 + 8)));
         c->pt_off = reinterpret_cast<uint32_t*>(p);
         c->path_idx = c->pt_off + cap;
         c->sp_first = c->path_idx + cap;
         c->seg_count = c->sp_first + cap;
-        c->seg_off = reinterpret_cast<uint64_t*>(c->seg_count + cap);
+        c->seg_tail = c->seg_count + cap;
+        c->walk_list = c->seg_tail + cap;
+        c->seg_off = reinterpret_cast<uint64_t*>(c->walk_list + cap);
         c->cap_segs = cap;
+    }
+    // leaf buffer: 4 pieces per segment to begin with, or what the scenes seen on this context needed (+ 15 %); a buffer
+    // that turns out too small costs speed, not correctness (the tiles that find no room take the walk)
+    double per_seg = c->leaves_per_seg * 1.15 > 4.0 ? c->leaves_per_seg * 1.15 : 4.0;
+    uint64_t need_leaves = static_cast<uint64_t>(per_seg * static_cast<double>(n)) + 4096;
+    if (need_leaves > 0xfffffff0ull) need_leaves = 0xfffffff0ull;
+    if (need_leaves > c->leaf_cap) {
+        if (c->leaves) SX_CUDA(cudaFree(c->leaves));
+        c->leaves = nullptr; c->leaf_cap = 0;
+        SX_CUDA(cudaMalloc(&c->leaves, need_leaves * sizeof(sx::LeafRec)));
+        c->leaf_cap = need_leaves;
     }
     return SX_OK;
 }
@@ -107,15 +131,15 @@ static sx_status check_inputs(const uint8_t* d_tags, uint64_t n_tags, const floa
     return SX_OK;
 }
 
-// resets the per-call device state and runs (a) the tag scan; fills c->A for k_expand
-static sx_status begin_call(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, const float* d_points_xy, uint64_t n_points,
-                            const sx_style* d_styles, uint64_t n_paths, const float* h_affine, float tolerance, int32_t mode,
-                            uint64_t* d_path_offsets, cudaStream_t s) {
+// phase 1: resets the per-call device state and runs (a) the tag scan, (b) the count pass, (c) the allocation scan
+static sx_status run_count(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, const float* d_points_xy, uint64_t n_points,
+                           const sx_style* d_styles, uint64_t n_paths, const float* h_affine, float tolerance, int32_t mode,
+                           uint64_t* d_path_offsets, cudaStream_t s) {
     SX_CUDA(cudaSetDevice(c->device));
     sx_status rc = ensure_scratch(c, n_tags);
     if (rc != SX_OK) return rc;
-    sx::ExArgs& A = c->A;
-    sx::Params& P = A.P;
+    sx::CountArgs& C = c->C;
+    sx::Params& P = C.P;
     P.tags = d_tags; P.pts = d_points_xy; P.styles = reinterpret_cast<const uint8_t*>(d_styles);
     P.pt_off = c->pt_off; P.path_idx = c->path_idx; P.sp_first = c->sp_first;
     for (int k = 0; k < 6; k++) P.A[k] = h_affine[k];
@@ -125,45 +149,64 @@ static sx_status begin_call(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, c
     P.tol_fl = 0.8f * tolerance;
     P.mode = mode;
     P.n_tags = static_cast<uint32_t>(n_tags);
-    A.n_paths = static_cast<uint32_t>(n_paths);
-    A.states = ctx_states(c);
-    A.ticket = ctx_ticket(c, 1);
-    A.err = ctx_err(c);
-    A.path_off = d_path_offsets;
-    A.d_total = ctx_total(c);
-    A.seg_count = nullptr; A.seg_off = nullptr;
-    A.out = nullptr; A.cap_records = 0;
-    A.stats = ctx_stats(c);
-    A.hint = c->d_hint;
-    A.force_tiles = c->force_tiles;
+    C.n_paths = static_cast<uint32_t>(n_paths);
+    C.ticket = ctx_ticket(c, 1);
+    C.err = ctx_err(c);
+    C.seg_count = c->seg_count; C.seg_tail = c->seg_tail;
+    C.leaves = c->leaves; C.leaf_cap = static_cast<uint32_t>(c->leaf_cap);
+    C.leaf_counter = ctx_leaf_counter(c); C.leaf_end_inv = ctx_leaf_end_inv(c);
+    C.walk_list = c->walk_list; C.walk_count = ctx_walk_count(c);
+    C.stats = ctx_stats(c);
+    C.hint = c->d_hint;
+    C.force = c->force_tiles;
+    sx::WriteArgs& W = c->W;
+    W.P = P;
+    W.seg_count = c->seg_count; W.seg_tail = c->seg_tail; W.seg_off = c->seg_off;
+    W.leaves = c->leaves; W.leaf_cap = C.leaf_cap; W.leaf_counter = C.leaf_counter; W.leaf_end_inv = C.leaf_end_inv;
+    W.walk_list = c->walk_list; W.walk_count = C.walk_count;
+    W.out = nullptr; W.cap_records = 0; W.err = C.err;
     c->total_known = false;
-    c->info_valid = false;
     c->total = 0;
-    // error flag, tickets, statistics, total, look-back words of both scans
+    c->timed = false;
+    // error flag, tickets, statistics, counters, total, look-back words of both scans
     SX_CUDA(cudaMemsetAsync(c->sync_area, 0, c->sync_bytes, s));
     if (n_tags == 0) {
         SX_CUDA(cudaMemsetAsync(d_path_offsets, 0, 8, s));
         return SX_OK;
     }
     uint32_t n = P.n_tags;
-    uint32_t n_tag_tiles = (n + sx::kTagTile - 1) / sx::kTagTile;
-    c->timed = false;
     if (c->time_kernels) SX_CUDA(cudaEventRecord(c->ev[0], s));
-    sx::TagTileState* tag_states = reinterpret_cast<sx::TagTileState*>(c->sync_area + 128 + states_bytes(n));
+    uint32_t n_tag_tiles = (n + sx::kTagTile - 1) / sx::kTagTile;
+    sx::TagTileState* tag_states = reinterpret_cast<sx::TagTileState*>(c->sync_area + kHeadBytes + states_bytes(n));
     sx::k_tag_scan<<<n_tag_tiles, sx::kScanThreads, 0, s>>>(d_tags, n, (uint32_t)n_points, (uint32_t)n_paths, c->pt_off, c->path_idx, c->sp_first,
-                                                           tag_states, ctx_ticket(c, 0), ctx_err(c));
-    c->launches += 1;
+                                                           tag_states, ctx_ticket(c, 0), ctx_err(c), c->d_hint);
     if (c->time_kernels) SX_CUDA(cudaEventRecord(c->ev[1], s));
+    // persistent one-warp blocks: no more of them than there are tiles of the smallest size
+    uint64_t tiles = (n + sx::kCtSub - 1) / sx::kCtSub;
+    unsigned grid = (unsigned)(tiles < (uint64_t)c->count_blocks ? tiles : (uint64_t)c->count_blocks);
+    sx::k_count<<<grid, 32, sizeof(sx::CtWarp), s>>>(C);
+    if (c->time_kernels) SX_CUDA(cudaEventRecord(c->ev[2], s));
+    uint32_t n_cnt_tiles = (n + sx::kCntTile - 1) / sx::kCntTile;
+    sx::k_alloc_scan<<<n_cnt_tiles, sx::kScanThreads, 0, s>>>(c->seg_count, n, d_tags, c->path_idx, (uint32_t)n_paths, c->seg_off, d_path_offsets,
+                                                             ctx_total(c), ctx_states(c), ctx_ticket(c, 2), ctx_err(c));
+    if (c->time_kernels) SX_CUDA(cudaEventRecord(c->ev[3], s));
+    c->launches += 3;
+    SX_CUDA(cudaGetLastError());
     return SX_OK;
 }
 
-template <bool WRITE>
-static sx_status launch_expand(sx_ctx* c, cudaStream_t s) {
-    uint32_t n = c->A.P.n_tags;
+// phase 2: (d) the writers
+static sx_status run_write(sx_ctx* c, void* d_out_records, uint64_t cap_records, cudaStream_t s) {
+    uint32_t n = c->W.P.n_tags;
     if (n == 0) return SX_OK;
-    sx::k_expand<WRITE><<<(unsigned)n_ranges(n), sx::kExThreads, sizeof(sx::ExShared), s>>>(c->A);
-    c->launches += 1;
-    if (c->time_kernels) { SX_CUDA(cudaEventRecord(c->ev[2], s)); c->timed = true; }
+    c->W.out = static_cast<float4*>(d_out_records);
+    c->W.cap_records = cap_records;
+    sx::k_write_segments<<<(n + sx::kWrThreads - 1) / sx::kWrThreads, sx::kWrThreads, 0, s>>>(c->W);
+    sx::k_write_simple<<<c->simple_blocks, sx::kWrThreads, 0, s>>>(c->W);
+    sx::k_write_general<<<c->general_blocks, sx::kWrThreads, 0, s>>>(c->W);
+    sx::k_write_walk<<<c->sm_count, sx::kWrThreads, 0, s>>>(c->W);
+    c->launches += 4;
+    if (c->time_kernels) { SX_CUDA(cudaEventRecord(c->ev[4], s)); c->timed = true; }
     SX_CUDA(cudaGetLastError());
     return SX_OK;
 }
@@ -172,12 +215,19 @@ static sx_status launch_expand(sx_ctx* c, cudaStream_t s) {
 static sx_status read_total(sx_ctx* c, cudaStream_t s, uint64_t* h_total) {
     SX_CUDA(cudaMemcpyAsync(&c->h_pinned[0], ctx_total(c), 8, cudaMemcpyDeviceToHost, s));
     SX_CUDA(cudaMemcpyAsync(&c->h_pinned[1], ctx_err(c), 4, cudaMemcpyDeviceToHost, s));
+    SX_CUDA(cudaMemcpyAsync(&c->h_pinned[4], ctx_leaf_counter(c), 8, cudaMemcpyDeviceToHost, s));
     SX_CUDA(cudaStreamSynchronize(s));
     uint32_t flags = static_cast<uint32_t>(c->h_pinned[1] & 0xffffffffu);
     if (flags & sx::kErrBadStream) { *h_total = 0; return SX_E_BAD_STREAM; }
     *h_total = c->h_pinned[0];
     c->total = c->h_pinned[0];
     c->total_known = true;
+    // how many pieces the scene has per segment: sizes the leaf buffer of the calls that follow
+    uint64_t leaves = (c->h_pinned[4] & 0xffffffffull) + (c->h_pinned[4] >> 32);
+    if (c->C.P.n_tags > 0) {
+        double per_seg = static_cast<double>(leaves) / static_cast<double>(c->C.P.n_tags);
+        if (per_seg > c->leaves_per_seg) c->leaves_per_seg = per_seg;
+    }
     return SX_OK;
 }
 
@@ -199,13 +249,18 @@ sx_status sx_create(sx_ctx** out, int32_t device) {
     cudaError_t e = cudaMallocHost(reinterpret_cast<void**>(&c->h_pinned), 64);
     if (e != cudaSuccess) { g_last_cuda = e; free(c); return SX_E_CUDA; }
     e = cudaMalloc(&c->d_hint, 64);
-    uint32_t one = 1u;
-    if (e == cudaSuccess) e = cudaMemcpy(c->d_hint, &one, 4, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sx::k_expand<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(sx::ExShared));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sx::k_expand<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(sx::ExShared));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sx::k_expand<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sx::k_expand<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    for (int k = 0; k < 3 && e == cudaSuccess; k++) e = cudaEventCreate(&c->ev[k]);
+    uint32_t first[2] = {(uint32_t)sx::kCtTile, (uint32_t)sx::kCtTile};
+    if (e == cudaSuccess) e = cudaMemcpy(c->d_hint, first, 8, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sx::k_count, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(sx::CtWarp));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sx::k_count, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    int per_sm = 0;
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sx::k_count, 32, sizeof(sx::CtWarp));
+    c->count_blocks = c->sm_count * (per_sm > 0 ? per_sm : 1);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sx::k_write_simple, sx::kWrThreads, 0);
+    c->simple_blocks = c->sm_count * (per_sm > 0 ? per_sm : 1);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sx::k_write_general, sx::kWrThreads, 0);
+    c->general_blocks = c->sm_count * (per_sm > 0 ? per_sm : 1);
+    for (int k = 0; k < kEvents && e == cudaSuccess; k++) e = cudaEventCreate(&c->ev[k]);
     if (e != cudaSuccess) { g_last_cuda = e; cudaFree(c->d_hint); cudaFreeHost(c->h_pinned); free(c); return SX_E_CUDA; }
     *out = c;
     return SX_OK;
@@ -215,8 +270,9 @@ sx_status sx_destroy(sx_ctx* c) {
     if (!c) return SX_E_INVALID_ARG;
     cudaSetDevice(c->device);
     cudaDeviceSynchronize();
-    for (int k = 0; k < 3; k++) cudaEventDestroy(c->ev[k]);
+    for (int k = 0; k < kEvents; k++) cudaEventDestroy(c->ev[k]);
     cudaFree(c->pt_off);
+    cudaFree(c->leaves);
     cudaFree(c->sync_area);
     cudaFree(c->d_hint);
     cudaFree(c->st_in);
@@ -235,13 +291,9 @@ sx_status sx_count(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, const floa
     sx_status rc = check_inputs(d_tags, n_tags, d_points_xy, n_points, d_styles, n_paths, h_affine, tolerance, mode, d_path_offsets);
     if (rc != SX_OK) return rc;
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-    rc = begin_call(c, d_tags, n_tags, d_points_xy, n_points, d_styles, n_paths, h_affine, tolerance, mode, d_path_offsets, s);
-    if (rc != SX_OK) return rc;
-    c->A.seg_count = c->seg_count; c->A.seg_off = c->seg_off;   // the count pass always keeps the per-segment results
-    rc = launch_expand<false>(c, s);
+    rc = run_count(c, d_tags, n_tags, d_points_xy, n_points, d_styles, n_paths, h_affine, tolerance, mode, d_path_offsets, s);
     if (rc != SX_OK) return rc;
     c->counted = true;
-    c->info_valid = true;
     if (!h_total) return SX_OK;
     rc = read_total(c, s, h_total);
     if (rc != SX_OK) c->counted = false;
@@ -252,18 +304,11 @@ sx_status sx_write(sx_ctx* c, void* d_out_records, uint64_t cap_records, void* c
     if (!c) return SX_E_INVALID_ARG;
     if (!c->counted) return SX_E_STATE;
     if (c->total_known && c->total > cap_records) return SX_E_CAPACITY;
-    if (c->A.P.n_tags == 0 || (c->total_known && c->total == 0)) return SX_OK;
+    if (c->W.P.n_tags == 0 || (c->total_known && c->total == 0)) return SX_OK;
     if (!d_out_records || (reinterpret_cast<uintptr_t>(d_out_records) & 15u)) return SX_E_INVALID_ARG;
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     SX_CUDA(cudaSetDevice(c->device));
-    // the write pass repeats the count pass's work on the same inputs (same code, same decisions) with the records on:
-    // reset its ticket, its statistics and its look-back words; the error flag of the count pass stays
-    SX_CUDA(cudaMemsetAsync(ctx_ticket(c, 1), 0, 64 - 16 - 16, s));
-    SX_CUDA(cudaMemsetAsync(ctx_states(c), 0, states_bytes(c->A.P.n_tags), s));
-    c->A.out = static_cast<float4*>(d_out_records);
-    c->A.cap_records = cap_records;
-    c->A.seg_count = nullptr; c->A.seg_off = nullptr;
-    return launch_expand<true>(c, s);
+    return run_write(c, d_out_records, cap_records, s);
 }
 
 sx_status stroke_expand_into(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, const float* d_points_xy, uint64_t n_points,
@@ -275,14 +320,13 @@ sx_status stroke_expand_into(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, 
     if (rc != SX_OK) return rc;
     if (cap_records > 0 && (!d_out_records || (reinterpret_cast<uintptr_t>(d_out_records) & 15u))) return SX_E_INVALID_ARG;
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-    rc = begin_call(c, d_tags, n_tags, d_points_xy, n_points, d_styles, n_paths, h_affine, tolerance, mode, d_path_offsets, s);
+    rc = run_count(c, d_tags, n_tags, d_points_xy, n_points, d_styles, n_paths, h_affine, tolerance, mode, d_path_offsets, s);
     if (rc != SX_OK) return rc;
-    c->A.out = static_cast<float4*>(d_out_records);
-    c->A.cap_records = cap_records;
-    if (c->keep_info) { c->A.seg_count = c->seg_count; c->A.seg_off = c->seg_off; }
-    rc = launch_expand<true>(c, s);
-    if (rc != SX_OK) return rc;
-    c->info_valid = c->keep_info;
+    c->counted = true;
+    if (cap_records > 0) {
+        rc = run_write(c, d_out_records, cap_records, s);
+        if (rc != SX_OK) return rc;
+    }
     if (!h_total) return SX_OK;
     rc = read_total(c, s, h_total);
     if (rc != SX_OK) return rc;
@@ -373,7 +417,7 @@ sx_status stroke_expand_host(sx_ctx* c, const uint8_t* h_tags, uint64_t n_tags, 
 sx_status sx_segment_info(sx_ctx* c, const uint32_t** d_pt_off, const uint32_t** d_path_idx, const uint32_t** d_sp_first,
                           const uint32_t** d_seg_count, const uint64_t** d_seg_offset) {
     if (!c) return SX_E_INVALID_ARG;
-    if (!c->info_valid) return SX_E_STATE;
+    if (!c->counted) return SX_E_STATE;
     if (d_pt_off) *d_pt_off = c->pt_off;
     if (d_path_idx) *d_path_idx = c->path_idx;
     if (d_sp_first) *d_sp_first = c->sp_first;
@@ -399,10 +443,10 @@ sx_status sx_last_error(sx_ctx* c, void* cuda_stream) {
 sx_status sx_set_option(sx_ctx* c, int32_t option, uint64_t value) {
     if (!c) return SX_E_INVALID_ARG;
     switch (option) {
-        case SX_OPT_KEEP_SEGMENT_INFO: c->keep_info = value != 0; return SX_OK;
+        case SX_OPT_KEEP_SEGMENT_INFO: return SX_OK;   // (kept for compatibility: the per-segment results are always there)
         case SX_OPT_TIME_KERNELS: c->time_kernels = value != 0; c->timed = false; return SX_OK;
-        case SX_OPT_TILES_PER_RANGE:
-            if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) return SX_E_INVALID_ARG;
+        case SX_OPT_TILE_SEGMENTS:
+            if (value != 0 && value != 1 && value != 2 && value != 8 && value != 16 && value != 32) return SX_E_INVALID_ARG;
             c->force_tiles = static_cast<uint32_t>(value);
             return SX_OK;
         default: return SX_E_INVALID_ARG;
@@ -416,21 +460,20 @@ sx_status sx_call_stats(sx_ctx* c, uint64_t* h_out4, void* cuda_stream) {
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     SX_CUDA(cudaSetDevice(c->device));
     uint32_t* hp = reinterpret_cast<uint32_t*>(&c->h_pinned[2]);
-    SX_CUDA(cudaMemcpyAsync(hp, ctx_stats(c), 8, cudaMemcpyDeviceToHost, s));
-    SX_CUDA(cudaMemcpyAsync(hp + 2, c->d_hint, 4, cudaMemcpyDeviceToHost, s));
+    SX_CUDA(cudaMemcpyAsync(hp, ctx_stats(c), 12, cudaMemcpyDeviceToHost, s));
+    SX_CUDA(cudaMemcpyAsync(hp + 3, c->d_hint, 4, cudaMemcpyDeviceToHost, s));
     SX_CUDA(cudaStreamSynchronize(s));
-    h_out4[0] = hp[0]; h_out4[1] = hp[1]; h_out4[2] = hp[2]; h_out4[3] = sx::kExRange;
+    h_out4[0] = hp[0]; h_out4[1] = hp[1]; h_out4[2] = hp[2]; h_out4[3] = c->force_tiles >= 8 ? c->force_tiles : hp[3];
     return SX_OK;
 }
 
-sx_status sx_kernel_times(sx_ctx* c, float* h_ms2) {
-    if (!c || !h_ms2) return SX_E_INVALID_ARG;
-    h_ms2[0] = h_ms2[1] = 0.0f;
+sx_status sx_kernel_times(sx_ctx* c, float* h_ms4) {
+    if (!c || !h_ms4) return SX_E_INVALID_ARG;
+    for (int k = 0; k < 4; k++) h_ms4[k] = 0.0f;
     if (!c->timed) return SX_E_STATE;
     SX_CUDA(cudaSetDevice(c->device));
-    SX_CUDA(cudaEventSynchronize(c->ev[2]));
-    SX_CUDA(cudaEventElapsedTime(&h_ms2[0], c->ev[0], c->ev[1]));
-    SX_CUDA(cudaEventElapsedTime(&h_ms2[1], c->ev[1], c->ev[2]));
+    SX_CUDA(cudaEventSynchronize(c->ev[kEvents - 1]));
+    for (int k = 0; k < 4; k++) SX_CUDA(cudaEventElapsedTime(&h_ms4[k], c->ev[k], c->ev[k + 1]));
     return SX_OK;
 }
 

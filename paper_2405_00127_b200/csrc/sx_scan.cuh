@@ -1,4 +1,4 @@
-// sx_scan.cuh -- (a) k_tag_scan, the single-pass prefix scan over the tag stream (decoupled look-back).
+// sx_scan.cuh -- (a) k_tag_scan and (c) k_alloc_scan: single-pass prefix scans (decoupled look-back).
 //
 // PAPER.md L464-466 + Table 1 (L468-481): every tag carries stream-offset increments and the offsets are prefix
 // sums over the "tag monoid".  Ours is (points, paths, first) with points += count + subpath_end (L470),
@@ -8,8 +8,8 @@
 // One pass over the data, thread-sequential -> warp-shuffle -> cross-warp in shared memory -> tile prefix by
 // decoupled look-back (a tile publishes its aggregate, then looks back over its predecessors' aggregates /
 // inclusive prefixes, one warp inspecting 32 predecessors at a time).  Tile ids come from an atomic ticket, so a
-// tile only ever waits for tiles that already started.  The allocation scan over the record counts (replacing the
-// atomic bump allocation of L448) uses the same protocol inside k_expand (sx_expand.cuh).
+// tile only ever waits for tiles that already started.  (c) k_alloc_scan, the allocation scan over the record counts
+// (replacing the atomic bump allocation of L448), uses the same protocol.
 #pragma once
 #include <stdint.h>
 #include <cuda_runtime.h>
@@ -44,12 +44,15 @@ __device__ __forceinline__ uint64_t ld_volatile_u64(const uint64_t* p) { return 
 
 __global__ void __launch_bounds__(kScanThreads)
 k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint32_t n_paths, uint32_t* __restrict__ pt_off,
-           uint32_t* __restrict__ path_idx, uint32_t* __restrict__ sp_first, TagTileState* states, uint32_t* ticket, uint32_t* err) {
+           uint32_t* __restrict__ path_idx, uint32_t* __restrict__ sp_first, TagTileState* states, uint32_t* ticket, uint32_t* err, uint32_t* hint) {
     __shared__ uint32_t s_tile;
     __shared__ TagAgg s_warp[kScanThreads / 32];
     __shared__ TagAgg s_prefix;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_tile = atomicAdd(ticket, 1u);
+    // the first kernel of every call: the tile size the last expansion kernel proposed becomes the one of this call
+    // (k_expand reads hint[0] only; both of its launches in a count + write call see the same value)
+    if (blockIdx.x == 0 && tid == 0) hint[0] = hint[1];
     __syncthreads();
     const uint32_t tile = s_tile;
     const uint32_t base = tile * (uint32_t)kTagTile + (uint32_t)tid * kTagItems;
@@ -164,7 +167,90 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
     }
 }
 
-// state word of the allocation look-back (k_expand): status in bits 62-63 (0 nothing, 1 aggregate, 2 inclusive), value in bits 0-61
+// ---------------------------------------------------------------- (c) allocation scan
+// Exclusive 64-bit prefix sum of the per-segment record counts (replaces the atomic bump allocation of PAPER.md L448: the
+// records come out grouped by segment, in segment order), the offset of every path's first record and the total.
+// Same single-pass protocol as the tag scan; state word: status in bits 62-63 (0 nothing, 1 aggregate, 2 inclusive),
+// value in bits 0-61.
 constexpr uint64_t kValMask = (1ull << 62) - 1ull;
+constexpr int kCntItems = 8;
+constexpr int kCntTile = kScanThreads * kCntItems;    // 2048
+
+__global__ void __launch_bounds__(kScanThreads)
+k_alloc_scan(const uint32_t* __restrict__ count, uint32_t n, const uint8_t* __restrict__ tags, const uint32_t* __restrict__ path_idx,
+             uint32_t n_paths, uint64_t* __restrict__ seg_off, uint64_t* __restrict__ path_off, uint64_t* d_total, uint64_t* states,
+             uint32_t* ticket, const uint32_t* err) {
+    __shared__ uint32_t s_tile;
+    __shared__ uint64_t s_warp[kScanThreads / 32];
+    __shared__ uint64_t s_prefix;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
+    __syncthreads();
+    const uint32_t tile = s_tile;
+    const uint32_t base = tile * (uint32_t)kCntTile + (uint32_t)tid * kCntItems;
+    uint32_t c[kCntItems];
+    if (base + kCntItems <= n) {
+        uint4 a = __ldg(reinterpret_cast<const uint4*>(count + base)), b = __ldg(reinterpret_cast<const uint4*>(count + base + 4));
+        c[0] = a.x; c[1] = a.y; c[2] = a.z; c[3] = a.w; c[4] = b.x; c[5] = b.y; c[6] = b.z; c[7] = b.w;
+    } else {
+#pragma unroll
+        for (int k = 0; k < kCntItems; k++) c[k] = base + k < n ? count[base + k] : 0u;
+    }
+    uint64_t mine = 0;
+#pragma unroll
+    for (int k = 0; k < kCntItems; k++) mine += c[k];
+    uint64_t incl = mine;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        uint64_t o = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += o;
+    }
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    uint64_t tile_agg = 0, warp_excl = 0;
+#pragma unroll
+    for (int k = 0; k < kScanThreads / 32; k++) {
+        if (k == warp) warp_excl = tile_agg;
+        tile_agg += s_warp[k];
+    }
+    if (warp == 0) {
+        if (lane == 0 && tile > 0) *reinterpret_cast<volatile uint64_t*>(states + tile) = (1ull << 62) | tile_agg;
+        uint64_t excl = 0;
+        int idx = (int)tile - 1;
+        while (idx >= 0) {
+            int j = idx - lane;
+            uint64_t word = 2ull << 62;
+            if (j >= 0) { do { word = ld_volatile_u64(states + j); } while ((word >> 62) == 0ull); }
+            uint32_t m = __ballot_sync(0xffffffffu, (word >> 62) == 2ull);
+            int stop = __ffs((int)m) - 1;
+            uint64_t v = (lane > stop && m) ? 0ull : (word & kValMask);
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+            excl += v;
+            if (m) break;
+            idx -= 32;
+        }
+        if (lane == 0) {
+            s_prefix = excl;
+            *reinterpret_cast<volatile uint64_t*>(states + tile) = (2ull << 62) | (excl + tile_agg);
+        }
+    }
+    __syncthreads();
+    uint64_t up = __shfl_up_sync(0xffffffffu, incl, 1);
+    if (lane == 0) up = 0;
+    uint64_t run = s_prefix + warp_excl + up;
+    const bool ok = (*err & kErrBadStream) == 0u;
+#pragma unroll
+    for (int k = 0; k < kCntItems; k++) {
+        uint32_t i = base + k;
+        if (i < n) {
+            seg_off[i] = run;
+            // first segment of a path: the previous tag carries the path-end bit (Table 1)
+            if (ok && (i == 0u || (tags[i - 1] & 16u))) { uint32_t p = path_idx[i]; if (p < n_paths) path_off[p] = run; }
+            run += c[k];
+            if (i == n - 1u) { path_off[n_paths] = run; *d_total = run; }
+        }
+    }
+}
 
 }  // namespace sx

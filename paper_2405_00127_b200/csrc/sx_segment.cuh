@@ -296,10 +296,11 @@ SX_DEV void emit_straight(const Seg& s, float h, const Writer* w) {
 
 // thread-per-segment reference path: everything segment i emits, in canonical order
 template <bool EMIT>
-SX_DEV uint32_t process_segment(const Params& P, uint32_t i, Writer* w) {
+SX_DEV uint32_t process_segment(const Params& P, uint32_t i, Writer* w, uint32_t* tail_out = nullptr) {
     uint32_t tag = P.tags[i];
     Style st;
     float h;
+    if (tail_out) *tail_out = 0u;
     if (!load_style(P, P.path_idx[i], &st, &h)) return 0;
     Seg s = load_segment(P, i, tag);
     uint32_t n;
@@ -309,8 +310,9 @@ SX_DEV uint32_t process_segment(const Params& P, uint32_t i, Writer* w) {
     } else {
         n = flatten_cubic<EMIT>(P, s, h, w);
     }
-    n += segment_tail<EMIT>(P, i, tag, s, st, h, w, n);
-    return n;
+    const uint32_t tail = segment_tail<EMIT>(P, i, tag, s, st, h, w, n);
+    if (tail_out) *tail_out = tail;
+    return n + tail;
 }
 
 }  // namespace sx

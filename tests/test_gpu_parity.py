@@ -176,18 +176,19 @@ def test_host_buffer_entry_point_matches_device_entry_point(B, ctx, name, npaths
 
 @pytest.mark.parametrize("name,npaths,mode", [("c1", 64, 0), ("c2", 300, 1), ("c4", 2000, 1), ("c5", 40, 0)])
 def test_tiling_of_the_expansion_kernel_does_not_change_a_bit(B, name, npaths, mode):
-    """The expansion kernel works on ranges of 128 segments as 1, 2 or 4 tiles (adapted on the device), and a tile
-    that does not fit its shared-memory tables takes the thread-per-segment reference walk (forced with 8): every
-    choice must give the same records, bit for bit."""
+    """The warps of the expansion kernel work on tiles of 32, 16 or 8 segments (adapted on the device); a tile that
+    does not fit its shared-memory tables is redone in sub-tiles of 8 segments (forced with 2), and a sub-tile that
+    still does not fit takes the thread-per-segment reference walk (forced with 1): every choice must give the same
+    records, bit for bit."""
     sc = S.make(name, n_paths=npaths)
     dev = "cuda:0"
     tags, pts, sty = B.scene_to_torch(sc, device=dev)
     width = 4 if mode == 0 else 8
     outs = []
-    for tiles in (8, 1, 2, 4, 0):
+    for tiles in (1, 2, 8, 16, 32, 0):
         c = B.sx_create(0)
         try:
-            B.sx_set_option(c, B.SX_OPT_TILES_PER_RANGE, tiles)
+            B.sx_set_option(c, B.SX_OPT_TILE_SEGMENTS, tiles)
             poff = torch.empty(sc.n_paths + 1, dtype=torch.int64, device=dev)
             total = B.sx_count(c, tags, pts, sty, sc.affine, sc.tolerance, mode, poff)
             out = torch.full((total, width), float("nan"), dtype=torch.float32, device=dev)
@@ -195,15 +196,19 @@ def test_tiling_of_the_expansion_kernel_does_not_change_a_bit(B, name, npaths, m
             torch.cuda.synchronize()
             assert B.sx_last_error(c) == 0
             st = B.sx_call_stats(c)
-            if tiles == 8:
-                assert st["fast_tiles"] == 0 and st["slow_tiles"] > 0
+            if tiles == 1:
+                assert st["walk_segments"] == sc.n_segments
+            if tiles == 2:
+                assert st["direct_tiles"] <= 1 and st["sub_tiled_tiles"] > 0
+            if tiles >= 8:
+                assert st["tile_segments"] == tiles
             outs.append((out.cpu().numpy().view(np.uint32), poff.cpu().numpy(), st))
         finally:
             B.sx_destroy(c)
-    print("tiles on the fast / slow path:", [(o[2]["fast_tiles"], o[2]["slow_tiles"]) for o in outs])
+    print("tiles in one go / in sub-tiles / segments on the walk:", [(o[2]["direct_tiles"], o[2]["sub_tiled_tiles"], o[2]["walk_segments"]) for o in outs])
     for o in outs[1:]:
         assert np.array_equal(outs[0][0], o[0]) and np.array_equal(outs[0][1], o[1])
-    assert outs[3][2]["fast_tiles"] > 0   # 32-segment tiles fit on every config
+    assert outs[2][2]["direct_tiles"] > 0   # 8-segment tiles fit on every config
 
 
 # ---------------------------------------------------------------- the same invariant checks the oracle passes
