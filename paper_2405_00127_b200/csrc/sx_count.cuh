@@ -11,7 +11,7 @@
 //                  visits -- a rejected node evaluates its mid point once and pushes its two children, an accepted
 //                  node becomes a LEAF (one Euler-spiral piece).  The bisection tree is kept (parent links).  Queue
 //                  positions come from warp ballots: no atomics.
-//   C  pieces      lane pair per leaf: end-tangent angles (reading R-17), App. A parameters (L628-653), and per side
+//   C  pieces      lane per leaf: end-tangent angles (reading R-17), App. A parameters (L628-653), and per side
 //                  the cusp split (L380-386) and the subdivision counts (sections 4, 5, 6).
 //   D  counts      subtree sums over the bisection tree give every leaf the number of records that precede it in
 //                  its segment (canonical order = increasing t) and every segment its count.
@@ -95,11 +95,11 @@ struct __align__(16) CtSeg {
     uint32_t pad;
 };
 struct CtLeaf {
-    uint32_t ab;         // point indices a | b << 16 (phases B, C); class rank | simple << 31 (phase D)
+    uint32_t ab;         // point indices a | b << 16 (phases B, C); rank within the class | class << 30 (phase D)
     uint32_t seg_slot;   // segment (tile-local) | tree slot << 8
     uint32_t key;
     float k0, k1, L;
-    uint32_t n;          // n_minus | n_plus << 16
+    uint16_t n[2];       // n_minus, n_plus
 };
 struct CtWarp {
     CtSeg seg[kCtTile];
@@ -139,6 +139,49 @@ SX_DEV uint32_t count_tail(const CtWarp& S, const Params& P, uint32_t s0, uint32
 
 // the thread-per-segment walk of a sub-tile that does not fit the tables: out of line (rarely executed, large)
 __device__ __noinline__ uint32_t slow_count(const Params& P, uint32_t i, uint32_t* tail) { return process_segment<false>(P, i, nullptr, tail); }
+
+// One leaf of the bisection, straight-line: the end-tangent angles of the accepted piece (L211-213: th0 from the start
+// tangent to the chord, th1 from the chord to the end tangent; reading R-17; a zero chord is accepted at the deepest level
+// only: th0 = th1 = atan2(0, 1) = 0, as in fit_error), the App. A parameters, and per side either the count of the one
+// offset range of a side that is regular throughout -- decided from approximate cusp factors 1 - kappa eta at both ends,
+// positive by a wide margin, so that side_plan's own exactly rounded ones have the same signs; the count is offset_plan's,
+// the call the writers repeat -- or the request for the full plan.
+struct LeafEval { float k0, k1, L; uint32_t n[2]; bool full[2]; };
+// (one copy of each: the count pass's working set has to stay inside the instruction cache -- 16 unsynchronised warps per SM)
+__device__ __noinline__ float atan2_r_core_call(float y, float x) { return atan2_r_core(y, x); }
+__device__ __noinline__ uint32_t offset_count(float k0, float k1, float L, float eta, int mode, float tol_fl) {
+    Piece p;
+    p.k0 = k0; p.k1 = k1; p.L = L;
+    return (uint32_t)offset_plan(p, eta, 0.0f, 1.0f, mode, tol_fl).n;
+}
+SX_DEV LeafEval leaf_eval(float4 pa, float4 pb, float h, int mode, float tol_fl) {
+    LeafEval e;
+    const V2 ch = v2(pb.x, pb.y) - v2(pa.x, pa.y);
+    const float chord2 = len2(ch), chord = sqrtf(chord2);
+    const V2 uc = v2(ch.x / chord, ch.y / chord);
+    const bool flat = !(chord2 >= kEpsQ2);
+    float th[2];
+#pragma unroll 1
+    for (int k = 0; k < 2; k++) {
+        const V2 f0 = k ? uc : v2(pa.z, pa.w), f1 = k ? v2(pb.z, pb.w) : uc;
+        th[k] = atan2_r_core_call(flat ? 0.0f : cross(f0, f1), flat ? 1.0f : dot(f0, f1));
+    }
+    Piece p;
+    piece_params(p, th[0], th[1], chord);
+    e.k0 = p.k0; e.k1 = p.k1; e.L = p.L;
+    const float il = rcp_fast(p.L), ka = (p.k0 - 0.5f * p.k1) * il, kb = (p.k0 + 0.5f * p.k1) * il;
+    // (arc mode: the count of a regular side does not depend on the sign of eta -- "same arc approximation ... both sides", L181)
+    const uint32_t n_arc = mode == kModeArc ? offset_count(p.k0, p.k1, p.L, h, kModeArc, tol_fl) : 0u;
+#pragma unroll 1
+    for (int side = 0; side < 2; side++) {
+        const float eta = side ? h : -h;
+        e.full[side] = !(fmaf(-ka, eta, 1.0f) > 1e-3f && fmaf(-kb, eta, 1.0f) > 1e-3f);
+        e.n[side] = n_arc;
+        if (mode != kModeArc && !e.full[side]) e.n[side] = offset_count(p.k0, p.k1, p.L, eta, kModeLine, tol_fl);
+        if (e.full[side]) e.n[side] = 0xffffu;   // (not simple until the full plan says so)
+    }
+    return e;
+}
 
 // ---------------------------------------------------------------- the kernel
 __global__ void __launch_bounds__(32, kCtWarpsPerSM)
@@ -248,10 +291,8 @@ k_count(const CountArgs A) {
                 if (__any_sync(kFull, bad) || n_leaf + n_acc > (uint32_t)kCtLeafCap || n_split + n_push > (uint32_t)kCtSplitCap ||
                     q_tail + 2u * n_push - q_head > (uint32_t)kCtQueueCap) { overflow = true; break; }
                 if (accept) {
-                    CtLeaf lf;
+                    CtLeaf& lf = S.leaf[n_leaf + __popc(m_acc & lt)];
                     lf.ab = qy; lf.seg_slot = qz; lf.key = (qx & 0xffffu) | ((qx >> 20) << 16);
-                    lf.k0 = lf.k1 = lf.L = 0.0f; lf.n = 0;
-                    S.leaf[n_leaf + __popc(m_acc & lt)] = lf;
                 }
                 if (push) {
                     // children: one point, two tree slots, two queue entries per split
@@ -273,54 +314,61 @@ k_count(const CountArgs A) {
             }
             __syncwarp();
 
-            // ================================================================ C: pieces (lane pair per leaf)
-            uint32_t n_simple = 0, n_other = 0;
+            // ================================================================ C: pieces (lane per leaf)
+            uint32_t n_triv = 0, n_multi = 0, n_other = 0;
             if (!overflow) {
-                const int side = lane & 1;
-                for (uint32_t l0 = 0; l0 < n_leaf; l0 += 16u) {
-                    const uint32_t li = l0 + (uint32_t)(lane >> 1);
+                // C1, lane per leaf: angles, App. A parameters, and the counts of the sides that are regular throughout by a wide
+                // margin (the usual case)
+                uint16_t* const full_list = reinterpret_cast<uint16_t*>(S.qx);   // (the queue is dead: qx, qy = 512 entries)
+                uint32_t n_full = 0;
+                for (uint32_t l0 = 0; l0 < n_leaf; l0 += 32u) {
+                    const uint32_t li = l0 + (uint32_t)lane;
                     const bool live = li < n_leaf;
-                    CtLeaf lf;
-                    lf.ab = 0; lf.seg_slot = 0; lf.key = 0; lf.k0 = lf.k1 = lf.L = 0.0f; lf.n = 0;
-                    if (live) lf = S.leaf[li];
-                    const uint32_t a = lf.ab & 0xffffu, b = lf.ab >> 16, sl = lf.seg_slot & 0xffu, slot = lf.seg_slot >> 8;
-                    const float4 pa = S.pts[a], pb = S.pts[b];
-                    const V2 ch = v2(pb.x, pb.y) - v2(pa.x, pa.y);
-                    const float chord2 = len2(ch), chord = sqrtf(chord2);
-                    // the lane's angle: th0 (side 0) from the start tangent to the chord, th1 (side 1) from the chord to the end
-                    // tangent; ONE call for both kinds of lane (a zero chord is accepted at the deepest level only:
-                    // th0 = th1 = atan2(0, 1) = 0, as in fit_error)
-                    float ay = 0.0f, ax = 1.0f;
-                    if (live && chord2 >= kEpsQ2) {
-                        const V2 uc = v2(ch.x / chord, ch.y / chord);
-                        const V2 ut = side ? v2(pb.z, pb.w) : v2(pa.z, pa.w);
-                        const V2 f0 = side ? uc : ut, f1 = side ? ut : uc;
-                        ay = cross(f0, f1); ax = dot(f0, f1);
-                    }
-                    const float th = atan2_r(ay, ax);
-                    const float tho = __shfl_xor_sync(kFull, th, 1);
-                    Piece p;
-                    piece_params(p, side ? tho : th, side ? th : tho, chord);
-                    const float h = S.seg[sl].h;
-                    uint32_t n = 0;
-                    bool simple = false;
+                    const uint32_t lab = live ? S.leaf[li].ab : 0u, sl = live ? (S.leaf[li].seg_slot & 0xffu) : 0u;
+                    const LeafEval ev = leaf_eval(S.pts[lab & 0xffffu], S.pts[lab >> 16], S.seg[sl].h, P.mode, P.tol_fl);
+                    const bool f0 = live && ev.full[0], f1 = live && ev.full[1];
+                    const uint32_t m0 = __ballot_sync(kFull, f0), m1 = __ballot_sync(kFull, f1);
                     if (live) {
-                        const SidePlan sp = side_plan(p, side ? h : -h, P.mode, P.tol_fl);
-                        n = (uint32_t)sp.total;
-                        simple = sp.nr == 1 && !sp.sup[0] && n <= (uint32_t)kDirectMax;
+                        CtLeaf& lf = S.leaf[li];
+                        lf.k0 = ev.k0; lf.k1 = ev.k1; lf.L = ev.L;
+                        lf.n[0] = (uint16_t)ev.n[0]; lf.n[1] = (uint16_t)ev.n[1];
+                        lf.ab = (ev.n[0] <= (uint32_t)kDirectMax ? 1u : 0u) | (ev.n[1] <= (uint32_t)kDirectMax ? 0x100u : 0u);   // simple flags of the two sides (bytes 0, 1)
                     }
-                    const uint32_t no = __shfl_xor_sync(kFull, n, 1);
-                    const bool so = __shfl_xor_sync(kFull, simple ? 1 : 0, 1) != 0;
-                    const bool owner = live && side == 0;
-                    const bool too_long = owner && (n > 0xffffu || no > 0xffffu);   // a side of more than 65535 records: the walk
-                    const bool both = owner && simple && so;
-                    const uint32_t m_both = __ballot_sync(kFull, both), m_other = __ballot_sync(kFull, owner && !both);
-                    if (owner) {
-                        lf.k0 = p.k0; lf.k1 = p.k1; lf.L = p.L;
-                        lf.n = (n & 0xffffu) | (no << 16);
-                        // rank within its class (the leaf buffer takes simple leaves from the front, the others from the back)
-                        lf.ab = both ? ((n_simple + __popc(m_both & lt)) | 0x80000000u) : (n_other + __popc(m_other & lt));
-                        S.leaf[li] = lf;
+                    if (f0) full_list[n_full + __popc(m0 & lt)] = (uint16_t)(2u * li);
+                    n_full += __popc(m0);
+                    if (f1) full_list[n_full + __popc(m1 & lt)] = (uint16_t)(2u * li + 1u);
+                    n_full += __popc(m1);
+                }
+                __syncwarp();
+                // C2, lane per side that has a cusp or a super-critical range: the full plan (cusp split L380-386, evolute L195)
+                bool too_long = false;
+                for (uint32_t e0 = 0; e0 < n_full; e0 += 32u) {
+                    if (e0 + (uint32_t)lane < n_full) {
+                        const uint32_t e = full_list[e0 + (uint32_t)lane], l = e >> 1, side = e & 1u;
+                        CtLeaf& lf = S.leaf[l];
+                        Piece p;
+                        p.k0 = lf.k0; p.k1 = lf.k1; p.L = lf.L;
+                        const float h = S.seg[lf.seg_slot & 0xffu].h;
+                        const SidePlan sp = side_plan(p, side ? h : -h, P.mode, P.tol_fl);
+                        too_long |= (uint32_t)sp.total > 0xffffu;   // a side of more than 65535 records: the walk
+                        lf.n[side] = (uint16_t)sp.total;
+                        reinterpret_cast<uint8_t*>(&lf.ab)[side] = (sp.nr == 1 && !sp.sup[0] && sp.total <= kDirectMax) ? 1 : 0;
+                    }
+                }
+                __syncwarp();
+                if (__any_sync(kFull, too_long)) overflow = true;
+                // C3, lane per leaf: class, rank within the class, subtree sums
+                for (uint32_t l0 = 0; l0 < n_leaf; l0 += 32u) {
+                    const uint32_t l = l0 + (uint32_t)lane;
+                    const bool live = l < n_leaf;
+                    uint32_t n = 0, no = 0, fl = 0, slot = 0;
+                    if (live) { const CtLeaf& lf = S.leaf[l]; n = lf.n[0]; no = lf.n[1]; fl = lf.ab; slot = lf.seg_slot >> 8; }
+                    // classes: 1 both sides one record (the simple writer's straight path), 2 both sides simple, 0 the others
+                    const bool both = live && (fl & 0x101u) == 0x101u;
+                    const bool triv = both && n == 1u && no == 1u;
+                    const uint32_t m_triv = __ballot_sync(kFull, triv), m_multi = __ballot_sync(kFull, both && !triv), m_other = __ballot_sync(kFull, live && !both);
+                    if (live) {
+                        S.leaf[l].ab = triv ? ((n_triv + __popc(m_triv & lt)) | 0x40000000u) : (both ? ((n_multi + __popc(m_multi & lt)) | 0x80000000u) : (n_other + __popc(m_other & lt)));
                         // subtree sums: the leaf's records are added to itself and to all its ancestors
                         const uint32_t c = n + no;
                         uint32_t cur = slot;
@@ -330,8 +378,7 @@ k_count(const CountArgs A) {
                             cur = S.parent[cur];
                         }
                     }
-                    n_simple += __popc(m_both); n_other += __popc(m_other);
-                    if (__any_sync(kFull, too_long)) overflow = true;
+                    n_triv += __popc(m_triv); n_multi += __popc(m_multi); n_other += __popc(m_other);
                 }
             }
             __syncwarp();
@@ -342,6 +389,7 @@ k_count(const CountArgs A) {
 
             // ================================================================ D: counts, leaf records
             bool walk = overflow;
+            const uint32_t n_simple = n_triv + n_multi;
             if (!walk && n_leaf) {
                 // room in the leaf buffer for the (sub-)tile: one atomic for both ends
                 unsigned long long got = 0;
@@ -364,10 +412,12 @@ k_count(const CountArgs A) {
                         }
                         const uint32_t sl = lf.seg_slot & 0xffu;
                         LeafRec r;
-                        r.seg = s0 + sl; r.key = lf.key; r.n = lf.n; r.rel = rel;
+                        r.seg = s0 + sl; r.key = lf.key; r.n = (uint32_t)lf.n[0] | ((uint32_t)lf.n[1] << 16); r.rel = rel;
                         r.k0 = lf.k0; r.k1 = lf.k1; r.L = lf.L; r.h = S.seg[sl].h;
-                        const uint32_t rank = lf.ab & 0x7fffffffu;
-                        const uint32_t pos = (lf.ab >> 31) ? base_simple + rank : A.leaf_cap - 1u - (base_other + rank);
+                        // the tile's simple leaves: the one-record ones from the front of its block, the others from its back,
+                        // so that the warps of the simple writer see (mostly) one kind
+                        const uint32_t rank = lf.ab & 0x3fffffffu, cls = lf.ab >> 30;
+                        const uint32_t pos = cls == 1u ? base_simple + rank : (cls == 2u ? base_simple + n_simple - 1u - rank : A.leaf_cap - 1u - (base_other + rank));
                         uint4* dst = reinterpret_cast<uint4*>(A.leaves + pos);
                         dst[0] = make_uint4(r.seg, r.key, r.n, r.rel);
                         dst[1] = make_uint4(__float_as_uint(r.k0), __float_as_uint(r.k1), __float_as_uint(r.L), __float_as_uint(r.h));

@@ -26,6 +26,7 @@ static thread_local cudaError_t g_last_cuda = cudaSuccess;
         if (e_ != cudaSuccess) { g_last_cuda = e_; return SX_E_CUDA; } \
     } while (0)
 
+constexpr int kSideStreams = 3;
 constexpr int kEvents = 5;   // SX_OPT_TIME_KERNELS: before the tag scan, after it, after the count, after the allocation scan, after the writers
 
 struct sx_ctx {
@@ -45,6 +46,8 @@ struct sx_ctx {
     int count_blocks, simple_blocks, general_blocks;   // persistent grids: resident blocks on the device
     cudaEvent_t ev[kEvents];
     bool time_kernels, timed;
+    cudaStream_t side[kSideStreams];   // the writers are independent of one another: three of them run beside the caller's stream
+    cudaEvent_t fork, join[kSideStreams];
     // options
     uint32_t force_tiles; // SX_OPT_TILE_SEGMENTS
     // last sx_count / stroke_expand_into
@@ -201,10 +204,18 @@ static sx_status run_write(sx_ctx* c, void* d_out_records, uint64_t cap_records,
     if (n == 0) return SX_OK;
     c->W.out = static_cast<float4*>(d_out_records);
     c->W.cap_records = cap_records;
-    sx::k_write_segments<<<(n + sx::kWrThreads - 1) / sx::kWrThreads, sx::kWrThreads, 0, s>>>(c->W);
-    sx::k_write_simple<<<c->simple_blocks, sx::kWrThreads, 0, s>>>(c->W);
+    // the four writers side by side: the general writer (the long one on evolute-heavy scenes) on the caller's stream, the
+    // others on the context's side streams, forked from and joined to the caller's stream with events
+    SX_CUDA(cudaEventRecord(c->fork, s));
+    for (int k = 0; k < kSideStreams; k++) SX_CUDA(cudaStreamWaitEvent(c->side[k], c->fork, 0));
     sx::k_write_general<<<c->general_blocks, sx::kWrThreads, 0, s>>>(c->W);
-    sx::k_write_walk<<<c->sm_count, sx::kWrThreads, 0, s>>>(c->W);
+    sx::k_write_simple<<<c->simple_blocks, sx::kWrThreads, 0, c->side[0]>>>(c->W);
+    sx::k_write_segments<<<(n + sx::kWrThreads - 1) / sx::kWrThreads, sx::kWrThreads, 0, c->side[1]>>>(c->W);
+    sx::k_write_walk<<<c->sm_count, sx::kWrThreads, 0, c->side[2]>>>(c->W);
+    for (int k = 0; k < kSideStreams; k++) {
+        SX_CUDA(cudaEventRecord(c->join[k], c->side[k]));
+        SX_CUDA(cudaStreamWaitEvent(s, c->join[k], 0));
+    }
     c->launches += 4;
     if (c->time_kernels) { SX_CUDA(cudaEventRecord(c->ev[4], s)); c->timed = true; }
     SX_CUDA(cudaGetLastError());
@@ -261,6 +272,11 @@ sx_status sx_create(sx_ctx** out, int32_t device) {
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sx::k_write_general, sx::kWrThreads, 0);
     c->general_blocks = c->sm_count * (per_sm > 0 ? per_sm : 1);
     for (int k = 0; k < kEvents && e == cudaSuccess; k++) e = cudaEventCreate(&c->ev[k]);
+    for (int k = 0; k < kSideStreams && e == cudaSuccess; k++) {
+        e = cudaStreamCreateWithFlags(&c->side[k], cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->join[k], cudaEventDisableTiming);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->fork, cudaEventDisableTiming);
     if (e != cudaSuccess) { g_last_cuda = e; cudaFree(c->d_hint); cudaFreeHost(c->h_pinned); free(c); return SX_E_CUDA; }
     *out = c;
     return SX_OK;
@@ -271,6 +287,8 @@ sx_status sx_destroy(sx_ctx* c) {
     cudaSetDevice(c->device);
     cudaDeviceSynchronize();
     for (int k = 0; k < kEvents; k++) cudaEventDestroy(c->ev[k]);
+    for (int k = 0; k < kSideStreams; k++) { cudaStreamDestroy(c->side[k]); cudaEventDestroy(c->join[k]); }
+    cudaEventDestroy(c->fork);
     cudaFree(c->pt_off);
     cudaFree(c->leaves);
     cudaFree(c->sync_area);

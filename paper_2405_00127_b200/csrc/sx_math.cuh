@@ -101,43 +101,29 @@ SX_DEV V2 pick_tangent(V2 a, V2 b, V2 c, bool* degenerate) {
 
 SX_DEV float2 ldg2(const float* p) { return __ldg(reinterpret_cast<const float2*>(p)); }
 
-// pt = index of the segment's first point (pt_off[i] from the tag scan)
+// pt = index of the segment's first point (pt_off[i] from the tag scan).  Branch-free: the three kinds (line, quadratic,
+// cubic) differ in selects only, so that a warp over a mixed tile stays converged (and the code stays small).
 SX_DEV Seg load_segment_at(const Params& P, uint32_t pt, uint32_t tag) {
     Seg s;
-    int cnt = tag & 3;
+    const int cnt = tag & 3;
+    const bool quad = cnt == 2, cubic = cnt == 3;
     const float* p = P.pts + 2 * (uint64_t)pt;
-    auto a0 = ldg2(p), a1 = ldg2(p + 2);
-    V2 q0 = xform(P.A, a0.x, a0.y), q1 = xform(P.A, a1.x, a1.y);
+    const float2 a0 = ldg2(p), a1 = ldg2(p + 2), a2 = ldg2(p + (cnt >= 2 ? 4 : 2)), a3 = ldg2(p + (cubic ? 6 : (quad ? 4 : 2)));
+    const V2 q0 = xform(P.A, a0.x, a0.y), q1 = xform(P.A, a1.x, a1.y), q2 = xform(P.A, a2.x, a2.y), q3 = xform(P.A, a3.x, a3.y);
     s.kind = cnt;
-    s.P0 = q0;
+    s.P0 = q0; s.P3 = q3;   // (q3 repeats the last point of a line or a quadratic)
+    const V2 a = q1 - q0, b = q2 - q0, d = q3 - q0;
+    // degree elevation (L349).  line: c1 = d / 3, c2 = 2/3 d; quadratic: c1 = 2/3 a, c2 = b + 2/3 (a - b); cubic: as given
+    const V2 c1l = v2(a.x / 3.0f, a.y / 3.0f), c2l = v2(a.x * (2.0f / 3.0f), a.y * (2.0f / 3.0f));
+    const V2 c2q = v2(b.x + (a.x - b.x) * (2.0f / 3.0f), b.y + (a.y - b.y) * (2.0f / 3.0f));
+    s.c1 = cubic ? a : (quad ? c2l : c1l);
+    s.c2 = cubic ? b : (quad ? c2q : c2l);
+    s.c3 = d;
+    // the legs the limit tangents are picked from (R-5).  line: d, d, d both ways; quadratic: a, b, b / b - a, b, b;
+    // cubic: c1, c2, c3 / c3 - c2, c3 - c1, c3
     bool dg, dg2;
-    if (cnt == 1) {
-        s.P3 = q1;
-        V2 d = q1 - q0;
-        s.c3 = d;
-        s.c1 = v2(d.x / 3.0f, d.y / 3.0f);
-        s.c2 = v2(d.x * (2.0f / 3.0f), d.y * (2.0f / 3.0f));
-        s.ts = s.te = pick_tangent(d, d, d, &dg);
-    } else if (cnt == 2) {
-        auto a2 = ldg2(p + 4);
-        V2 q2 = xform(P.A, a2.x, a2.y);
-        s.P3 = q2;
-        V2 a = q1 - q0, b = q2 - q0;
-        s.c1 = v2(a.x * (2.0f / 3.0f), a.y * (2.0f / 3.0f));
-        s.c2 = v2(b.x + (a.x - b.x) * (2.0f / 3.0f), b.y + (a.y - b.y) * (2.0f / 3.0f));
-        s.c3 = b;
-        s.ts = pick_tangent(a, b, b, &dg);
-        s.te = pick_tangent(b - a, b, b, &dg2);
-    } else {
-        auto a2 = ldg2(p + 4), a3 = ldg2(p + 6);
-        V2 q2 = xform(P.A, a2.x, a2.y), q3 = xform(P.A, a3.x, a3.y);
-        s.P3 = q3;
-        s.c1 = q1 - q0;
-        s.c2 = q2 - q0;
-        s.c3 = q3 - q0;
-        s.ts = pick_tangent(s.c1, s.c2, s.c3, &dg);
-        s.te = pick_tangent(s.c3 - s.c2, s.c3 - s.c1, s.c3, &dg2);
-    }
+    s.ts = pick_tangent(a, b, d, &dg);
+    s.te = pick_tangent(cubic ? d - b : (quad ? b - a : d), cubic ? d - a : d, d, &dg2);
     s.degenerate = dg;
     return s;
 }
@@ -196,18 +182,64 @@ SX_DEV void eval_cubic(const Seg& s, float t, float dt, V2* pos, float* qmag, V2
 // L215 unit-chord normalisation; L217 d-bar; L221 e1; L225 area; L227 e2; L229 e3; guards R-4.
 //
 // Angles (reading R-17): th = the fp32 value nearest to the angle of (x, y): atan2 in double, rounded once.  The
-// oracle computes the same number with its own libm; the two agree unless the double result falls within an
+// oracle computes the same number with its own libm; the two agree unless the double result falls within a few
 // ulp(double) of a rounding boundary of fp32 (probability ~1e-8 per call).  th0, th1 fix k0, k1, L and hence every
 // subdivision parameter and every evolute radius of the piece.
-__device__ __noinline__ float atan2_r(float y, float x) { return (float)atan2((double)y, (double)x); }
+//
+// Own double-precision atan2 (the library's costs ~140 instructions per call, two calls per piece): with
+// mn = min(|x|, |y|), mx = max(|x|, |y|) and c = k/4 the quarter nearest to mn/mx,
+//     atan(mn/mx) = atan(c) + atan(t),  t = (mn - c mx) / (mx + c mn),  |t| <= 0.125 (+ the rounding of k),
+// one division (reciprocal seed from the fp32 unit, two Newton steps, one residual correction: full double accuracy)
+// and the Taylor series of atan to t^19 (remainder < 2^-63 / 21): error below 2 ulp(double) in all.
+SX_DEV float rcp_fast(float a) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
+SX_DEV float rsqrt_fast(float a) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
+
+// (x, y) finite and not both zero
+SX_DEV float atan2_r_core(float y, float x) {
+    const float ax = fabsf(x), ay = fabsf(y);
+    const float mxf = fmaxf(ax, ay), mnf = fminf(ax, ay);
+    const float kf = rintf(4.0f * mnf * rcp_fast(mxf));   // 0 .. 4
+    const double c = 0.25 * (double)kf;
+    // atan(k / 4), k = 0 .. 4
+    const double at = kf < 0.5f ? 0.0 : (kf < 1.5f ? 0.24497866312686415417 : (kf < 2.5f ? 0.46364760900080611621 : (kf < 3.5f ? 0.64350110879328438680 : 0.78539816339744830962)));
+    const double mx = (double)mxf, mn = (double)mnf;
+    const double num = fma(-c, mx, mn), den = fma(c, mn, mx);   // den in [mx, 2 mx]
+    double r = (double)rcp_fast((float)den);
+    r = fma(r, fma(-den, r, 1.0), r);
+    r = fma(r, fma(-den, r, 1.0), r);
+    double t = num * r;
+    t = fma(r, fma(-den, t, num), t);
+    const double z = t * t;
+    double p = -1.0 / 19.0;
+    p = fma(p, z, 1.0 / 17.0);
+    p = fma(p, z, -1.0 / 15.0);
+    p = fma(p, z, 1.0 / 13.0);
+    p = fma(p, z, -1.0 / 11.0);
+    p = fma(p, z, 1.0 / 9.0);
+    p = fma(p, z, -1.0 / 7.0);
+    p = fma(p, z, 1.0 / 5.0);
+    p = fma(p, z, -1.0 / 3.0);
+    double a = at + fma(t * z, p, t);
+    if (ay > ax) a = 1.57079632679489661923 - a;
+    if (x < 0.0f) a = 3.14159265358979323846 - a;
+    const float f = (float)a;
+    return y < 0.0f ? -f : f;
+}
+// (one out-of-line copy for the call sites that are not hot; the count pass inlines its two calls per piece so that the
+// two dependent chains interleave)
+__device__ __noinline__ float atan2_r(float y, float x) {
+    const float m = fmaxf(fabsf(x), fabsf(y));
+    if (!(m > 0.0f) || !(m < INFINITY)) return (float)atan2((double)y, (double)x);   // zeros, infinities, NaN: the library's rules
+    return atan2_r_core(y, x);
+}
 
 // atan2 for the accept/split DECISION of Alg. 2 only (the error estimate of section 7.1 is compared with a tolerance):
-// IEEE division, odd minimax polynomial on [0, 1] (max error ~1e-7 rad).  The angles a piece is built from come
-// from atan2_r.
+// approximate division, odd minimax polynomial on [0, 1] (max error ~1e-7 rad).  The angles a piece is built from come
+// from atan2_r.  (x, y) is (cos, sin) of an angle: max(|x|, |y|) >= 0.7.
 SX_DEV float atan2_dec(float y, float x) {
     const float ax = fabsf(x), ay = fabsf(y);
     const float mx = fmaxf(ax, ay), mn = fminf(ax, ay);
-    const float a = mx > 0.0f ? mn / mx : 0.0f;
+    const float a = mn * rcp_fast(fmaxf(mx, 1e-30f));
     const float s = a * a;
     float r = fmaf(s, 0.00282363896258175373077393f, -0.0159569028764963150024414f);
     r = fmaf(r, s, 0.0425049886107444763183594f);
@@ -222,28 +254,29 @@ SX_DEV float atan2_dec(float y, float x) {
     return y < 0.0f ? -r : r;
 }
 
-// section 7.1 with the decision-grade angles: the estimated error of the node (u0, q0mag) -> (u1, q1mag) over chord ch
+// section 7.1 with the decision-grade angles: the estimated error of the node (u0, q0mag) -> (u1, q1mag) over chord ch.
+// Everything here feeds one comparison with the tolerance: MUFU-grade reciprocals and square roots, explicit fused
+// multiply-adds, area(d0, d1) - area(db0, db1) expanded term by term (L225-227).
 SX_DEV float node_error(V2 u0, V2 u1, float q0mag, float q1mag, V2 ch, float dt) {
-    const float chord2 = len2(ch);
-    const float chord = sqrtf(chord2);
+    const float chord2 = fmaf(ch.x, ch.x, ch.y * ch.y);
     if (chord2 < kEpsQ2) return INFINITY;
-    const V2 uc = v2(ch.x / chord, ch.y / chord);
-    const float s0 = cross(u0, uc), c0 = dot(u0, uc);
-    const float s1 = cross(uc, u1), c1 = dot(uc, u1);
+    const float rc = rsqrt_fast(chord2), chord = chord2 * rc;
+    const float ucx = ch.x * rc, ucy = ch.y * rc;
+    const float s0 = fmaf(u0.x, ucy, -(u0.y * ucx)), c0 = fmaf(u0.x, ucx, u0.y * ucy);
+    const float s1 = fmaf(ucx, u1.y, -(ucy * u1.x)), c1 = fmaf(ucx, u1.x, ucy * u1.y);
     if (c0 < -0.5f || c1 < -0.5f) return 2.0f * chord;
     const float th0 = atan2_dec(s0, c0), th1 = atan2_dec(s1, c1);
-    const float d0 = div_fast(q0mag * dt, chord), d1 = div_fast(q1mag * dt, chord);
-    const float db0 = div_fast(2.0f, 3.0f * (1.0f + c0)), db1 = div_fast(2.0f, 3.0f * (1.0f + c1));
-    const float s01 = s0 * c1 + c0 * s1;
-    const float area = 0.15f * (2.0f * d0 * s0 + 2.0f * d1 * s1 - d0 * d1 * s01);
-    const float areb = 0.15f * (2.0f * db0 * s0 + 2.0f * db1 * s1 - db0 * db1 * s01);
+    const float sc = dt * rc;
+    const float dd0 = (2.0f / 3.0f) * rcp_fast(1.0f + c0) - q0mag * sc, dd1 = (2.0f / 3.0f) * rcp_fast(1.0f + c1) - q1mag * sc;   // d-bar - d (L217)
+    const float d0 = q0mag * sc, d1 = q1mag * sc, db0 = dd0 + d0, db1 = dd1 + d1;
+    const float s01 = fmaf(s0, c1, c0 * s1);
+    // area(d0, d1) - area(db0, db1), area(a, b) = 3/20 (2 a s0 + 2 b s1 - a b s01)
+    const float darea = fmaf(0.15f * s01, fmaf(db0, db1, -(d0 * d1)), -0.3f * fmaf(dd0, s0, dd1 * s1));
     const float ksum = fabsf(th0 + th1), kdif = fabsf(th0 - th1);
     const float k2 = ksum * ksum;
-    const float e1 = 4.6255e-6f * k2 * k2 * ksum + 7.5e-3f * k2 * kdif;
-    const float e2 = 1.55f * fabsf(area - areb);
-    const float dd0 = db0 - d0, dd1 = db1 - d1;
-    const float e3 = (0.005f * ksum + 0.07f * kdif) * sqrt_fast(dd0 * dd0 + dd1 * dd1);
-    return chord * (e1 + e2 + e3);
+    const float e1 = k2 * fmaf(4.6255e-6f * k2, ksum, 7.5e-3f * kdif);
+    const float e3 = fmaf(0.005f, ksum, 0.07f * kdif) * sqrt_fast(fmaf(dd0, dd0, dd1 * dd1));
+    return chord * (e1 + fmaf(1.55f, fabsf(darea), e3));
 }
 
 

@@ -105,19 +105,68 @@ k_write_segments(const WriteArgs A) {
 }
 
 // ---------------------------------------------------------------- simple leaves: thread per (leaf, side)
-__global__ void __launch_bounds__(kWrThreads)
+// control points of a curve segment (quadratic or cubic) without its tangents: what load_segment_at computes, branch-free
+// (the same expressions, hence the same bits); l* / e*: the legs pick_tangent chooses the start / end tangent from
+struct Ctrl { V2 P0, P3, c1, c2, c3, l1, l2, l3, e1, e2, e3; };
+SX_DEV Ctrl load_ctrl(const Params& P, uint32_t pt, uint32_t tag) {
+    const bool cubic = (tag & 3u) == 3u;
+    const float* p = P.pts + 2 * (uint64_t)pt;
+    const float2 a0 = ldg2(p), a1 = ldg2(p + 2), a2 = ldg2(p + 4), a3 = ldg2(p + (cubic ? 6 : 4));
+    const V2 q0 = xform(P.A, a0.x, a0.y), q1 = xform(P.A, a1.x, a1.y), q2 = xform(P.A, a2.x, a2.y), q3 = xform(P.A, a3.x, a3.y);
+    Ctrl c;
+    c.P0 = q0; c.P3 = q3;
+    const V2 a = q1 - q0, b = q2 - q0, d = q3 - q0;
+    // quadratic (L349): c1 = 2/3 a, c2 = b + 2/3 (a - b), c3 = b; cubic: the control points themselves
+    const V2 e1q = v2(a.x * (2.0f / 3.0f), a.y * (2.0f / 3.0f));
+    const V2 e2q = v2(b.x + (a.x - b.x) * (2.0f / 3.0f), b.y + (a.y - b.y) * (2.0f / 3.0f));
+    c.c1 = cubic ? a : e1q; c.c2 = cubic ? b : e2q; c.c3 = cubic ? d : b;
+    c.l1 = a; c.l2 = b; c.l3 = cubic ? d : b;
+    c.e1 = cubic ? d - b : b - a; c.e2 = cubic ? d - a : b; c.e3 = cubic ? d : b;
+    return c;
+}
+
+__global__ void __launch_bounds__(kWrThreads, 8)
 k_write_simple(const WriteArgs A) {
     const Params& P = A.P;
     const bool arc = P.mode == kModeArc;
     const uint64_t n_sides = 2ull * n_simple_leaves(A);
+    // (n_sides is even and the two sides of a leaf are neighbouring lanes: a lane pair is in the loop together)
     for (uint64_t idx = (uint64_t)blockIdx.x * kWrThreads + threadIdx.x; idx < n_sides; idx += (uint64_t)gridDim.x * kWrThreads) {
+        const uint32_t act = __activemask();   // (whole lane pairs)
         const LeafRec r = load_leaf(A.leaves + (idx >> 1));
         const int side = (int)(idx & 1ull);
-        const uint32_t n_minus = r.n & 0xffffu, nrec = side ? r.n >> 16 : n_minus;
+        const uint32_t n_minus = r.n & 0xffffu, n_plus = r.n >> 16;
+        uint32_t nrec = side ? n_plus : n_minus;
         const uint64_t base = A.seg_off[r.seg] + r.rel + (side ? n_minus : 0u);
-        if (base + nrec > A.cap_records) { atomicOr(A.err, kErrCapacity); continue; }
+        const Ctrl c = load_ctrl(P, P.pt_off[r.seg], P.tags[r.seg]);
+        // the lane's own end of the piece: side 0 the start point, side 1 the end point (exchanged below); at an end of the
+        // segment the cubic's own point and limit tangent (R-5), inside it cubic_point() as in the count pass
+        const uint32_t t0_u = r.key & 0xffffu, level = (r.key >> 16) & 31u;
+        const float dt = __uint_as_float((127u - level) << 23);
+        const bool at0 = t0_u == 0u, at1 = t0_u + 1u == (1u << level);
+        Seg s;
+        s.kind = 3; s.degenerate = false; s.P0 = c.P0; s.P3 = c.P3; s.c1 = c.c1; s.c2 = c.c2; s.c3 = c.c3;
+        s.ts = s.te = v2(0.0f, 0.0f);
+        float4 mine;
+        if (side ? at1 : at0) {
+            bool dg;
+            const V2 u = pick_tangent(side ? c.e1 : c.l1, side ? c.e2 : c.l2, side ? c.e3 : c.l3, &dg);
+            mine = side ? make_float4(c.c3.x, c.c3.y, u.x, u.y) : make_float4(0.0f, 0.0f, u.x, u.y);
+        } else {
+            float qm, q2;
+            mine = cubic_point(s, (float)(t0_u + (uint32_t)side) * dt, &qm, &q2);
+        }
+        float4 other;
+        other.x = __shfl_xor_sync(act, mine.x, 1); other.y = __shfl_xor_sync(act, mine.y, 1);
+        other.z = __shfl_xor_sync(act, mine.z, 1); other.w = __shfl_xor_sync(act, mine.w, 1);
+        const float4 a = side ? other : mine, b = side ? mine : other;
         Piece p;
-        leaf_piece(P, r, p);
+        p.base = c.P0; p.P3 = c.P3; p.at0 = at0; p.at1 = at1;
+        p.la = v2(a.x, a.y); p.ua = v2(a.z, a.w);
+        p.lb = v2(b.x, b.y); p.ub = v2(b.z, b.w);
+        p.ch = p.lb - p.la;
+        p.k0 = r.k0; p.k1 = r.k1; p.L = r.L;
+        if (base + nrec > A.cap_records) { atomicOr(A.err, kErrCapacity); nrec = 0; }   // the side is not written
         const float eta = side ? r.h : -r.h;
         const float4 nocusp = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
         const uint32_t kind = side ? (uint32_t)(kOffset | kPlus) : (uint32_t)kOffset;
@@ -125,7 +174,7 @@ k_write_simple(const WriteArgs A) {
         o.n = (int)nrec; o.rule = kRuleUniform; o.ta = 0.0f; o.tb = 1.0f; o.ua = o.ub = 0.0f;
         Spiral z;
         if (nrec > 1u) {
-            if (!arc) o = offset_plan(p, eta, 0.0f, 1.0f, P.mode, P.tol_fl);   // (same call, same count as the count pass's side plan)
+            if (!arc) o = offset_plan(p, eta, 0.0f, 1.0f, P.mode, P.tol_fl);   // (same call, same count as in the count pass)
             es_prepare(p, z);
         }
         float tp;
