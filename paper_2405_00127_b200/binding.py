@@ -135,7 +135,7 @@ def sx_write(ctx, out_records, cap_records, mode=None, stream=None):
 
 
 def stroke_expand_into(ctx, tags, points, styles, affine, tolerance, mode, out_records, path_offsets, want_total=True, stream=None):
-    """The whole path in one pass into a caller-provided CUDA tensor (float32 [cap,4] line / [cap,8] arc).  Returns
+    """The whole path in one asynchronous call into a caller-provided CUDA tensor (float32 [cap,4] line / [cap,8] arc).  Returns
     the record count (None when want_total is False: the call stays asynchronous).  Raises SX_E_CAPACITY with the
     needed count in .needed when the records do not fit."""
     args = _dev_streams(tags, points, styles)

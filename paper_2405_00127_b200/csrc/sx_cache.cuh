@@ -1,52 +1,16 @@
-// sx_cache.cuh -- the piece cache between the count kernel (b) and the write kernel (d), and the
-// record-indexed evaluation of one side of one Euler-spiral piece.
+// sx_cache.cuh -- the record-indexed evaluation of one side of one Euler-spiral piece: packed side plans and PART tables.
 //
-// The count kernel runs Alg. 2 once per curve segment and stores every accepted
-// Euler-spiral piece as an 80-byte descriptor; the write kernel never repeats the cubic -> spiral fit.
-// It maps one thread to one OUTPUT RECORD (the per-output-point balance the paper leaves as future
-// work, L585): a block stages a tile of descriptors in shared memory, rebuilds the two side plans of
-// each piece (same device functions as the count kernel, hence the same counts), turns them into a
-// table of PARTS (below) and lets every thread locate its record by binary search over the parts.
+// The general writer (k_write_general, sx_write.cuh) maps one thread to one OUTPUT RECORD (the per-output-point balance
+// the paper leaves as future work, L585): a warp stages 16 pieces in shared memory, builds the two side plans of
+// each (same device functions as the count pass, hence the same counts), turns them into a table of PARTS (below)
+// and lets every thread locate its record by binary search over the parts.
 #pragma once
 #include "sx_segment.cuh"
 
 namespace sx {
 
-constexpr uint32_t kInvalidSeg = 0xffffffffu;  // "no piece" marker of a staging thread beyond the cache's end
-constexpr uint32_t kRelMask = 0x3fffffffu, kAt0Bit = 1u << 30, kAt1Bit = 1u << 31;
-constexpr int kDescQuads = 5;   // 5 x 16 B
-
 SX_DEV float f_of_u(uint32_t u) { return __uint_as_float(u); }
 SX_DEV uint32_t u_of_f(float f) { return __float_as_uint(f); }
-
-// q0: P0 P3 | q1: la lb | q2: ua ub | q3: k0 k1 L h | q4: seg, rel|flags, n_minus, n_plus
-SX_DEV void piece_store(float4* slot, const Piece& p, float h, uint32_t seg, uint32_t rel, uint32_t n_minus, uint32_t n_plus) {
-    slot[0] = make_float4(p.base.x, p.base.y, p.P3.x, p.P3.y);
-    slot[1] = make_float4(p.la.x, p.la.y, p.lb.x, p.lb.y);
-    slot[2] = make_float4(p.ua.x, p.ua.y, p.ub.x, p.ub.y);
-    slot[3] = make_float4(p.k0, p.k1, p.L, h);
-    uint32_t r = (rel & kRelMask) | (p.at0 ? kAt0Bit : 0u) | (p.at1 ? kAt1Bit : 0u);
-    slot[4] = make_float4(f_of_u(seg), f_of_u(r), f_of_u(n_minus), f_of_u(n_plus));
-}
-
-struct PieceHead { uint32_t seg, rel, n_minus, n_plus; bool at0, at1; };
-SX_DEV PieceHead piece_head(float4 q) {  // q = quad 4 of the descriptor
-    PieceHead hd;
-    hd.seg = u_of_f(q.x);
-    uint32_t r = u_of_f(q.y);
-    hd.rel = r & kRelMask; hd.at0 = (r & kAt0Bit) != 0u; hd.at1 = (r & kAt1Bit) != 0u;
-    hd.n_minus = u_of_f(q.z); hd.n_plus = u_of_f(q.w);
-    return hd;
-}
-SX_DEV void piece_load(const float4* slot, const PieceHead& hd, Piece& p, float* h) {
-    float4 a = __ldg(slot), b = __ldg(slot + 1), c = __ldg(slot + 2), d = __ldg(slot + 3);
-    p.base = v2(a.x, a.y); p.P3 = v2(a.z, a.w);
-    p.la = v2(b.x, b.y); p.lb = v2(b.z, b.w);
-    p.ua = v2(c.x, c.y); p.ub = v2(c.z, c.w);
-    p.ch = p.lb - p.la;  // the same subtraction fit_next performed
-    p.k0 = d.x; p.k1 = d.y; p.L = d.z; *h = d.w;
-    p.at0 = hd.at0; p.at1 = hd.at1;
-}
 
 // ---------------------------------------------------------------- the side plan as the writer keeps it in shared memory
 // 52 bytes instead of sizeof(SidePlan) = 100: range bounds are implied by the cusp parameter (range 0 = [0, tc],

@@ -51,7 +51,7 @@ k_tag_scan(const uint8_t* __restrict__ tags, uint32_t n, uint32_t n_points, uint
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_tile = atomicAdd(ticket, 1u);
     // the first kernel of every call: the tile size the last expansion kernel proposed becomes the one of this call
-    // (k_expand reads hint[0] only; both of its launches in a count + write call see the same value)
+    // (k_count reads hint[0] only)
     if (blockIdx.x == 0 && tid == 0) hint[0] = hint[1];
     __syncthreads();
     const uint32_t tile = s_tile;

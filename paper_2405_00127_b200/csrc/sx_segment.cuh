@@ -1,9 +1,10 @@
 // sx_segment.cuh -- one input segment end to end (Alg. 1 L306-343 per thread, Alg. 2 L351-438 inside).
 //
-// The pieces the kernels are made of: fit_next (Alg. 2 as a resumable generator: the count kernel), joins and caps
-// (segment_tail: the count kernel with EMIT = false, the segment writer with EMIT = true) and process_segment, the
-// thread-per-segment reference walk of everything a segment emits, in canonical order (the fallback writer, and the
-// definition the table-driven piece writer of sx_cache.cuh / sx_kernels.cu reproduces bit for bit).  Counting and
+// The pieces the kernels are made of: joins and caps (emit_join / emit_cap: the count pass with EMIT = false, the segment
+// writer with EMIT = true), fit_next (Alg. 2 as a resumable generator) and process_segment, the thread-per-segment
+// reference walk of everything a segment emits, in canonical order: the walk writer (k_write_walk) and the walk count of
+// sx_count.cuh -- what a tile that does not fit the count pass's tables falls back to -- and the definition the
+// node-parallel count pass and the table-driven writers reproduce bit for bit (tests/test_gpu_parity.py).  Counting and
 // writing instantiate the same plan functions, so the counts agree by construction.
 #pragma once
 #include "sx_piece.cuh"
@@ -188,8 +189,8 @@ SX_DEV uint32_t emit_cap(const Params& P, const Style& st, V2 V, V2 T, float h, 
 // ---------------------------------------------------------------- Alg. 2: cubic -> Euler spirals
 // Iterative bisection with the two-word stack (t0_u, dt), pop by count-trailing-zeros (L444).  One pass
 // serves both sides: the fit does not depend on the offset.  The loop is written as a resumable
-// generator (fit_next returns one accepted piece per call) so that the thread-per-segment writer, the
-// count kernel and the piece cache all run the identical instruction sequence.
+// generator (fit_next returns one accepted piece per call): the walk count and the walk writer run the identical
+// instruction sequence.
 struct FitState {
     uint32_t t0_u;
     float dt;

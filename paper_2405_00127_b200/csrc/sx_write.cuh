@@ -88,20 +88,23 @@ k_write_segments(const WriteArgs A) {
     const Params& P = A.P;
     const uint32_t i = blockIdx.x * (uint32_t)kWrThreads + threadIdx.x;
     if (i >= P.n_tags) return;
-    const uint32_t count = A.seg_count[i];
-    if (count == 0u) return;   // width <= 0, or a malformed stream
+    // first level of loads in one batch (the kernel is bound by the latency of its dependent loads): the segment's own scan
+    // results, its successor's tag and point offset (the join partner of every segment that does not end a subpath)
+    const uint32_t jn = i + 1u < P.n_tags ? i + 1u : i;
+    const uint32_t count = A.seg_count[i], tail = A.seg_tail[i], tag = P.tags[i], pt = P.pt_off[i], path = P.path_idx[i], first_seg = P.sp_first[i];
+    const uint32_t tag_n = P.tags[jn], pt_n = P.pt_off[jn];
     const uint64_t base = A.seg_off[i];
+    if (count == 0u) return;   // width <= 0, or a malformed stream
     if (base + count > A.cap_records) { atomicOr(A.err, kErrCapacity); return; }   // nothing of the segment is written
-    const uint32_t tag = P.tags[i];
     Style st;
     float h;
-    load_style(P, P.path_idx[i], &st, &h);
-    const Seg s = load_segment(P, i, tag);
+    load_style(P, path, &st, &h);
+    const Seg s = load_segment_at(P, pt, tag);
     Writer w;
     w.out = A.out; w.base = base; w.seg = i; w.mode = P.mode;
-    uint32_t first = count - A.seg_tail[i];
+    uint32_t first = count - tail;
     if (s.kind == 1 || s.degenerate) { emit_straight(s, h, &w); first = 2u; }
-    segment_tail<true>(P, i, tag, s, st, h, &w, first);
+    segment_tail<true>(P, tag, s, st, h, first_seg, tag_n, pt_n, &w, first);
 }
 
 // ---------------------------------------------------------------- simple leaves: thread per (leaf, side)

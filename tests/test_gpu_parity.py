@@ -53,7 +53,7 @@ class GpuResult:
 
 
 def gpu_run(B, ctx, sc, mode, host=False, into=False):
-    """host: stroke_expand_host (pinned host buffers); into: stroke_expand_into (the one-pass path, per-segment
+    """host: stroke_expand_host (pinned host buffers); into: stroke_expand_into (one asynchronous call, per-segment
     results kept); default: stroke_expand = sx_count + allocation callback + sx_write."""
     dev = "cuda:0"
     if into:
@@ -153,7 +153,7 @@ CASES = [("c1", None, 0), ("c2", None, 0), ("c2", None, 1), ("c3", 6000, 0), ("c
 
 @pytest.mark.parametrize("name,npaths,mode", CASES)
 def test_parity_with_oracle(B, ctx, name, npaths, mode):
-    """The one-pass path (stroke_expand_into) element by element against the oracle; the two-phase path (sx_count,
+    """The one-call path (stroke_expand_into) element by element against the oracle; the two-phase path (sx_count,
     allocation callback, sx_write) must give the same bits."""
     sc = S.make(name, n_paths=npaths)
     g = gpu_run(B, ctx, sc, mode, into=True)
