@@ -37,7 +37,7 @@ UNIT = "segments/s"
 MODE_OF = {"c3": 0, "c4": 1, "c5": 0, "c1": 0, "c2": 0}
 # whole-step dram__bytes_read.sum + dram__bytes_write.sum per step from the committed `ncu --set full` captures
 # (profiles/r2_counters.md names the command and the commit of each); None = not captured for that workload / mode
-NCU_TRAFFIC = {}
+NCU_TRAFFIC = {"c4-arc": 529.0e6}
 NCU_TRAFFIC_SOURCE = "profiles/r2_counters.md"
 REF_SAMPLE_PATHS = {"c4": 20000, "c5": 1000, "c3": 20000, "c1": 256, "c2": 2000}
 # issue slots (FMA = 1) and special-function operations per unit of the method's own work
@@ -312,6 +312,35 @@ def run_ours(args):
     assert rec1.shape[0] == total
     del rec1
 
+    # ---- tile binning of the records just written (line mode only), device-timed
+    binning = None
+    if args.binning and mode == 0:
+        ext = float(sc.points.max()) + 128.0
+        tiles_xy = int(np.ceil(ext / 16.0))
+        toff = torch.empty(tiles_xy * tiles_xy + 1, dtype=torch.int32, device=dev)
+        try:
+            B.sx_bin_lines(ctx, out, tiles_xy, tiles_xy, toff, None)
+            pairs = 0
+        except B.StrokeExpandError as e:
+            pairs = e.needed
+        B.sx_last_error(ctx)
+        tlines = torch.empty(max(pairs, 1), dtype=torch.int32, device=dev)
+        b_evs = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(5)]
+        for k in range(8):
+            flush.fill_(k)
+            if k >= 3:
+                b_evs[k - 3][0].record(stream)
+            B.sx_bin_lines(ctx, out, tiles_xy, tiles_xy, toff, tlines, want_total=False)
+            if k >= 3:
+                b_evs[k - 3][1].record(stream)
+        torch.cuda.synchronize()
+        assert B.sx_last_error(ctx) == 0 and int(toff[-1].item()) == pairs
+        t_bin = float(np.mean([e[0].elapsed_time(e[1]) for e in b_evs])) * 1e-3
+        b_bytes = 2 * 16 * total + 4 * pairs + 12 * (tiles_xy * tiles_xy + 1)
+        binning = {"call": "sx_bin_lines (count, scan, scatter) on the records of this step", "tiles": [tiles_xy, tiles_xy], "pairs": int(pairs),
+                   "ms_per_call": 1e3 * t_bin, "records_per_s": total / t_bin, "algorithmic_bytes": int(b_bytes),
+                   "achieved_gbs": b_bytes / t_bin / 1e9}
+
     # ---- end to end through the host-buffer entry point (pinned host memory, copies inside the timed region)
     htags, hpts, hsty = B.scene_to_torch(sc, pin=True)
     hout = torch.empty((total, width), dtype=torch.float32).pin_memory()
@@ -352,6 +381,7 @@ def run_ours(args):
                 "kernel_ms": {"k_tag_scan": 1e3 * t_scan, "k_count": 1e3 * t_count, "k_alloc_scan": 1e3 * t_alloc, "writers": 1e3 * t_write,
                               "timed_by": "library events on the launching stream, mean of %d steps" % k_steps},
                 "tiles": stats,
+                **({"binning": dict(binning, frac_of_hbm_peak=binning["achieved_gbs"] / peak)} if binning else {}),
                 "gpu_launches": int(launches), "clocks": clocks,
                 "one_shot": {"call": "stroke_expand (count pass, host read of the total, allocation callback, write pass)",
                              "ms_per_call_wall": 1e3 * t_one, "value": n_seg / t_one, "unit": UNIT},
@@ -402,6 +432,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--mode", default=None, choices=["line", "arc"], help="override the workload's output mode")
+    ap.add_argument("--binning", action="store_true", help="line mode: also time the tile binning of the records (SURVEY 8(f)-4)")
     ap.add_argument("--paths", type=int, default=None, help="profiling only: shrink the workload to this many paths")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:

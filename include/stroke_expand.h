@@ -175,6 +175,26 @@ sx_status stroke_expand_host(sx_ctx* ctx, const uint8_t* h_tags, uint64_t n_tags
                              void* h_out_records, uint64_t cap_records, uint64_t* h_n_records, uint64_t* h_path_offsets,
                              void* cuda_stream);
 
+/* ------------------------------------------------------------------ tile binning of the line soup
+ * PAPER.md L450 (section 8.1, Fig. 14): "the line soup elements are spatially sorted by subsequent compute stages
+ * into a grid of 16x16 pixel tiles" -- the first stage of the tile-based renderer downstream of the stroke expansion.
+ * The paper leaves the details out; the definition is reading R-19 of DESIGN.md: a coordinate v belongs to tile index
+ * floor(v / 16); a record is binned, row of tiles by row, into the tiles its part inside the row's closed slab
+ * 16 r <= y <= 16 r + 16 spans in x (fp32, one rounding per operation); rows / columns outside the viewport of
+ * tiles_x x tiles_y tiles and records with a non-finite coordinate are skipped.
+ *   d_lines[n_lines]            device, read-only, 16-byte aligned: sx_line records (e.g. the line-mode output above)
+ *   d_tile_offsets[tiles + 1]   device, written: CSR offsets over the tiles in row-major order (tile = r * tiles_x + c);
+ *                               the last entry is the number of (tile, record) pairs
+ *   d_tile_lines[cap_entries]   device, written: per tile the indices of its records, in NO defined order (the soup is
+ *                               unordered, L450).  cap_entries == 0: count and scan only (d_tile_lines may be NULL)
+ *   h_total                     HOST, optional: when non-NULL the call synchronises the stream and writes the pair count;
+ *                               SX_E_CAPACITY when it exceeds cap_entries (nothing is written past the capacity; the
+ *                               device-side flag is raised either way, see sx_last_error) or 2^32 - 1
+ * n_lines < 2^32, tiles_x * tiles_y < 2^31.  Asynchronous on cuda_stream unless h_total is given. */
+sx_status sx_bin_lines(sx_ctx* ctx, const sx_line* d_lines, uint64_t n_lines, uint32_t tiles_x, uint32_t tiles_y,
+                       uint32_t* d_tile_offsets, uint32_t* d_tile_lines, uint64_t cap_entries, uint64_t* h_total,
+                       void* cuda_stream);
+
 /* ------------------------------------------------------------------ introspection
  * Device pointers into the context's scratch of the last sx_count (valid until the next call on the
  * context): the tag-scan results and the per-segment record counts / offsets.  Any out pointer may

@@ -24,7 +24,7 @@ ARC_DTYPE = np.dtype([("x0", "<f4"), ("y0", "<f4"), ("x1", "<f4"), ("y1", "<f4")
 SX_OPT_KEEP_SEGMENT_INFO, SX_OPT_TILE_SEGMENTS, SX_OPT_TIME_KERNELS = 1, 2, 3
 
 EXPORTS = ["sx_create", "sx_destroy", "sx_count", "sx_write", "stroke_expand", "stroke_expand_into", "stroke_expand_host",
-           "sx_segment_info", "sx_last_error", "sx_set_option", "sx_call_stats", "sx_kernel_times", "sx_measure_issue_peaks", "sx_launch_count",
+           "sx_bin_lines", "sx_segment_info", "sx_last_error", "sx_set_option", "sx_call_stats", "sx_kernel_times", "sx_measure_issue_peaks", "sx_launch_count",
            "sx_strerror"]
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
@@ -58,6 +58,7 @@ def lib():
         L.sx_last_error.argtypes = [vp, vp]
         L.sx_set_option.argtypes = [vp, i32, u64]
         L.sx_call_stats.argtypes = [vp, C.POINTER(u64), vp]
+        L.sx_bin_lines.argtypes = [vp, vp, u64, C.c_uint32, C.c_uint32, vp, vp, u64, C.POINTER(u64), vp]
         L.sx_kernel_times.argtypes = [vp, C.POINTER(C.c_float)]
         L.sx_measure_issue_peaks.argtypes = [i32, C.POINTER(C.c_double)]
         L.sx_launch_count.argtypes = [vp]
@@ -206,6 +207,28 @@ def stroke_expand_host(ctx, tags, points, styles, affine, tolerance, mode, out_r
         raise e
     _check(st, "stroke_expand_host")
     return int(n_rec.value)
+
+
+def sx_bin_lines(ctx, lines, tiles_x, tiles_y, tile_offsets, tile_lines=None, want_total=True, stream=None):
+    """Tile binning of line records.  lines: float32 CUDA tensor [n, 4]; tile_offsets: int32 CUDA tensor
+    [tiles_x * tiles_y + 1] (written, CSR); tile_lines: int32 CUDA tensor [cap] or None (count and scan only).  Returns the
+    number of (tile, record) pairs when want_total (synchronises); raises StrokeExpandError with .needed on SX_E_CAPACITY."""
+    assert lines.is_cuda and lines.is_contiguous() and lines.dtype == torch.float32 and lines.dim() == 2 and lines.shape[1] == 4
+    assert tile_offsets.is_cuda and tile_offsets.is_contiguous() and tile_offsets.element_size() == 4
+    assert tile_offsets.numel() >= int(tiles_x) * int(tiles_y) + 1
+    cap = 0
+    if tile_lines is not None:
+        assert tile_lines.is_cuda and tile_lines.is_contiguous() and tile_lines.element_size() == 4
+        cap = tile_lines.numel()
+    total = C.c_uint64(0)
+    st = lib().sx_bin_lines(ctx, C.c_void_p(lines.data_ptr()), lines.shape[0], int(tiles_x), int(tiles_y), C.c_void_p(tile_offsets.data_ptr()),
+                            C.c_void_p(tile_lines.data_ptr() if cap else 0), cap, C.byref(total) if want_total else None, _stream_ptr(stream))
+    if st == SX_E_CAPACITY:
+        e = StrokeExpandError(st, "sx_bin_lines")
+        e.needed = int(total.value)
+        raise e
+    _check(st, "sx_bin_lines")
+    return int(total.value) if want_total else None
 
 
 def _view(ptr, n, dtype, device):

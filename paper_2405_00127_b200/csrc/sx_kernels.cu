@@ -15,6 +15,7 @@
 
 #include "../../include/stroke_expand.h"
 #include "sx_write.cuh"
+#include "sx_bin.cuh"
 #include "sx_peaks.cuh"
 
 // ====================================================================== host side
@@ -56,6 +57,8 @@ struct sx_ctx {
     bool counted, total_known;
     uint64_t total;
     uint64_t launches;
+    // scratch of sx_bin_lines: [ticket, total: 64 B][look-back words][tile counters][tile cursors]
+    uint8_t* bin_area; uint64_t bin_bytes;
     // staging for stroke_expand_host
     uint8_t* st_in;  uint64_t st_in_bytes;
     uint8_t* st_out; uint64_t st_out_bytes;
@@ -293,6 +296,7 @@ sx_status sx_destroy(sx_ctx* c) {
     cudaFree(c->leaves);
     cudaFree(c->sync_area);
     cudaFree(c->d_hint);
+    cudaFree(c->bin_area);
     cudaFree(c->st_in);
     cudaFree(c->st_out);
     cudaFree(c->st_path);
@@ -430,6 +434,46 @@ sx_status stroke_expand_host(sx_ctx* c, const uint8_t* h_tags, uint64_t n_tags, 
     }
     SX_CUDA(cudaStreamSynchronize(s));
     return SX_OK;
+}
+
+sx_status sx_bin_lines(sx_ctx* c, const sx_line* d_lines, uint64_t n_lines, uint32_t tiles_x, uint32_t tiles_y, uint32_t* d_tile_offsets,
+                       uint32_t* d_tile_lines, uint64_t cap_entries, uint64_t* h_total, void* cuda_stream) {
+    if (!c || !d_tile_offsets) return SX_E_INVALID_ARG;
+    if (n_lines >= (1ull << 32) || tiles_x == 0 || tiles_y == 0 || (uint64_t)tiles_x * tiles_y >= (1ull << 31)) return SX_E_INVALID_ARG;
+    if (n_lines > 0 && (!d_lines || (reinterpret_cast<uintptr_t>(d_lines) & 15u))) return SX_E_INVALID_ARG;
+    if (cap_entries > 0 && !d_tile_lines) return SX_E_INVALID_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    SX_CUDA(cudaSetDevice(c->device));
+    sx_status rc = ensure_scratch(c, 0);   // (the error flag lives in the context's sync area)
+    if (rc != SX_OK) return rc;
+    const uint32_t tiles = tiles_x * tiles_y;
+    const uint32_t scan_tiles = (tiles + sx::kScan32Tile - 1) / sx::kScan32Tile;
+    const uint64_t o_states = 64, o_counts = o_states + round_up((uint64_t)(scan_tiles + 1) * 8, 64), o_cursor = o_counts + round_up((uint64_t)tiles * 4, 64);
+    const uint64_t need = o_cursor + round_up((uint64_t)tiles * 4, 64);
+    rc = grow(&c->bin_area, &c->bin_bytes, need);
+    if (rc != SX_OK) return rc;
+    uint32_t* ticket = reinterpret_cast<uint32_t*>(c->bin_area);
+    uint64_t* d_total = reinterpret_cast<uint64_t*>(c->bin_area + 8);
+    uint64_t* states = reinterpret_cast<uint64_t*>(c->bin_area + o_states);
+    uint32_t* counts = reinterpret_cast<uint32_t*>(c->bin_area + o_counts);
+    uint32_t* cursor = reinterpret_cast<uint32_t*>(c->bin_area + o_cursor);
+    SX_CUDA(cudaMemsetAsync(c->bin_area, 0, need, s));
+    const float4* lines = reinterpret_cast<const float4*>(d_lines);
+    const uint64_t want = (n_lines + sx::kBinThreads - 1) / sx::kBinThreads;
+    const unsigned grid = (unsigned)(want < (uint64_t)c->sm_count * 16 ? (want ? want : 1) : (uint64_t)c->sm_count * 16);
+    sx::k_bin_walk<false><<<grid, sx::kBinThreads, 0, s>>>(lines, n_lines, tiles_x, tiles_y, counts, nullptr, nullptr, 0, ctx_err(c));
+    sx::k_scan_u32<<<scan_tiles, sx::kScanThreads, 0, s>>>(counts, tiles, d_tile_offsets, d_total, states, ticket, ctx_err(c));
+    c->launches += 2;
+    if (cap_entries > 0) {
+        sx::k_bin_walk<true><<<grid, sx::kBinThreads, 0, s>>>(lines, n_lines, tiles_x, tiles_y, cursor, d_tile_offsets, d_tile_lines, cap_entries, ctx_err(c));
+        c->launches += 1;
+    }
+    SX_CUDA(cudaGetLastError());
+    if (!h_total) return SX_OK;
+    SX_CUDA(cudaMemcpyAsync(&c->h_pinned[5], d_total, 8, cudaMemcpyDeviceToHost, s));
+    SX_CUDA(cudaStreamSynchronize(s));
+    *h_total = c->h_pinned[5];
+    return (*h_total > cap_entries || (*h_total >> 32)) ? SX_E_CAPACITY : SX_OK;
 }
 
 sx_status sx_segment_info(sx_ctx* c, const uint32_t** d_pt_off, const uint32_t** d_path_idx, const uint32_t** d_sp_first,
