@@ -34,7 +34,7 @@ typedef struct {
     float miter_limit;
     uint8_t join; /* 0 miter 1 round 2 bevel */
     uint8_t cap;  /* 0 butt 1 square 2 round */
-    uint16_t pad;
+    uint16_t fill; /* bit 0: the path is FILLED, not stroked (Alg. 1); width, join, cap are then ignored */
     uint32_t rsv;
 } so_style;
 
@@ -43,7 +43,7 @@ enum { CAP_BUTT = 0, CAP_SQUARE = 1, CAP_ROUND = 2 };
 enum { MODE_LINE = 0, MODE_ARC = 1 };
 
 /* record kinds (low 3 bits) | side bit (8 = +h side) */
-enum { K_OFFSET = 0, K_OFFSET_REV = 1, K_EVOLUTE = 2, K_CONNECTOR = 3, K_JOIN_OUTER = 4, K_JOIN_INNER = 5, K_CAP = 6, K_PLUS = 8 };
+enum { K_OFFSET = 0, K_OFFSET_REV = 1, K_EVOLUTE = 2, K_CONNECTOR = 3, K_JOIN_OUTER = 4, K_JOIN_INNER = 5, K_CAP = 6, K_CLOSE = 7, K_PLUS = 8 };
 
 enum { ST_FIT_ITERS = 0, ST_PIECES, ST_RANGES_REG, ST_RANGES_SUP, ST_REC_OFFSET, ST_REC_EVOLUTE, ST_REC_CONNECTOR,
        ST_REC_JOIN, ST_REC_CAP, ST_LINE_SEGS, ST_CURVE_SEGS, ST_N };
@@ -253,6 +253,7 @@ typedef struct {
     int mode;
     float tol_es, tol_fl;
     uint32_t cur_seg;
+    int fill;        /* the current path is filled: offset 0, one side (Alg. 1) */
 } ctx_t;
 
 static int push_rec(ctx_t* c, v2d a, v2d b, double angle, int kind) {
@@ -502,6 +503,10 @@ static int piece_records(ctx_t* c, piece_t* p, float h) {
     side_records(c, p, -h, &l);
     for (size_t i = 0; i < l.n; i++)
         if (push_rec(c, l.r[i].a, l.r[i].b, c->mode == MODE_ARC ? l.r[i].angle : 0.0, l.r[i].kind)) return -1;
+    /* a fill is "flatten_cubic(segment, 0)" (Alg. 1): the curve itself, once.  With eta = 0 there is no cusp
+     * (1 - kappa eta = 1) and offset_params integrates the pure Euler-spiral density sqrt|kappa| (section 2.2;
+     * arcs: L171). */
+    if (c->fill) { free(l.r); return 0; }
     /* +h side: mirror image of its forward-t list (reverse order, swap end points, negate angle) */
     l.n = 0;
     side_records(c, p, h, &l);
@@ -757,7 +762,28 @@ int so_expand(const uint8_t* tags, uint64_t n_tags, const float* pts, uint64_t n
         while (next_path <= path) out->path_off[next_path++] = before;
         const so_style* st = &styles[path];
         float h = 0.5f * st->width * scale;
-        if (h > 0.0f && isfinite(h)) { /* width <= 0 or non-finite: the path emits nothing */
+        c.fill = st->fill & 1;
+        if (c.fill) {
+            /* Alg. 1: a filled path is flattened with offset 0; an open subpath is closed by a line from its last
+             * point to its first (always emitted, possibly of zero length: counts stay a function of the tags) */
+            seg_t s;
+            load_segment(tags, pts, affine, out->pt_off, i, &s);
+            v2d V0 = {s.P0.x, s.P0.y}, V3 = {s.P3.x, s.P3.y};
+            if (s.kind == 1 || s.degenerate) {
+                out->stats[ST_LINE_SEGS]++;
+                if (push_rec(&c, V0, V3, 0, K_OFFSET)) goto oom;
+            } else {
+                out->stats[ST_CURVE_SEGS]++;
+                if (flatten_cubic(&c, &s, 0.0f)) goto oom;
+            }
+            uint8_t tag = tags[i];
+            if ((((tag >> 2) | (tag >> 4)) & 1) && !((tag >> 7) & 1)) {
+                seg_t f;
+                load_segment(tags, pts, affine, out->pt_off, out->sp_first[i], &f);
+                v2d F0 = {f.P0.x, f.P0.y};
+                if (push_rec(&c, V3, F0, 0, K_CLOSE)) goto oom;
+            }
+        } else if (h > 0.0f && isfinite(h)) { /* width <= 0 or non-finite: the path emits nothing */
             seg_t s;
             load_segment(tags, pts, affine, out->pt_off, i, &s);
             if (s.kind == 1 || s.degenerate) {
@@ -821,7 +847,7 @@ int so_piece_expand(float k0, float k1, float L, float x0, float y0, float dir0,
     out->path_idx = (uint32_t*)calloc(2, sizeof(uint32_t));
     out->sp_first = (uint32_t*)calloc(2, sizeof(uint32_t));
     ctx_t c;
-    c.out = out; c.mode = mode; c.tol_es = 0; c.tol_fl = tol_fl; c.cur_seg = 0;
+    c.out = out; c.mode = mode; c.tol_es = 0; c.tol_fl = tol_fl; c.cur_seg = 0; c.fill = (h == 0.0f);   /* h = 0: the piece of a filled path */
     piece_t p;
     memset(&p, 0, sizeof(p));
     p.k0 = k0; p.k1 = k1; p.L = L;

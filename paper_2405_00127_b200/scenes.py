@@ -16,7 +16,7 @@ from __future__ import annotations
 import numpy as np
 
 STYLE_DTYPE = np.dtype([("width", "<f4"), ("miter_limit", "<f4"), ("join", "u1"), ("cap", "u1"),
-                        ("pad", "<u2"), ("rsv", "<u4")])
+                        ("fill", "<u2"), ("rsv", "<u4")])   # fill: bit 0 = the path is filled, not stroked
 JOIN_MITER, JOIN_ROUND, JOIN_BEVEL = 0, 1, 2
 CAP_BUTT, CAP_SQUARE, CAP_ROUND = 0, 1, 2
 MODE_LINE, MODE_ARC = 0, 1
@@ -255,6 +255,17 @@ def make(name, n_paths=None, seed=None):
     if seed is not None:
         kw["seed"] = seed
     return CONFIGS[name](**kw)
+
+
+def with_fill(scene, every=1, offset=0):
+    """Copy of the scene in which every `every`-th path (starting at `offset`) is FILLED instead of stroked (Alg. 1
+    L309-311: style bit only, no arithmetic here)."""
+    st = scene["styles"].copy()
+    st["fill"][offset::every] = 1
+    out = Scene(scene)
+    out["styles"] = st
+    out["name"] = scene["name"] + "-fill"
+    return out
 
 
 def subset_paths(scene, path_ids):
