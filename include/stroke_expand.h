@@ -55,13 +55,16 @@ enum {
  *   (its first point is the previous segment's last) and pt_off[i+1] = pt_off[i] + count_i +
  *   subpath_end_i.  A subpath of k segments owns 1 + sum(count) points.
  * Style: one per path.  half-width = width/2 * sqrt|det(affine)| (R-14).  width <= 0 or non-finite:
- *   the path emits no records (not an error). */
+ *   the path emits no records (not an error) -- unless it is a FILL (style bit, below). */
 typedef struct {
     float width;
     float miter_limit; /* SVG definition: miter used while 1/sin(beta/2) <= miter_limit              */
     uint8_t join;      /* SX_JOIN_*                                                                   */
     uint8_t cap;       /* SX_CAP_*                                                                    */
-    uint16_t _pad;
+    uint16_t fill;     /* bit 0: FILL the path instead of stroking it (Alg. 1: "if style is fill then
+                          flatten_cubic(segment, 0)"): its segments are flattened at offset 0, one record chain per
+                          segment in path direction, an open subpath is closed by one line from its last point to its
+                          first (kind SX_KIND_CLOSE); width, join, cap and miter_limit are ignored                     */
     uint32_t _rsv;
 } sx_style; /* 16 bytes */
 
@@ -95,6 +98,7 @@ enum {
     SX_KIND_JOIN_OUTER = 4,
     SX_KIND_JOIN_INNER = 5, /* through the vertex (strong correctness, L35)                           */
     SX_KIND_CAP = 6,
+    SX_KIND_CLOSE = 7,      /* the line that closes an open subpath of a FILLED path (Alg. 1)   */
     SX_KIND_PLUS = 8        /* flag: record belongs to the +h side                                    */
 };
 

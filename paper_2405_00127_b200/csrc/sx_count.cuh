@@ -128,6 +128,7 @@ SX_DEV uint32_t count_tail(const CtWarp& S, const Params& P, uint32_t s0, uint32
                            uint32_t first_seg) {
     const bool sp_end = ((tag >> 2) | (tag >> 4)) & 1u;
     const bool closed = (tag >> 7) & 1u;
+    if (st.fill) return (sp_end && !closed) ? 1u : 0u;   // a filled path: the closing line of an open subpath (Alg. 1)
     const uint32_t j = (!sp_end) ? i + 1u : first_seg;   // join partner, or the owner of the start cap
     V2 W, T1;
     if (j >= s0 && j - s0 < sn) { const CtSeg& r = S.seg[j - s0]; T1 = v2(r.tsx, r.tsy); W = v2(0.0f, 0.0f); }
@@ -180,6 +181,7 @@ SX_DEV LeafEval leaf_eval(float4 pa, float4 pb, float h, int mode, float tol_fl)
         if (mode != kModeArc && !e.full[side]) e.n[side] = offset_count(p.k0, p.k1, p.L, eta, kModeLine, tol_fl);
         if (e.full[side]) e.n[side] = 0xffffu;   // (not simple until the full plan says so)
     }
+    if (h == 0.0f) { e.n[1] = 0u; e.full[1] = false; }   // a filled path (Alg. 1): offset 0, the curve once
     return e;
 }
 
@@ -427,7 +429,7 @@ k_count(const CountArgs A) {
             if (lane < (int)sn) {
                 const uint32_t i = s0 + (uint32_t)lane;
                 uint32_t count = 0, tail = my_tail;
-                if (!overflow) { if (my_valid) count = (my_curve ? S.acc[lane] : 2u) + my_tail; }
+                if (!overflow) { if (my_valid) count = (my_curve ? S.acc[lane] : (S.seg[lane].h == 0.0f ? 1u : 2u)) + my_tail; }   // (h == 0: a fill)
                 else if (ok) count = slow_count(P, i, &tail);
                 A.seg_count[i] = count;
                 A.seg_tail[i] = tail;

@@ -36,7 +36,7 @@ constexpr float kKnot0 = 0.70107076f;        // f_approx(0.8), f_approx(1.25), f
 constexpr float kKnot1 = 0.90324929f;
 constexpr float kKnot2 = 2.03885779f;
 
-enum : uint32_t { kOffset = 0, kOffsetRev = 1, kEvolute = 2, kConnector = 3, kJoinOuter = 4, kJoinInner = 5, kCap = 6, kPlus = 8 };
+enum : uint32_t { kOffset = 0, kOffsetRev = 1, kEvolute = 2, kConnector = 3, kJoinOuter = 4, kJoinInner = 5, kCap = 6, kClose = 7, kPlus = 8 };
 enum : int { kJoinMiter = 0, kJoinRound = 1, kJoinBevel = 2, kCapButt = 0, kCapSquare = 1, kCapRound = 2, kModeLine = 0, kModeArc = 1 };
 
 // ---------------------------------------------------------------- float2 helpers (plain operators: no contraction)

@@ -114,7 +114,7 @@ SX_DEV void emit_round(const Writer* w, uint32_t first, int n, V2 V, V2 r, V2 A,
     }
 }
 
-struct Style { float width, miter_limit; int join, cap; };
+struct Style { float width, miter_limit; int join, cap; bool fill; };
 
 // join between this segment (end point V, end tangent T0) and its partner (start point W, start
 // tangent T1) -- R-10.  -h side runs forward A->B, +h side backward B'->A'.
@@ -235,16 +235,17 @@ SX_DEV bool fit_next(const Params& P, const Seg& s, FitState& f, Piece& p) {
     }
 }
 
+// fill: "flatten_cubic(segment, 0)" (Alg. 1): h = 0 and the curve itself, once
 template <bool EMIT>
-SX_DEV uint32_t flatten_cubic(const Params& P, const Seg& s, float h, const Writer* w) {
+SX_DEV uint32_t flatten_cubic(const Params& P, const Seg& s, float h, bool fill, const Writer* w) {
     uint32_t n = 0;
     FitState f = fit_begin(s);
     Piece p;
     Spiral z;
     while (fit_next(P, s, f, p)) {
         if (EMIT) es_prepare(p, z);
-        n += piece_side<EMIT>(p, z, -h, false, P, w, n);  // -h side, forward
-        n += piece_side<EMIT>(p, z, h, true, P, w, n);    // +h side, mirrored
+        n += piece_side<EMIT>(p, z, -h, false, P, w, n);             // -h side, forward
+        if (!fill) n += piece_side<EMIT>(p, z, h, true, P, w, n);    // +h side, mirrored
     }
     return n;
 }
@@ -256,8 +257,9 @@ SX_DEV bool load_style(const Params& P, uint32_t path, Style* st, float* h) {
     st->miter_limit = u2f(raw.y);
     st->join = (int)(raw.z & 0xffu);
     st->cap = (int)((raw.z >> 8) & 0xffu);
-    *h = 0.5f * st->width * P.scale;
-    return *h > 0.0f && *h < INFINITY;  // width <= 0 or non-finite: the path emits nothing
+    st->fill = ((raw.z >> 16) & 1u) != 0u;   // Alg. 1: the path is filled: offset 0, one side
+    *h = st->fill ? 0.0f : 0.5f * st->width * P.scale;
+    return st->fill || (*h > 0.0f && *h < INFINITY);  // a stroke of width <= 0 or non-finite: the path emits nothing
 }
 
 // what follows the offset curves of segment i (Alg. 1): the join with its partner, or, on the last
@@ -270,6 +272,15 @@ SX_DEV uint32_t segment_tail(const Params& P, uint32_t tag, const Seg& s, const 
     bool sp_end = ((tag >> 2) | (tag >> 4)) & 1u;
     bool closed = (tag >> 7) & 1u;
     uint32_t n = 0;
+    if (st.fill) {   // no joins, no caps: the line that closes an open subpath (always emitted: counts follow the tags)
+        if (!sp_end || closed) return 0u;
+        if (EMIT) {
+            V2 F, Tf;
+            load_segment_start(P, first_seg, &F, &Tf);
+            w->put(first, s.P3, F, 0.0f, kClose);
+        }
+        return 1u;
+    }
     if (!sp_end || closed) {
         V2 W, T1;
         if (sp_end) load_segment_start(P, first_seg, &W, &T1);
@@ -290,9 +301,11 @@ SX_DEV uint32_t segment_tail(const Params& P, uint32_t i, uint32_t tag, const Se
 }
 
 // straight fast path (R-1b): the two offset lines of a line (or fully degenerate) segment are exact
-SX_DEV void emit_straight(const Seg& s, float h, const Writer* w) {
+SX_DEV uint32_t emit_straight(const Seg& s, float h, bool fill, const Writer* w) {
+    if (fill) { w->put(0, s.P0, s.P3, 0.0f, kOffset); return 1u; }   // the segment itself
     w->put(0, offset_point(s.P0, s.ts, -h), offset_point(s.P3, s.te, -h), 0.0f, kOffset);
     w->put(1, offset_point(s.P3, s.te, h), offset_point(s.P0, s.ts, h), 0.0f, kOffset | kPlus);
+    return 2u;
 }
 
 // thread-per-segment reference path: everything segment i emits, in canonical order
@@ -306,10 +319,10 @@ SX_DEV uint32_t process_segment(const Params& P, uint32_t i, Writer* w, uint32_t
     Seg s = load_segment(P, i, tag);
     uint32_t n;
     if (s.kind == 1 || s.degenerate) {
-        if (EMIT) emit_straight(s, h, w);
-        n = 2;
+        if (EMIT) emit_straight(s, h, st.fill, w);
+        n = st.fill ? 1u : 2u;
     } else {
-        n = flatten_cubic<EMIT>(P, s, h, w);
+        n = flatten_cubic<EMIT>(P, s, h, st.fill, w);
     }
     const uint32_t tail = segment_tail<EMIT>(P, i, tag, s, st, h, w, n);
     if (tail_out) *tail_out = tail;

@@ -103,7 +103,7 @@ k_write_segments(const WriteArgs A) {
     Writer w;
     w.out = A.out; w.base = base; w.seg = i; w.mode = P.mode;
     uint32_t first = count - tail;
-    if (s.kind == 1 || s.degenerate) { emit_straight(s, h, &w); first = 2u; }
+    if (s.kind == 1 || s.degenerate) first = emit_straight(s, h, st.fill, &w);
     segment_tail<true>(P, tag, s, st, h, first_seg, tag_n, pt_n, &w, first);
 }
 
@@ -387,7 +387,7 @@ k_write_walk(const WriteArgs A) {
         const Seg s = load_segment(P, i, P.tags[i]);
         Writer w;
         w.out = A.out; w.base = base; w.seg = i; w.mode = P.mode;
-        flatten_cubic<true>(P, s, h, &w);
+        flatten_cubic<true>(P, s, h, st.fill, &w);
     }
 }
 

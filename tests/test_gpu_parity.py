@@ -17,7 +17,7 @@ pytestmark = pytest.mark.gpu
 COUNT_PARITY = 0.999   # north_star
 COORD_TOL = 1e-3       # px, north_star: every end point of every record, whatever its kind
 ANGLE_TOL = 2e-5       # rad: fp32 evaluation of an angle of a few radians
-KIND_NAMES = {0: "offset", 1: "offset_rev", 2: "evolute", 3: "connector", 4: "join_outer", 5: "join_inner", 6: "cap"}
+KIND_NAMES = {0: "offset", 1: "offset_rev", 2: "evolute", 3: "connector", 4: "join_outer", 5: "join_inner", 6: "cap", 7: "close"}
 
 
 def check_coords(d, kind, what=""):
@@ -163,6 +163,47 @@ def test_parity_with_oracle(B, ctx, name, npaths, mode):
     g2 = gpu_run(B, ctx, sc, mode)
     assert np.array_equal(g.xy.view(np.uint32), g2.xy.view(np.uint32)) and np.array_equal(g.path_off, g2.path_off)
     assert np.array_equal(g.seg_count, g2.seg_count) and np.array_equal(g.angle.view(np.uint32), g2.angle.view(np.uint32))
+
+
+@pytest.mark.parametrize("every,mode", [(1, 0), (1, 1), (2, 0), (2, 1)])
+def test_parity_of_filled_paths(B, ctx, every, mode):
+    """SURVEY 8(f)-1, Alg. 1: config 2 (every segment kind and degeneracy) with every path, or every second path,
+    FILLED instead of stroked -- offset 0, one record chain per segment, the closing line of open subpaths -- element by
+    element against the oracle; stroked and filled paths mix in one call."""
+    sc = S.with_fill(S.make("c2", n_paths=600), every=every, offset=every - 1)
+    g = gpu_run(B, ctx, sc, mode, into=True)
+    r = oracle_run(sc, mode)
+    assert compare(sc, mode, g, r) >= COUNT_PARITY
+    assert ck.watertight_violations(g.xy, g.path_off) == 0
+    g2 = gpu_run(B, ctx, sc, mode)
+    assert np.array_equal(g.xy.view(np.uint32), g2.xy.view(np.uint32)) and np.array_equal(g.path_off, g2.path_off)
+    gh = gpu_run(B, ctx, sc, mode, host=True)
+    assert np.array_equal(g.xy.view(np.uint32), gh.xy.view(np.uint32))
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_filled_paths_do_not_depend_on_the_tiling(B, mode):
+    """Fills through the sub-tile path and the thread-per-segment walk: the same records, bit for bit."""
+    sc = S.with_fill(S.make("c2", n_paths=200), every=2)
+    dev = "cuda:0"
+    tags, pts, sty = B.scene_to_torch(sc, device=dev)
+    width = 4 if mode == 0 else 8
+    outs = []
+    for tiles in (1, 2, 8, 0):
+        c = B.sx_create(0)
+        try:
+            B.sx_set_option(c, B.SX_OPT_TILE_SEGMENTS, tiles)
+            poff = torch.empty(sc.n_paths + 1, dtype=torch.int64, device=dev)
+            total = B.sx_count(c, tags, pts, sty, sc.affine, sc.tolerance, mode, poff)
+            out = torch.full((total, width), float("nan"), dtype=torch.float32, device=dev)
+            B.sx_write(c, out, total, mode)
+            torch.cuda.synchronize()
+            assert B.sx_last_error(c) == 0
+            outs.append((out.cpu().numpy().view(np.uint32), poff.cpu().numpy()))
+        finally:
+            B.sx_destroy(c)
+    for o in outs[1:]:
+        assert np.array_equal(outs[0][0], o[0]) and np.array_equal(outs[0][1], o[1])
 
 
 @pytest.mark.parametrize("name,npaths,mode", [("c1", 64, 0), ("c2", 300, 1)])
