@@ -419,7 +419,34 @@ static int evolute_params(const ctx_t* c, const piece_t* p, float ta, float tb, 
     float kp = fabsf(p->k1) / (p->L * p->L);
     float n_f, wa = 0, wb = 0;
     int uniform = 1;
-    if (fabsf(kb - ka) < 0.015625f * fabsf(km)) {
+    int arc = (c->mode == MODE_ARC);
+    if (arc) {
+        /* Arc mode: the evolute is approximated by arcs with the metric of section 5 (L171: arcs follow the
+         * derivative of curvature with respect to arc length).  With sigma the spiral's arc length from the inflection
+         * (kappa = kappa' sigma) the evolute has arc length element |kappa'| / kappa^2 dsigma and curvature kappa^3 / |kappa'|,
+         * so d kappa_E / d s_E = 3 kappa^4 / |kappa'| and
+         *   n = int cbrt(3 kappa^4 / (|kappa'| 120 d)) |kappa'| / kappa^2 dsigma = 3^(4/3) |cbrt(sigma_b) - cbrt(sigma_a)| / cbrt(120 d):
+         * the subdivision points are uniform in cbrt(sigma), the inverse is cubing.  Reading R-20: the constant 120 of L171
+         * belongs to a curve of CONSTANT curvature derivative; the evolute's varies along an arc and the measured deviation
+         * with 120 reaches 1.41 d (tests/test_oracle_pins.py): 80 is used here, which keeps it below d. */
+        if (fabsf(kb - ka) < 0.015625f * fabsf(km)) {
+            /* nearly constant curvature: constant density cbrt(3 kappa'^2 / (120 d kappa^2)) per unit of the spiral's arc length */
+            n_f = ceilf((tb - ta) * p->L * cbrtf(3.0f * kp * kp / (80.0f * c->tol_fl * km * km)));
+        } else {
+            wa = cbrtf(fabsf(ka) / kp);
+            wb = cbrtf(fabsf(kb) / kp);
+            n_f = ceilf(4.326748710922225f * fabsf(wb - wa) / cbrtf(80.0f * c->tol_fl)); /* 3^(4/3) */
+            uniform = 0;
+        }
+        /* The metric assumes arcs of small turning.  The evolute turns with the spiral (its tangent is the spiral's
+         * normal): a short evolute of a strongly turning piece would be ONE arc of several radians.  At least one arc per
+         * pi/4 of turning over the range, then uniform in t (no arc turns by more than ~pi/2; reading R-20). */
+        {
+            float dphi = fabsf((tb - ta) * (0.5f * p->k1 * (ta + tb) + (p->k0 - 0.5f * p->k1)));
+            float n_phi = ceilf(dphi / QUARTER_PI);
+            if (n_phi > n_f) { n_f = n_phi; uniform = 1; }
+        }
+    } else if (fabsf(kb - ka) < 0.015625f * fabsf(km)) {
         n_f = ceilf((tb - ta) * p->L * sqrtf(fabsf(kp / km) / (8.0f * c->tol_fl)));
     } else {
         wa = sqrtf(fabsf(ka) / kp);
@@ -436,7 +463,7 @@ static int evolute_params(const ctx_t* c, const piece_t* p, float ta, float tb, 
         if (uniform) t = ta + fr * (tb - ta);
         else {
             float w = wa + fr * (wb - wa);
-            float kap = (ka < 0 ? -kp : kp) * w * w;
+            float kap = (ka < 0 ? -kp : kp) * w * w * (arc ? w : 1.0f); /* sigma = w^2 (lines, L195) or w^3 (arcs) */
             t = 0.5f + (kap * p->L - p->k0) / p->k1;
         }
         ts[i] = clampf(t, ta, tb);
@@ -483,7 +510,8 @@ static void side_records(ctx_t* c, const piece_t* p, float eta, reclist* out) {
                 for (int i = 0; i < ne; i++) {
                     v2d a = (i == 0) ? Ea : es_evolute(p, te[i]);
                     v2d b = (i == ne - 1) ? Eb : es_evolute(p, te[i + 1]);
-                    rl_push(out, a, b, 0, K_EVOLUTE);
+                    /* the evolute's tangent is the spiral's normal: it turns by the same angle (used in arc mode only) */
+                    rl_push(out, a, b, es_phi(p, te[i + 1]) - es_phi(p, te[i]), K_EVOLUTE);
                 }
             free(te);
             for (int i = n; i > 0; i--) /* reversed offset (L403, L191) */

@@ -19,7 +19,7 @@ struct PlanLite {
     float eta, tc;
     uint32_t seg, total;
     uint16_t n0, n1, ne;
-    uint8_t flags;   // bit 0 two ranges, 1 sup0, 2 sup1, 5 uniform evolute
+    uint8_t flags;   // bit 0 two ranges, 1 sup0, 2 sup1, 5 uniform evolute, 6 evolute parameters by cubing (arc mode)
     uint8_t rules;   // spacing rule (kRule*) of range 0 | of range 1 << 2
     float ua0, ub0, ua1, ub1, wa, wb, skp;
 };
@@ -27,7 +27,7 @@ SX_DEV PlanLite plan_pack(const SidePlan& s) {
     PlanLite q;
     q.eta = s.eta; q.tc = s.off[0].tb; q.seg = s.seg; q.total = (uint32_t)s.total;
     q.n0 = (uint16_t)s.off[0].n; q.n1 = (uint16_t)s.off[1].n; q.ne = (uint16_t)s.evo.n;
-    q.flags = (uint8_t)((s.nr == 2 ? 1u : 0u) | (s.sup[0] ? 2u : 0u) | (s.sup[1] ? 4u : 0u) | (s.evo.uniform ? 32u : 0u));
+    q.flags = (uint8_t)((s.nr == 2 ? 1u : 0u) | (s.sup[0] ? 2u : 0u) | (s.sup[1] ? 4u : 0u) | (s.evo.uniform ? 32u : 0u) | (s.evo.cube ? 64u : 0u));
     q.rules = (uint8_t)((uint32_t)s.off[0].rule | ((uint32_t)s.off[1].rule << 2));
     q.ua0 = s.off[0].ua; q.ub0 = s.off[0].ub; q.ua1 = s.off[1].ua; q.ub1 = s.off[1].ub;
     q.wa = s.evo.wa; q.wb = s.evo.wb; q.skp = s.evo.skp;
@@ -56,7 +56,7 @@ SX_DEV SidePlan plan_unpack(const PlanLite& q) {
 SX_DEV EvoPlan plan_evo(const PlanLite& q) {
     EvoPlan e;
     const bool second = (q.flags & 1u) && !(q.flags & 2u);  // two ranges and the first one regular
-    e.n = q.ne; e.uniform = (q.flags & 32u) != 0u;
+    e.n = q.ne; e.uniform = (q.flags & 32u) != 0u; e.cube = (q.flags & 64u) != 0u;
     e.ta = second ? q.tc : 0.0f; e.tb = second ? 1.0f : q.tc;
     e.wa = q.wa; e.wb = q.wb; e.skp = q.skp;
     return e;
@@ -121,7 +121,7 @@ SX_DEV void side_parts(const SidePlan& s, uint32_t side_slot, bool mirror, bool 
 #pragma unroll 1
             for (int c = 0; c < (s.cusp_a ? 0 : 2); c++) push(1u, 0, false, 0u, 0u, false, kConnector, ca, ea);
 #pragma unroll 1
-            for (int c = 0; c < 2; c++) push((uint32_t)s.evo.n, 0, false, 2u, 0u, false, kEvolute, ea, eb);
+            for (int c = 0; c < 2; c++) push((uint32_t)s.evo.n, 0, false, 2u, 0u, true, kEvolute, ea, eb);   // (arc mode: the evolute turns with the spiral)
             push((uint32_t)o.n, o.n, true, 1u, (uint32_t)r, true, kOffsetRev, cb, ca);  // L403, L191
 #pragma unroll 1
             for (int c = 0; c < (s.cusp_b ? 0 : 2); c++) push(1u, 0, false, 0u, 0u, false, kConnector, eb, cb);

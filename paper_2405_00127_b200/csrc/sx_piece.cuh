@@ -226,7 +226,7 @@ SX_DEV V2 es_evolute(const Piece& p, const Spiral& sp, float t) { return normal_
 
 // ---------------------------------------------------------------- subdivision plans
 struct OffPlan { int n; int rule; float ta, tb, ua, ub; };   // rule: how the interior parameters are spaced (kRule*)
-struct EvoPlan { int n; bool uniform; float ta, tb, wa, wb, skp; };
+struct EvoPlan { int n; bool uniform, cube; float ta, tb, wa, wb, skp; };   // cube: arc mode, the parameters are uniform in cbrt(sigma)
 
 // offset range [ta,tb] of side eta (sections 4, 5): number of records and what the parameters need
 SX_DEV OffPlan offset_plan(const Piece& p, float eta, float ta, float tb, int mode, float tol_fl) {
@@ -286,15 +286,32 @@ SX_DEV float offset_t(const Piece& p, const OffPlan& o, float eta, int i) {
     return clampf(t, o.ta, o.tb);
 }
 
-// evolute range [ta,tb]: density |sigma|^-1/2, integral 2 sqrt(sigma), inverse squaring (L195)
-SX_DEV EvoPlan evolute_plan(const Piece& p, float ta, float tb, float tol_fl) {
+// evolute range [ta,tb].  Lines: density |sigma|^-1/2, integral 2 sqrt(sigma), inverse squaring (L195).  Arcs (SURVEY
+// 8(f)-1): the metric of section 5 (L171) applied to the evolute -- arc length element |kappa'| / kappa^2 dsigma, curvature
+// kappa^3 / |kappa'|, d kappa_E / d s_E = 3 kappa^4 / |kappa'| -- gives n = 3^(4/3) |cbrt(sigma_b) - cbrt(sigma_a)| / cbrt(80 d),
+// uniform in cbrt(sigma), inverse cubing (reading R-20: 80, not 120 -- the evolute's curvature derivative varies along an arc).
+SX_DEV EvoPlan evolute_plan(const Piece& p, float ta, float tb, int mode, float tol_fl) {
     EvoPlan e;
-    e.ta = ta; e.tb = tb; e.wa = 0.0f; e.wb = 0.0f; e.uniform = true;
+    e.ta = ta; e.tb = tb; e.wa = 0.0f; e.wb = 0.0f; e.uniform = true; e.cube = mode == kModeArc;
     float ka = es_kappa(p, ta), kb = es_kappa(p, tb), km = 0.5f * (ka + kb);
     float kp = (fabsf(p.k1)) / (p.L * p.L);
     e.skp = ka < 0.0f ? -kp : kp;
     float n_f;
-    if (fabsf(kb - ka) < 0.015625f * fabsf(km)) {
+    const bool flat = fabsf(kb - ka) < 0.015625f * fabsf(km);
+    if (mode == kModeArc) {
+        if (flat) {
+            n_f = ceilf((tb - ta) * p.L * cbrt_fast(div_fast(3.0f * kp * kp, 80.0f * tol_fl * km * km)));
+        } else {
+            e.wa = cbrtf(fabsf(ka) / kp);
+            e.wb = cbrtf(fabsf(kb) / kp);
+            n_f = ceilf(div_fast(4.326748710922225f * fabsf(e.wb - e.wa), cbrt_fast(80.0f * tol_fl)));
+            e.uniform = false;
+        }
+        // at least one arc per pi/4 of turning over the range (the evolute turns with the spiral), then uniform in t
+        const float dphi = fabsf((tb - ta) * (0.5f * p.k1 * (ta + tb) + (p.k0 - 0.5f * p.k1)));
+        const float n_phi = ceilf(dphi / kQuarterPi);
+        if (n_phi > n_f) { n_f = n_phi; e.uniform = true; }
+    } else if (flat) {
         n_f = ceilf((tb - ta) * p.L * sqrt_fast(div_fast(fabsf(div_fast(kp, km)), 8.0f * tol_fl)));
     } else {
         e.wa = sqrtf(fabsf(ka) / kp);
@@ -310,7 +327,7 @@ SX_DEV float evolute_t(const Piece& p, const EvoPlan& e, int i) {
     if (e.uniform) t = e.ta + fr * (e.tb - e.ta);
     else {
         float w = e.wa + fr * (e.wb - e.wa);
-        float kap = e.skp * w * w;
+        float kap = e.skp * w * w * (e.cube ? w : 1.0f);   // sigma = w^2 (lines) or w^3 (arcs)
         t = 0.5f + (kap * p.L - p.k0) / (p.k1);
     }
     return clampf(t, e.ta, e.tb);
@@ -360,7 +377,7 @@ __device__ __noinline__ SidePlan side_plan(const Piece& p, float eta, int mode, 
     if (first_sup || s.nr == 2) {
         s.cusp_a = (ea != 0.0f);
         s.cusp_b = (eb != 1.0f);
-        s.evo = evolute_plan(p, ea, eb, tol_fl);
+        s.evo = evolute_plan(p, ea, eb, mode, tol_fl);
         s.total += 2 * s.evo.n + (s.cusp_a ? 0 : 2) + (s.cusp_b ? 0 : 2);
     }
     return s;

@@ -69,11 +69,14 @@ SX_DEV uint32_t piece_side(const Piece& p, const Spiral& z, float eta, bool mirr
             if (!s.cusp_a) { k.put(idx, Oa, Ea, 0.0f, kConnector); k.put(idx + 1, Oa, Ea, 0.0f, kConnector); idx += 2; }  // "output twice", L197
             const int ne = s.evo.n;
             V2 pe = Ea;
+            float te_prev = s.evo.ta;
             for (int i = 0; i < ne; i++) {
-                V2 b = (i == ne - 1) ? Eb : es_evolute(p, z, evolute_t(p, s.evo, i + 1));
-                k.put(idx + i, pe, b, 0.0f, kEvolute);
-                k.put(idx + ne + i, pe, b, 0.0f, kEvolute);
-                pe = b;
+                const float te = (i == ne - 1) ? s.evo.tb : evolute_t(p, s.evo, i + 1);
+                V2 b = (i == ne - 1) ? Eb : es_evolute(p, z, te);
+                const float ang = arc ? es_dphi(p, te_prev, te) : 0.0f;   // the evolute's tangent is the spiral's normal
+                k.put(idx + i, pe, b, ang, kEvolute);
+                k.put(idx + ne + i, pe, b, ang, kEvolute);
+                pe = b; te_prev = te;
             }
             idx += 2 * ne;
             V2 prev = Ob;  // reversed offset (L403, L191)
