@@ -93,7 +93,7 @@ typedef struct {
 enum {
     SX_KIND_OFFSET = 0,     /* parallel curve, regular range                                          */
     SX_KIND_OFFSET_REV = 1, /* parallel curve over a super-critical range, reversed (L191, L403)      */
-    SX_KIND_EVOLUTE = 2,    /* evolute, output twice (L197)                                           */
+    SX_KIND_EVOLUTE = 2,    /* evolute, output twice (L197); arc mode: arcs by the metric of L171 (R-20) */
     SX_KIND_CONNECTOR = 3,  /* offset <-> evolute connecting line, output twice (L197)                */
     SX_KIND_JOIN_OUTER = 4,
     SX_KIND_JOIN_INNER = 5, /* through the vertex (strong correctness, L35)                           */
