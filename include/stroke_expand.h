@@ -238,6 +238,14 @@ sx_status sx_kernel_times(sx_ctx* ctx, float* h_ms4);
  * roofline. */
 sx_status sx_measure_issue_peaks(int32_t device, double* h_out3);
 
+/* Probes of single device functions of the kernels, for the tests (host buffers, host-synchronous, one thread per item):
+ *   SX_EVAL_ATAN2       h_in[2 i] = y, h_in[2 i + 1] = x  ->  the kernels' angle function (reading R-17 of DESIGN.md: the fp32
+ *                       value nearest to atan2(y, x), by an own double-precision evaluation)
+ *   SX_EVAL_NODE_ERROR  h_in[9 i ..] = u0.x u0.y u1.x u1.y |q0| |q1| chord.x chord.y dt  ->  the decision-grade error estimate
+ *                       of section 7.1 that Alg. 2's accept / split test uses */
+enum { SX_EVAL_ATAN2 = 0, SX_EVAL_NODE_ERROR = 1 };
+sx_status sx_eval(int32_t device, int32_t what, const float* h_in, float* h_out, uint64_t n);
+
 /* Number of kernel launches the library has issued on this context so far. */
 uint64_t sx_launch_count(const sx_ctx* ctx);
 

@@ -24,7 +24,7 @@ ARC_DTYPE = np.dtype([("x0", "<f4"), ("y0", "<f4"), ("x1", "<f4"), ("y1", "<f4")
 SX_OPT_KEEP_SEGMENT_INFO, SX_OPT_TILE_SEGMENTS, SX_OPT_TIME_KERNELS = 1, 2, 3
 
 EXPORTS = ["sx_create", "sx_destroy", "sx_count", "sx_write", "stroke_expand", "stroke_expand_into", "stroke_expand_host",
-           "sx_bin_lines", "sx_segment_info", "sx_last_error", "sx_set_option", "sx_call_stats", "sx_kernel_times", "sx_measure_issue_peaks", "sx_launch_count",
+           "sx_bin_lines", "sx_segment_info", "sx_last_error", "sx_set_option", "sx_call_stats", "sx_kernel_times", "sx_measure_issue_peaks", "sx_eval", "sx_launch_count",
            "sx_strerror"]
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
@@ -58,6 +58,7 @@ def lib():
         L.sx_last_error.argtypes = [vp, vp]
         L.sx_set_option.argtypes = [vp, i32, u64]
         L.sx_call_stats.argtypes = [vp, C.POINTER(u64), vp]
+        L.sx_eval.argtypes = [C.c_int32, C.c_int32, vp, vp, u64]
         L.sx_bin_lines.argtypes = [vp, vp, u64, C.c_uint32, C.c_uint32, vp, vp, u64, C.POINTER(u64), vp]
         L.sx_kernel_times.argtypes = [vp, C.POINTER(C.c_float)]
         L.sx_measure_issue_peaks.argtypes = [i32, C.POINTER(C.c_double)]
@@ -283,6 +284,19 @@ def sx_measure_issue_peaks(device=0):
     out = (C.c_double * 3)()
     _check(lib().sx_measure_issue_peaks(int(device), out), "sx_measure_issue_peaks")
     return dict(fp32_ffma=float(out[0]), fp32_mix=float(out[1]), mufu=float(out[2]))
+
+
+SX_EVAL_ATAN2, SX_EVAL_NODE_ERROR = 0, 1
+
+
+def sx_eval(what, values, device=0):
+    """Probe of one device function of the kernels (tests): values float32 numpy [n, 2] (atan2: y, x) or [n, 9] (node error:
+    u0, u1, |q0|, |q1|, chord, dt); returns float32 numpy [n]."""
+    v = np.ascontiguousarray(values, dtype=np.float32)
+    n = v.shape[0]
+    out = np.zeros(n, dtype=np.float32)
+    _check(lib().sx_eval(int(device), int(what), C.c_void_p(v.ctypes.data), C.c_void_p(out.ctypes.data), n), "sx_eval")
+    return out
 
 
 def sx_launch_count(ctx):

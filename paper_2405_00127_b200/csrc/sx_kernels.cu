@@ -539,6 +539,37 @@ sx_status sx_kernel_times(sx_ctx* c, float* h_ms4) {
     return SX_OK;
 }
 
+// probes of single device functions (tests): one thread per item
+__global__ void k_eval(int what, const float* in, float* out, uint64_t n) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    if (what == SX_EVAL_ATAN2) {
+        out[i] = sx::atan2_r(in[2 * i], in[2 * i + 1]);
+    } else if (what == SX_EVAL_NODE_ERROR) {
+        const float* v = in + 9 * i;
+        out[i] = sx::node_error(sx::v2(v[0], v[1]), sx::v2(v[2], v[3]), v[4], v[5], sx::v2(v[6], v[7]), v[8]);
+    }
+}
+
+sx_status sx_eval(int32_t device, int32_t what, const float* h_in, float* h_out, uint64_t n) {
+    if (!h_in || !h_out || (what != SX_EVAL_ATAN2 && what != SX_EVAL_NODE_ERROR)) return SX_E_INVALID_ARG;
+    if (n == 0) return SX_OK;
+    const uint64_t per = what == SX_EVAL_ATAN2 ? 2 : 9;
+    SX_CUDA(cudaSetDevice(device));
+    float *d_in = nullptr, *d_out = nullptr;
+    SX_CUDA(cudaMalloc(&d_in, n * per * sizeof(float)));
+    cudaError_t e = cudaMalloc(&d_out, n * sizeof(float));
+    if (e == cudaSuccess) e = cudaMemcpy(d_in, h_in, n * per * sizeof(float), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        k_eval<<<(unsigned)((n + 255) / 256), 256>>>(what, d_in, d_out, n);
+        e = cudaMemcpy(h_out, d_out, n * sizeof(float), cudaMemcpyDeviceToHost);
+    }
+    cudaFree(d_in);
+    cudaFree(d_out);
+    if (e != cudaSuccess) { g_last_cuda = e; return SX_E_CUDA; }
+    return SX_OK;
+}
+
 sx_status sx_measure_issue_peaks(int32_t device, double* h_out3) {
     if (!h_out3) return SX_E_INVALID_ARG;
     cudaError_t e = sx::measure_issue_peaks(device, h_out3);

@@ -194,11 +194,11 @@ SX_DEV void eval_cubic(const Seg& s, float t, float dt, V2* pos, float* qmag, V2
 SX_DEV float rcp_fast(float a) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
 SX_DEV float rsqrt_fast(float a) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
 
-// (x, y) finite and not both zero
+// 1e-30 < max(|x|, |y|) < 1e30 (the kernels' arguments are cross / dot products of unit vectors)
 SX_DEV float atan2_r_core(float y, float x) {
     const float ax = fabsf(x), ay = fabsf(y);
     const float mxf = fmaxf(ax, ay), mnf = fminf(ax, ay);
-    const float kf = rintf(4.0f * mnf * rcp_fast(mxf));   // 0 .. 4
+    const float kf = rintf(4.0f * (mnf * rcp_fast(mxf)));   // 0 .. 4
     const double c = 0.25 * (double)kf;
     // atan(k / 4), k = 0 .. 4
     const double at = kf < 0.5f ? 0.0 : (kf < 1.5f ? 0.24497866312686415417 : (kf < 2.5f ? 0.46364760900080611621 : (kf < 3.5f ? 0.64350110879328438680 : 0.78539816339744830962)));
@@ -229,7 +229,7 @@ SX_DEV float atan2_r_core(float y, float x) {
 // two dependent chains interleave)
 __device__ __noinline__ float atan2_r(float y, float x) {
     const float m = fmaxf(fabsf(x), fabsf(y));
-    if (!(m > 0.0f) || !(m < INFINITY)) return (float)atan2((double)y, (double)x);   // zeros, infinities, NaN: the library's rules
+    if (!(m > 1e-30f) || !(m < 1e30f)) return (float)atan2((double)y, (double)x);   // zeros, denormals, huge, infinities, NaN: the library
     return atan2_r_core(y, x);
 }
 
