@@ -420,9 +420,10 @@ k_count(const CountArgs A) {
                         // so that the warps of the simple writer see (mostly) one kind
                         const uint32_t rank = lf.ab & 0x3fffffffu, cls = lf.ab >> 30;
                         const uint32_t pos = cls == 1u ? base_simple + rank : (cls == 2u ? base_simple + n_simple - 1u - rank : A.leaf_cap - 1u - (base_other + rank));
-                        uint4* dst = reinterpret_cast<uint4*>(A.leaves + pos);
-                        dst[0] = make_uint4(r.seg, r.key, r.n, r.rel);
-                        dst[1] = make_uint4(__float_as_uint(r.k0), __float_as_uint(r.k1), __float_as_uint(r.L), __float_as_uint(r.h));
+                        // (one 256-bit store: a full 32-byte sector; the leaf buffer is the context's own, aligned allocation)
+                        asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(A.leaves + pos), "r"(r.seg), "r"(r.key), "r"(r.n), "r"(r.rel),
+                                     "r"(__float_as_uint(r.k0)), "r"(__float_as_uint(r.k1)), "r"(__float_as_uint(r.L)), "r"(__float_as_uint(r.h))
+                                     : "memory");
                     }
                 }
             }

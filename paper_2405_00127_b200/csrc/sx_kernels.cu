@@ -207,6 +207,7 @@ static sx_status run_write(sx_ctx* c, void* d_out_records, uint64_t cap_records,
     if (n == 0) return SX_OK;
     c->W.out = static_cast<float4*>(d_out_records);
     c->W.cap_records = cap_records;
+    c->W.wide = (reinterpret_cast<uintptr_t>(d_out_records) & 31u) == 0u ? 1u : 0u;
     // the four writers side by side: the general writer (the long one on evolute-heavy scenes) on the caller's stream, the
     // others on the context's side streams, forked from and joined to the caller's stream with events
     SX_CUDA(cudaEventRecord(c->fork, s));

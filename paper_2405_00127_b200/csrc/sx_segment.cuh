@@ -12,18 +12,31 @@
 namespace sx {
 
 // ---------------------------------------------------------------- record sink
+// a 32-byte arc record in ONE 256-bit store (sm_100: STG.256; a full 32-byte sector instead of two half sectors) when the
+// caller's buffer is 32-byte aligned, else as two 16-byte stores
+SX_DEV void store_arc(float4* out, uint64_t rec, bool wide, float4 a, float4 b) {
+    if (wide) {
+        asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(out + 2 * rec), "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w),
+                     "f"(b.x), "f"(b.y), "f"(b.z), "f"(b.w)
+                     : "memory");
+    } else {
+        out[2 * rec] = a;
+        out[2 * rec + 1] = b;
+    }
+}
+
 struct Writer {
     float4* out;     // sx_line[] (1 float4 per record) or sx_arc[] (2 float4 per record)
     uint64_t base;   // index of the segment's first record
     uint32_t seg;
     int mode;
+    bool wide;       // arc records by 256-bit stores (the buffer is 32-byte aligned)
     SX_DEV void put(uint32_t idx, V2 a, V2 b, float angle, uint32_t kind) const {
         uint64_t r = base + idx;
         if (mode == kModeLine) {
             out[r] = make_float4(a.x, a.y, b.x, b.y);
         } else {
-            out[2 * r] = make_float4(a.x, a.y, b.x, b.y);
-            out[2 * r + 1] = make_float4(angle, u2f(seg), u2f(kind), 0.0f);
+            store_arc(out, r, wide, make_float4(a.x, a.y, b.x, b.y), make_float4(angle, u2f(seg), u2f(kind), 0.0f));
         }
     }
 };

@@ -37,6 +37,7 @@ struct WriteArgs {
     float4* out;
     uint64_t cap_records;
     uint32_t* err;
+    uint32_t wide;   // the output buffer is 32-byte aligned: arc records go out as 256-bit stores
 };
 
 SX_DEV uint32_t n_simple_leaves(const WriteArgs& A) {
@@ -48,7 +49,9 @@ SX_DEV uint32_t n_other_leaves(const WriteArgs& A) {
     return reserved < valid ? reserved : valid;
 }
 SX_DEV LeafRec load_leaf(const LeafRec* p) {
-    const uint4 a = __ldg(reinterpret_cast<const uint4*>(p)), b = __ldg(reinterpret_cast<const uint4*>(p) + 1);
+    // (one 256-bit load, sm_100)
+    uint4 a, b;
+    asm volatile("ld.global.nc.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];" : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w), "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(p));
     LeafRec r;
     r.seg = a.x; r.key = a.y; r.n = a.z; r.rel = a.w;
     r.k0 = __uint_as_float(b.x); r.k1 = __uint_as_float(b.y); r.L = __uint_as_float(b.z); r.h = __uint_as_float(b.w);
@@ -73,13 +76,9 @@ SX_DEV void leaf_piece(const Params& P, const LeafRec& r, Piece& p) {
     p.k0 = r.k0; p.k1 = r.k1; p.L = r.L;
 }
 
-SX_DEV void put_record(float4* out, bool arc, uint64_t rec, V2 a, V2 b, float angle, uint32_t seg, uint32_t kind) {
-    if (!arc) {
-        out[rec] = make_float4(a.x, a.y, b.x, b.y);
-    } else {
-        out[2 * rec] = make_float4(a.x, a.y, b.x, b.y);
-        out[2 * rec + 1] = make_float4(angle, f_of_u(seg), f_of_u(kind), 0.0f);
-    }
+SX_DEV void put_record(float4* out, bool arc, bool wide, uint64_t rec, V2 a, V2 b, float angle, uint32_t seg, uint32_t kind) {
+    if (!arc) out[rec] = make_float4(a.x, a.y, b.x, b.y);
+    else store_arc(out, rec, wide, make_float4(a.x, a.y, b.x, b.y), make_float4(angle, f_of_u(seg), f_of_u(kind), 0.0f));
 }
 
 // ---------------------------------------------------------------- straight segments, joins, caps
@@ -101,7 +100,7 @@ k_write_segments(const WriteArgs A) {
     load_style(P, path, &st, &h);
     const Seg s = load_segment_at(P, pt, tag);
     Writer w;
-    w.out = A.out; w.base = base; w.seg = i; w.mode = P.mode;
+    w.out = A.out; w.base = base; w.seg = i; w.mode = P.mode; w.wide = A.wide != 0u;
     uint32_t first = count - tail;
     if (s.kind == 1 || s.degenerate) first = emit_straight(s, h, st.fill, &w);
     segment_tail<true>(P, tag, s, st, h, first_seg, tag_n, pt_n, &w, first);
@@ -188,7 +187,7 @@ k_write_simple(const WriteArgs A) {
             if (i < nrec) { t = offset_t(p, o, eta, (int)i); cur = normal_point(p, z, t, eta); }
             else cur = end_vertex(p, kEndT1, eta, nocusp, &t);
             const uint64_t rec = base + (side ? nrec - i : i - 1u);
-            put_record(A.out, arc, rec, side ? cur : prev, side ? prev : cur, (side ? es_dphi(p, t, tp) : es_dphi(p, tp, t)) + 0.0f, r.seg, kind);
+            put_record(A.out, arc, A.wide != 0u, rec, side ? cur : prev, side ? prev : cur, (side ? es_dphi(p, t, tp) : es_dphi(p, tp, t)) + 0.0f, r.seg, kind);
             prev = cur; tp = t;
         }
     }
@@ -361,7 +360,7 @@ k_write_general(const WriteArgs A) {
                     else Av = end_vertex(pc, (pt.info >> 16) & 7u, sp.eta, cusp, &tA);
                     if (e_int) { const float4 q = W.ring[(uint32_t)v_end & (uint32_t)(kRing - 1)]; Bv = v2(q.x, q.y); tB = q.z; }
                     else Bv = end_vertex(pc, (pt.info >> 19) & 7u, sp.eta, cusp, &tB);
-                    put_record(out, arc, pt.base + m, Av, Bv, (pt.info & 2048u) ? es_dphi(pc, tA, tB) + 0.0f : 0.0f, sp.seg, (pt.info >> 12) & 15u);
+                    put_record(out, arc, A.wide != 0u, pt.base + m, Av, Bv, (pt.info & 2048u) ? es_dphi(pc, tA, tB) + 0.0f : 0.0f, sp.seg, (pt.info >> 12) & 15u);
                 }
                 __syncwarp();
             }
@@ -386,7 +385,7 @@ k_write_walk(const WriteArgs A) {
         load_style(P, P.path_idx[i], &st, &h);
         const Seg s = load_segment(P, i, P.tags[i]);
         Writer w;
-        w.out = A.out; w.base = base; w.seg = i; w.mode = P.mode;
+        w.out = A.out; w.base = base; w.seg = i; w.mode = P.mode; w.wide = A.wide != 0u;
         flatten_cubic<true>(P, s, h, st.fill, &w);
     }
 }
