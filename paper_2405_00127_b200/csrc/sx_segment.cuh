@@ -282,33 +282,31 @@ SX_DEV bool load_style(const Params& P, uint32_t path, Style* st, float* h) {
 // segment of an open subpath, [end cap][start cap]
 // tag_n, pt_n: tag and point offset of segment i + 1, first: sp_first[i] -- loaded by the caller together with the
 // segment's own scan results, so that the partner's points are one dependent load away, not two
+// the tail with the partner's start point W and start tangent T1 given (the join partner, or the subpath's first segment
+// for the caps and for the closing line of a fill)
+template <bool EMIT>
+SX_DEV uint32_t segment_tail_given(const Params& P, uint32_t tag, const Seg& s, const Style& st, float h, V2 W, V2 T1, const Writer* w, uint32_t first) {
+    const bool sp_end = ((tag >> 2) | (tag >> 4)) & 1u;
+    const bool closed = (tag >> 7) & 1u;
+    if (st.fill) {   // no joins, no caps: the line that closes an open subpath (always emitted: counts follow the tags)
+        if (!sp_end || closed) return 0u;
+        if (EMIT) w->put(first, s.P3, W, 0.0f, kClose);
+        return 1u;
+    }
+    if (!sp_end || closed) return emit_join<EMIT>(P, st, s.P3, s.te, W, T1, h, w, first);
+    uint32_t n = emit_cap<EMIT>(P, st, s.P3, s.te, h, w, first);
+    n += emit_cap<EMIT>(P, st, W, v2(-T1.x, -T1.y), h, w, first + n);
+    return n;
+}
 template <bool EMIT>
 SX_DEV uint32_t segment_tail(const Params& P, uint32_t tag, const Seg& s, const Style& st, float h, uint32_t first_seg, uint32_t tag_n,
                              uint32_t pt_n, const Writer* w, uint32_t first) {
-    bool sp_end = ((tag >> 2) | (tag >> 4)) & 1u;
-    bool closed = (tag >> 7) & 1u;
-    uint32_t n = 0;
-    if (st.fill) {   // no joins, no caps: the line that closes an open subpath (always emitted: counts follow the tags)
-        if (!sp_end || closed) return 0u;
-        if (EMIT) {
-            V2 F, Tf;
-            load_segment_start(P, first_seg, &F, &Tf);
-            w->put(first, s.P3, F, 0.0f, kClose);
-        }
-        return 1u;
-    }
-    if (!sp_end || closed) {
-        V2 W, T1;
-        if (sp_end) load_segment_start(P, first_seg, &W, &T1);
-        else load_segment_start_at(P, pt_n, tag_n, &W, &T1);
-        n += emit_join<EMIT>(P, st, s.P3, s.te, W, T1, h, w, first);
-    } else {
-        V2 F, Tf;
-        load_segment_start(P, first_seg, &F, &Tf);
-        n += emit_cap<EMIT>(P, st, s.P3, s.te, h, w, first);
-        n += emit_cap<EMIT>(P, st, F, v2(-Tf.x, -Tf.y), h, w, first + n);
-    }
-    return n;
+    const bool sp_end = ((tag >> 2) | (tag >> 4)) & 1u;
+    const bool closed = (tag >> 7) & 1u;
+    V2 W = v2(0.0f, 0.0f), T1 = v2(1.0f, 0.0f);
+    if (!sp_end) load_segment_start_at(P, pt_n, tag_n, &W, &T1);
+    else if (!st.fill || !closed) load_segment_start(P, first_seg, &W, &T1);
+    return segment_tail_given<EMIT>(P, tag, s, st, h, W, T1, w, first);
 }
 template <bool EMIT>
 SX_DEV uint32_t segment_tail(const Params& P, uint32_t i, uint32_t tag, const Seg& s, const Style& st, float h, const Writer* w, uint32_t first) {

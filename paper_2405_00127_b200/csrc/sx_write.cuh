@@ -86,24 +86,32 @@ __global__ void __launch_bounds__(kWrThreads)
 k_write_segments(const WriteArgs A) {
     const Params& P = A.P;
     const uint32_t i = blockIdx.x * (uint32_t)kWrThreads + threadIdx.x;
-    if (i >= P.n_tags) return;
-    // first level of loads in one batch (the kernel is bound by the latency of its dependent loads): the segment's own scan
-    // results, its successor's tag and point offset (the join partner of every segment that does not end a subpath)
-    const uint32_t jn = i + 1u < P.n_tags ? i + 1u : i;
-    const uint32_t count = A.seg_count[i], tail = A.seg_tail[i], tag = P.tags[i], pt = P.pt_off[i], path = P.path_idx[i], first_seg = P.sp_first[i];
-    const uint32_t tag_n = P.tags[jn], pt_n = P.pt_off[jn];
-    const uint64_t base = A.seg_off[i];
-    if (count == 0u) return;   // width <= 0, or a malformed stream
-    if (base + count > A.cap_records) { atomicOr(A.err, kErrCapacity); return; }   // nothing of the segment is written
+    const bool in = i < P.n_tags;
+    const uint32_t ii = in ? i : P.n_tags - 1u;
+    // first level of loads in one batch (the kernel is bound by the latency of its dependent loads)
+    const uint32_t count = in ? A.seg_count[ii] : 0u, tail = A.seg_tail[ii], tag = P.tags[ii], pt = P.pt_off[ii], path = P.path_idx[ii], first_seg = P.sp_first[ii];
+    const uint64_t base = A.seg_off[ii];
     Style st;
     float h;
     load_style(P, path, &st, &h);
     const Seg s = load_segment_at(P, pt, tag);
+    // the join partner of a segment that does not end its subpath is the next segment: the next lane's start point and start
+    // tangent (the same load_segment_at, hence the bits the partner itself uses); only the warp's last lane and the segments
+    // that close a subpath or carry the caps load theirs
+    const int lane = threadIdx.x & 31;
+    V2 W, T1;
+    W.x = __shfl_down_sync(kFull, s.P0.x, 1); W.y = __shfl_down_sync(kFull, s.P0.y, 1);
+    T1.x = __shfl_down_sync(kFull, s.ts.x, 1); T1.y = __shfl_down_sync(kFull, s.ts.y, 1);
+    if (count == 0u) return;   // width <= 0, a malformed stream, or beyond the end
+    if (base + count > A.cap_records) { atomicOr(A.err, kErrCapacity); return; }   // nothing of the segment is written
+    const bool sp_end = ((tag >> 2) | (tag >> 4)) & 1u;
+    if (sp_end) { if (!st.fill || !((tag >> 7) & 1u)) load_segment_start(P, first_seg, &W, &T1); }
+    else if (lane == 31) load_segment_start(P, i + 1u, &W, &T1);
     Writer w;
     w.out = A.out; w.base = base; w.seg = i; w.mode = P.mode; w.wide = A.wide != 0u;
     uint32_t first = count - tail;
     if (s.kind == 1 || s.degenerate) first = emit_straight(s, h, st.fill, &w);
-    segment_tail<true>(P, tag, s, st, h, first_seg, tag_n, pt_n, &w, first);
+    segment_tail_given<true>(P, tag, s, st, h, W, T1, &w, first);
 }
 
 // ---------------------------------------------------------------- simple leaves: thread per (leaf, side)
