@@ -95,8 +95,8 @@ struct __align__(16) CtSeg {
     uint32_t pad;
 };
 struct CtLeaf {
-    uint32_t ab;         // point indices a | b << 16 (phases B, C); rank within the class | class << 30 (phase D)
-    uint32_t seg_slot;   // segment (tile-local) | tree slot << 8
+    uint32_t w;          // bytes: [0] point a, [1] point b (phases B, C1) -> simple flags of the two sides (C1, C2) -> rank within the
+                         // class, class (C3, D); [2] segment (tile-local); [3] tree slot
     uint32_t key;
     float k0, k1, L;
     uint16_t n[2];       // n_minus, n_plus
@@ -106,8 +106,7 @@ struct CtWarp {
     float4 pts[kCtPointCap];       // x, y local position; z, w unit tangent
     float qmag[kCtPointCap];
     uint32_t qx[kCtQueueCap];      // t0_u | level << 20
-    uint32_t qy[kCtQueueCap];      // point indices a | b << 16
-    uint32_t qz[kCtQueueCap];      // seg | tree slot << 8
+    uint32_t qy[kCtQueueCap];      // bytes: point a, point b, segment (tile-local), tree slot
     uint32_t acc[kCtTreeCap];
     uint8_t parent[kCtTreeCap];
     CtLeaf leaf[kCtLeafCap];
@@ -247,8 +246,7 @@ k_count(const CountArgs A) {
             if (my_curve) {
                 const uint32_t q = __popc(root_mask & lt);
                 S.qx[q] = 0u;
-                S.qy[q] = (uint32_t)(2 * lane) | ((uint32_t)(2 * lane + 1) << 16);
-                S.qz[q] = (uint32_t)lane | ((uint32_t)lane << 8);
+                S.qy[q] = (uint32_t)(2 * lane) | ((uint32_t)(2 * lane + 1) << 8) | ((uint32_t)lane << 16) | ((uint32_t)lane << 24);
             }
             __syncwarp();
             // join / cap record counts (partners from the tile's records)
@@ -266,14 +264,14 @@ k_count(const CountArgs A) {
             while (q_head != q_tail && !overflow) {
                 const uint32_t n_round = min(q_tail - q_head, 32u);
                 bool accept = false, push = false, bad = false;
-                uint32_t qx = 0, qy = 0, qz = 0;
+                uint32_t qx = 0, qy = 0;
                 float4 mid = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
                 float mid_q = 0.0f;
                 if ((uint32_t)lane < n_round) {
                     const uint32_t qi = (q_head + (uint32_t)lane) & (uint32_t)(kCtQueueCap - 1);
-                    qx = S.qx[qi]; qy = S.qy[qi]; qz = S.qz[qi];
+                    qx = S.qx[qi]; qy = S.qy[qi];
                     const uint32_t t0_u = qx & 0xfffffu, level = qx >> 20;
-                    const uint32_t pa_i = qy & 0xffffu, pb_i = qy >> 16;
+                    const uint32_t pa_i = qy & 0xffu, pb_i = (qy >> 8) & 0xffu;
                     const float4 a = S.pts[pa_i], b = S.pts[pb_i];
                     const float dt = __uint_as_float((127u - level) << 23);
                     const float err = node_error(v2(a.z, a.w), v2(b.z, b.w), S.qmag[pa_i], S.qmag[pb_i], v2(b.x, b.y) - v2(a.x, a.y), dt);
@@ -283,7 +281,7 @@ k_count(const CountArgs A) {
                         // split: the mid point is evaluated once, for both children (Alg. 2 L369 with the rule of L251)
                         push = true;
                         float q2;
-                        mid = cubic_point(seg_of(S.seg[qz & 0xffu]), (float)t0_u * dt + 0.5f * dt, &mid_q, &q2);
+                        mid = cubic_point(seg_of(S.seg[(qy >> 16) & 0xffu]), (float)t0_u * dt + 0.5f * dt, &mid_q, &q2);
                         bad = q2 < kEpsQ2;   // zero derivative inside the curve: the visiting order matters (L251)
                     }
                 }
@@ -294,22 +292,22 @@ k_count(const CountArgs A) {
                     q_tail + 2u * n_push - q_head > (uint32_t)kCtQueueCap) { overflow = true; break; }
                 if (accept) {
                     CtLeaf& lf = S.leaf[n_leaf + __popc(m_acc & lt)];
-                    lf.ab = qy; lf.seg_slot = qz; lf.key = (qx & 0xffffu) | ((qx >> 20) << 16);
+                    lf.w = qy; lf.key = (qx & 0xffffu) | ((qx >> 20) << 16);
                 }
                 if (push) {
                     // children: one point, two tree slots, two queue entries per split
                     const uint32_t rank = __popc(m_push & lt);
                     const uint32_t k = n_split + rank;
                     const uint32_t pm = 2u * (uint32_t)kCtTile + k, ts = (uint32_t)kCtTile + 2u * k;
-                    const uint32_t sl = qz & 0xffu, slot = qz >> 8;
+                    const uint32_t slot = qy >> 24;
                     S.pts[pm] = mid;
                     S.qmag[pm] = mid_q;
                     S.parent[ts] = (uint8_t)slot; S.parent[ts + 1u] = (uint8_t)slot;
                     S.acc[ts] = 0u; S.acc[ts + 1u] = 0u;
                     const uint32_t q = (q_tail + 2u * rank) & (uint32_t)(kCtQueueCap - 1), q1 = (q + 1u) & (uint32_t)(kCtQueueCap - 1);
                     const uint32_t t0_u = qx & 0xfffffu, lv = ((qx >> 20) + 1u) << 20;
-                    S.qx[q] = (2u * t0_u) | lv;       S.qy[q] = (qy & 0xffffu) | (pm << 16);  S.qz[q] = sl | (ts << 8);
-                    S.qx[q1] = (2u * t0_u + 1u) | lv; S.qy[q1] = pm | (qy & 0xffff0000u);     S.qz[q1] = sl | ((ts + 1u) << 8);
+                    S.qx[q] = (2u * t0_u) | lv;       S.qy[q] = (qy & 0x00ff00ffu) | (pm << 8) | (ts << 24);
+                    S.qx[q1] = (2u * t0_u + 1u) | lv; S.qy[q1] = (qy & 0x00ffff00u) | pm | ((ts + 1u) << 24);
                 }
                 q_head += n_round; q_tail += 2u * n_push; n_leaf += n_acc; n_split += n_push;
                 __syncwarp();
@@ -326,15 +324,15 @@ k_count(const CountArgs A) {
                 for (uint32_t l0 = 0; l0 < n_leaf; l0 += 32u) {
                     const uint32_t li = l0 + (uint32_t)lane;
                     const bool live = li < n_leaf;
-                    const uint32_t lab = live ? S.leaf[li].ab : 0u, sl = live ? (S.leaf[li].seg_slot & 0xffu) : 0u;
-                    const LeafEval ev = leaf_eval(S.pts[lab & 0xffffu], S.pts[lab >> 16], S.seg[sl].h, P.mode, P.tol_fl);
+                    const uint32_t lw = live ? S.leaf[li].w : 0u;
+                    const LeafEval ev = leaf_eval(S.pts[lw & 0xffu], S.pts[(lw >> 8) & 0xffu], S.seg[(lw >> 16) & 0xffu].h, P.mode, P.tol_fl);
                     const bool f0 = live && ev.full[0], f1 = live && ev.full[1];
                     const uint32_t m0 = __ballot_sync(kFull, f0), m1 = __ballot_sync(kFull, f1);
                     if (live) {
                         CtLeaf& lf = S.leaf[li];
                         lf.k0 = ev.k0; lf.k1 = ev.k1; lf.L = ev.L;
                         lf.n[0] = (uint16_t)ev.n[0]; lf.n[1] = (uint16_t)ev.n[1];
-                        lf.ab = (ev.n[0] <= (uint32_t)kDirectMax ? 1u : 0u) | (ev.n[1] <= (uint32_t)kDirectMax ? 0x100u : 0u);   // simple flags of the two sides (bytes 0, 1)
+                        lf.w = (lw & 0xffff0000u) | (ev.n[0] <= (uint32_t)kDirectMax ? 1u : 0u) | (ev.n[1] <= (uint32_t)kDirectMax ? 0x100u : 0u);   // simple flags of the two sides (bytes 0, 1)
                     }
                     if (f0) full_list[n_full + __popc(m0 & lt)] = (uint16_t)(2u * li);
                     n_full += __popc(m0);
@@ -350,11 +348,11 @@ k_count(const CountArgs A) {
                         CtLeaf& lf = S.leaf[l];
                         Piece p;
                         p.k0 = lf.k0; p.k1 = lf.k1; p.L = lf.L;
-                        const float h = S.seg[lf.seg_slot & 0xffu].h;
+                        const float h = S.seg[(lf.w >> 16) & 0xffu].h;
                         const SidePlan sp = side_plan(p, side ? h : -h, P.mode, P.tol_fl);
                         too_long |= (uint32_t)sp.total > 0xffffu;   // a side of more than 65535 records: the walk
                         lf.n[side] = (uint16_t)sp.total;
-                        reinterpret_cast<uint8_t*>(&lf.ab)[side] = (sp.nr == 1 && !sp.sup[0] && sp.total <= kDirectMax) ? 1 : 0;
+                        reinterpret_cast<uint8_t*>(&lf.w)[side] = (sp.nr == 1 && !sp.sup[0] && sp.total <= kDirectMax) ? 1 : 0;
                     }
                 }
                 __syncwarp();
@@ -364,13 +362,13 @@ k_count(const CountArgs A) {
                     const uint32_t l = l0 + (uint32_t)lane;
                     const bool live = l < n_leaf;
                     uint32_t n = 0, no = 0, fl = 0, slot = 0;
-                    if (live) { const CtLeaf& lf = S.leaf[l]; n = lf.n[0]; no = lf.n[1]; fl = lf.ab; slot = lf.seg_slot >> 8; }
+                    if (live) { const CtLeaf& lf = S.leaf[l]; n = lf.n[0]; no = lf.n[1]; fl = lf.w; slot = fl >> 24; }
                     // classes: 1 both sides one record (the simple writer's straight path), 2 both sides simple, 0 the others
                     const bool both = live && (fl & 0x101u) == 0x101u;
                     const bool triv = both && n == 1u && no == 1u;
                     const uint32_t m_triv = __ballot_sync(kFull, triv), m_multi = __ballot_sync(kFull, both && !triv), m_other = __ballot_sync(kFull, live && !both);
                     if (live) {
-                        S.leaf[l].ab = triv ? ((n_triv + __popc(m_triv & lt)) | 0x40000000u) : (both ? ((n_multi + __popc(m_multi & lt)) | 0x80000000u) : (n_other + __popc(m_other & lt)));
+                        S.leaf[l].w = (fl & 0xffff0000u) | (triv ? ((n_triv + __popc(m_triv & lt)) | 0x100u) : (both ? ((n_multi + __popc(m_multi & lt)) | 0x200u) : (n_other + __popc(m_other & lt))));
                         // subtree sums: the leaf's records are added to itself and to all its ancestors
                         const uint32_t c = n + no;
                         uint32_t cur = slot;
@@ -407,18 +405,18 @@ k_count(const CountArgs A) {
                     for (uint32_t li = (uint32_t)lane; li < n_leaf; li += 32u) {
                         const CtLeaf lf = S.leaf[li];
                         // records that precede the leaf in its segment: over the path to the root, the left siblings' subtree sums
-                        uint32_t cur = lf.seg_slot >> 8, rel = 0;
+                        uint32_t cur = lf.w >> 24, rel = 0;
                         while (cur >= (uint32_t)kCtTile) {
                             if ((cur - (uint32_t)kCtTile) & 1u) rel += S.acc[cur - 1u];
                             cur = S.parent[cur];
                         }
-                        const uint32_t sl = lf.seg_slot & 0xffu;
+                        const uint32_t sl = (lf.w >> 16) & 0xffu;
                         LeafRec r;
                         r.seg = s0 + sl; r.key = lf.key; r.n = (uint32_t)lf.n[0] | ((uint32_t)lf.n[1] << 16); r.rel = rel;
                         r.k0 = lf.k0; r.k1 = lf.k1; r.L = lf.L; r.h = S.seg[sl].h;
                         // the tile's simple leaves: the one-record ones from the front of its block, the others from its back,
                         // so that the warps of the simple writer see (mostly) one kind
-                        const uint32_t rank = lf.ab & 0x3fffffffu, cls = lf.ab >> 30;
+                        const uint32_t rank = lf.w & 0xffu, cls = (lf.w >> 8) & 0xffu;
                         const uint32_t pos = cls == 1u ? base_simple + rank : (cls == 2u ? base_simple + n_simple - 1u - rank : A.leaf_cap - 1u - (base_other + rank));
                         // (one 256-bit store: a full 32-byte sector; the leaf buffer is the context's own, aligned allocation)
                         asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(A.leaves + pos), "r"(r.seg), "r"(r.key), "r"(r.n), "r"(r.rel),
