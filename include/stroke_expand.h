@@ -138,7 +138,7 @@ sx_status sx_count(sx_ctx* ctx, const uint8_t* d_tags, uint64_t n_tags, const fl
 
 /* ------------------------------------------------------------------ phase 2: write
  * Writes the records of the preceding sx_count into d_out_records (sx_line[] or sx_arc[] by mode, 16-byte
- * aligned) of capacity cap_records: kernels (d), the writers, which read the per-segment offsets and the piece
+ * aligned; a 32-byte aligned buffer lets the kernels write an arc record in one 256-bit store) of capacity cap_records: kernels (d), the writers, which read the per-segment offsets and the piece
  * records phase 1 left (the fit is not repeated).  SX_E_CAPACITY if the capacity is known to be too small (the total
  * is known on the host only when sx_count was given h_total; otherwise the kernels themselves refuse to write past
  * the capacity and the error is reported by sx_last_error after a stream sync). */

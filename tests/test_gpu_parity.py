@@ -521,3 +521,26 @@ def test_very_long_chains(B, ctx):
     compare(sc, 0, g, r)
     assert ck.watertight_violations(g.xy, g.path_off) == 0
     assert g.seg_count.max() > 5000
+
+
+def test_arc_records_do_not_depend_on_the_alignment_of_the_buffer(B, ctx):
+    """A 32-byte aligned buffer takes arc records as 256-bit stores, a buffer aligned to 16 bytes only as two 16-byte stores:
+    the same bits."""
+    sc = S.make("c2", n_paths=150)
+    dev = "cuda:0"
+    tags, pts, sty = B.scene_to_torch(sc, device=dev)
+    poff = torch.empty(sc.n_paths + 1, dtype=torch.int64, device=dev)
+    total = B.sx_count(ctx, tags, pts, sty, sc.affine, sc.tolerance, 1, poff)
+    raw = torch.full((total * 8 + 8,), float("nan"), dtype=torch.float32, device=dev)
+    assert raw.data_ptr() % 32 == 0
+    a = raw[:total * 8].view(total, 8)
+    B.sx_write(ctx, a, total, 1)
+    torch.cuda.synchronize()
+    wide = a.cpu().numpy().view(np.uint32).copy()
+    raw.fill_(float("nan"))
+    b = raw[4:4 + total * 8].view(total, 8)
+    assert b.data_ptr() % 32 == 16
+    B.sx_write(ctx, b, total, 1)
+    torch.cuda.synchronize()
+    assert B.sx_last_error(ctx) == 0
+    assert np.array_equal(wide, b.cpu().numpy().view(np.uint32))
