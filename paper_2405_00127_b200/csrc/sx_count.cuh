@@ -149,10 +149,8 @@ __device__ __noinline__ uint32_t slow_count(const Params& P, uint32_t i, uint32_
 struct LeafEval { float k0, k1, L; uint32_t n[2]; bool full[2]; };
 // (one copy of each: the count pass's working set has to stay inside the instruction cache -- 16 unsynchronised warps per SM)
 __device__ __noinline__ float atan2_r_core_call(float y, float x) { return atan2_r_core(y, x); }
-__device__ __noinline__ uint32_t offset_count(float k0, float k1, float L, float eta, int mode, float tol_fl) {
-    Piece p;
-    p.k0 = k0; p.k1 = k1; p.L = L;
-    return (uint32_t)offset_plan(p, eta, 0.0f, 1.0f, mode, tol_fl).n;
+SX_DEV uint32_t offset_count(float k0, float k1, float L, float eta, int mode, float tol_fl) {
+    return (uint32_t)offset_plan_call(k0, k1, L, eta, 0.0f, 1.0f, mode, tol_fl).n;
 }
 SX_DEV LeafEval leaf_eval(float4 pa, float4 pb, float h, int mode, float tol_fl) {
     LeafEval e;

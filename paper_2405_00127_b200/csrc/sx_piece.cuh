@@ -272,6 +272,13 @@ SX_DEV OffPlan offset_plan(const Piece& p, float eta, float ta, float tb, int mo
     o.n = count_clamp(n_f);
     return o;
 }
+// (ONE out-of-line copy per kernel: the side plan calls it for each of its ranges, the count pass and the simple writer for
+// their single range; the kernels' working sets have to stay inside the instruction cache)
+__device__ __noinline__ OffPlan offset_plan_call(float k0, float k1, float L, float eta, float ta, float tb, int mode, float tol_fl) {
+    Piece p;
+    p.k0 = k0; p.k1 = k1; p.L = L;
+    return offset_plan(p, eta, ta, tb, mode, tol_fl);
+}
 // parameter of interior subdivision point i (0 < i < n)
 SX_DEV float offset_t(const Piece& p, const OffPlan& o, float eta, int i) {
     float fr = (float)i / (float)o.n, t;
@@ -363,11 +370,11 @@ __device__ __noinline__ SidePlan side_plan(const Piece& p, float eta, int mode, 
     s.total = 0;
     s.cusp_a = s.cusp_b = false;
     s.evo.n = 0;
-    s.off[0] = offset_plan(p, eta, 0.0f, tc, mode, tol_fl);
+    s.off[0] = offset_plan_call(p.k0, p.k1, p.L, eta, 0.0f, tc, mode, tol_fl);
     s.total += s.off[0].n;
     float ea = 0.0f, eb = tc;
     if (s.nr == 2) {
-        s.off[1] = offset_plan(p, eta, tc, 1.0f, mode, tol_fl);
+        s.off[1] = offset_plan_call(p.k0, p.k1, p.L, eta, tc, 1.0f, mode, tol_fl);
         s.total += s.off[1].n;
         if (!first_sup) { ea = tc; eb = 1.0f; }
     } else {

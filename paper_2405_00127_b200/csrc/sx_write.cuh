@@ -184,7 +184,7 @@ k_write_simple(const WriteArgs A) {
         o.n = (int)nrec; o.rule = kRuleUniform; o.ta = 0.0f; o.tb = 1.0f; o.ua = o.ub = 0.0f;
         Spiral z;
         if (nrec > 1u) {
-            if (!arc) o = offset_plan(p, eta, 0.0f, 1.0f, P.mode, P.tol_fl);   // (same call, same count as in the count pass)
+            if (!arc) o = offset_plan_call(p.k0, p.k1, p.L, eta, 0.0f, 1.0f, P.mode, P.tol_fl);   // (same call, same count as in the count pass)
             es_prepare(p, z);
         }
         float tp;
