@@ -3,7 +3,7 @@
 //
 //   k_write_segments   thread per input segment: the two exact offset lines of a straight segment (R-1b), the join with
 //                      the next segment or the caps (Alg. 1; sx_segment.cuh).
-//   k_write_simple     thread per (leaf, side) over the SIMPLE leaves (both sides one regular range of at most
+//   k_write_simple     thread per leaf over the SIMPLE leaves (both sides one regular range of at most
 //                      kDirectMax records): end points from the cubic, interior vertices from the spiral, no tables.
 //   k_write_general    warp per 16 leaves over the other leaves, thread per output record: side plans, spiral anchors and
 //                      the part tables of sx_cache.cuh staged in shared memory, 32 records per iteration, interior
@@ -135,68 +135,70 @@ SX_DEV Ctrl load_ctrl(const Params& P, uint32_t pt, uint32_t tag) {
     return c;
 }
 
-__global__ void __launch_bounds__(kWrThreads, 8)
+__global__ void __launch_bounds__(kWrThreads, 6)
 k_write_simple(const WriteArgs A) {
     const Params& P = A.P;
     const bool arc = P.mode == kModeArc;
-    const uint64_t n_sides = 2ull * n_simple_leaves(A);
-    // (n_sides is even and the two sides of a leaf are neighbouring lanes: a lane pair is in the loop together)
-    for (uint64_t idx = (uint64_t)blockIdx.x * kWrThreads + threadIdx.x; idx < n_sides; idx += (uint64_t)gridDim.x * kWrThreads) {
-        const uint32_t act = __activemask();   // (whole lane pairs)
-        const LeafRec r = load_leaf(A.leaves + (idx >> 1));
-        const int side = (int)(idx & 1ull);
+    const uint64_t n_leaves = n_simple_leaves(A);
+    // thread per LEAF: the segment's control points and the piece's two end points once, then its two sides (their records
+    // are neighbours in the output: [-h side][+h side]).  The count pass stores a tile's one-record leaves first, so the
+    // warps here are (mostly) of one kind.
+    for (uint64_t idx = (uint64_t)blockIdx.x * kWrThreads + threadIdx.x; idx < n_leaves; idx += (uint64_t)gridDim.x * kWrThreads) {
+        const LeafRec r = load_leaf(A.leaves + idx);
         const uint32_t n_minus = r.n & 0xffffu, n_plus = r.n >> 16;
-        uint32_t nrec = side ? n_plus : n_minus;
-        const uint64_t base = A.seg_off[r.seg] + r.rel + (side ? n_minus : 0u);
+        const uint64_t leaf_base = A.seg_off[r.seg] + r.rel;
         const Ctrl c = load_ctrl(P, P.pt_off[r.seg], P.tags[r.seg]);
-        // the lane's own end of the piece: side 0 the start point, side 1 the end point (exchanged below); at an end of the
-        // segment the cubic's own point and limit tangent (R-5), inside it cubic_point() as in the count pass
+        // the piece's end points: at an end of the segment the cubic's own point and limit tangent (R-5), inside it
+        // cubic_point() as in the count pass
         const uint32_t t0_u = r.key & 0xffffu, level = (r.key >> 16) & 31u;
         const float dt = __uint_as_float((127u - level) << 23);
-        const bool at0 = t0_u == 0u, at1 = t0_u + 1u == (1u << level);
         Seg s;
         s.kind = 3; s.degenerate = false; s.P0 = c.P0; s.P3 = c.P3; s.c1 = c.c1; s.c2 = c.c2; s.c3 = c.c3;
         s.ts = s.te = v2(0.0f, 0.0f);
-        float4 mine;
-        if (side ? at1 : at0) {
-            bool dg;
-            const V2 u = pick_tangent(side ? c.e1 : c.l1, side ? c.e2 : c.l2, side ? c.e3 : c.l3, &dg);
-            mine = side ? make_float4(c.c3.x, c.c3.y, u.x, u.y) : make_float4(0.0f, 0.0f, u.x, u.y);
-        } else {
-            float qm, q2;
-            mine = cubic_point(s, (float)(t0_u + (uint32_t)side) * dt, &qm, &q2);
-        }
-        float4 other;
-        other.x = __shfl_xor_sync(act, mine.x, 1); other.y = __shfl_xor_sync(act, mine.y, 1);
-        other.z = __shfl_xor_sync(act, mine.z, 1); other.w = __shfl_xor_sync(act, mine.w, 1);
-        const float4 a = side ? other : mine, b = side ? mine : other;
         Piece p;
-        p.base = c.P0; p.P3 = c.P3; p.at0 = at0; p.at1 = at1;
-        p.la = v2(a.x, a.y); p.ua = v2(a.z, a.w);
-        p.lb = v2(b.x, b.y); p.ub = v2(b.z, b.w);
+        p.base = c.P0; p.P3 = c.P3; p.at0 = t0_u == 0u; p.at1 = t0_u + 1u == (1u << level);
+        float4 pa = make_float4(0.0f, 0.0f, 0.0f, 0.0f), pb = pa;
+#pragma unroll 1
+        for (int k = 0; k < 2; k++) {
+            float4 q;
+            if (k ? p.at1 : p.at0) {
+                bool dg;
+                const V2 u = pick_tangent(k ? c.e1 : c.l1, k ? c.e2 : c.l2, k ? c.e3 : c.l3, &dg);
+                q = k ? make_float4(c.c3.x, c.c3.y, u.x, u.y) : make_float4(0.0f, 0.0f, u.x, u.y);
+            } else {
+                float qm, q2;
+                q = cubic_point(s, (float)(t0_u + (uint32_t)k) * dt, &qm, &q2);
+            }
+            if (k) pb = q; else pa = q;
+        }
+        p.la = v2(pa.x, pa.y); p.ua = v2(pa.z, pa.w);
+        p.lb = v2(pb.x, pb.y); p.ub = v2(pb.z, pb.w);
         p.ch = p.lb - p.la;
         p.k0 = r.k0; p.k1 = r.k1; p.L = r.L;
-        if (base + nrec > A.cap_records) { atomicOr(A.err, kErrCapacity); nrec = 0; }   // the side is not written
-        const float eta = side ? r.h : -r.h;
         const float4 nocusp = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-        const uint32_t kind = side ? (uint32_t)(kOffset | kPlus) : (uint32_t)kOffset;
-        OffPlan o;
-        o.n = (int)nrec; o.rule = kRuleUniform; o.ta = 0.0f; o.tb = 1.0f; o.ua = o.ub = 0.0f;
         Spiral z;
-        if (nrec > 1u) {
-            if (!arc) o = offset_plan_call(p.k0, p.k1, p.L, eta, 0.0f, 1.0f, P.mode, P.tol_fl);   // (same call, same count as in the count pass)
-            es_prepare(p, z);
-        }
-        float tp;
-        V2 prev = end_vertex(p, kEndT0, eta, nocusp, &tp);
-        for (uint32_t i = 1; i <= nrec; i++) {
-            float t;
-            V2 cur;
-            if (i < nrec) { t = offset_t(p, o, eta, (int)i); cur = normal_point(p, z, t, eta); }
-            else cur = end_vertex(p, kEndT1, eta, nocusp, &t);
-            const uint64_t rec = base + (side ? nrec - i : i - 1u);
-            put_record(A.out, arc, A.wide != 0u, rec, side ? cur : prev, side ? prev : cur, (side ? es_dphi(p, t, tp) : es_dphi(p, tp, t)) + 0.0f, r.seg, kind);
-            prev = cur; tp = t;
+        if (n_minus > 1u || n_plus > 1u) es_prepare(p, z);
+#pragma unroll 1
+        for (int side = 0; side < 2; side++) {
+            const uint32_t nrec = side ? n_plus : n_minus;
+            const uint64_t base = leaf_base + (side ? n_minus : 0u);
+            if (base + nrec > A.cap_records) { atomicOr(A.err, kErrCapacity); continue; }   // the side is not written
+            const float eta = side ? r.h : -r.h;
+            const uint32_t kind = side ? (uint32_t)(kOffset | kPlus) : (uint32_t)kOffset;
+            OffPlan o;
+            o.n = (int)nrec; o.rule = kRuleUniform; o.ta = 0.0f; o.tb = 1.0f; o.ua = o.ub = 0.0f;
+            if (nrec > 1u && !arc) o = offset_plan_call(p.k0, p.k1, p.L, eta, 0.0f, 1.0f, P.mode, P.tol_fl);   // (same call, same count as in the count pass)
+            float tp;
+            V2 prev = end_vertex(p, kEndT0, eta, nocusp, &tp);
+            for (uint32_t i = 1; i <= nrec; i++) {
+                float t;
+                V2 cur;
+                if (i < nrec) { t = offset_t(p, o, eta, (int)i); cur = normal_point(p, z, t, eta); }
+                else cur = end_vertex(p, kEndT1, eta, nocusp, &t);
+                const uint64_t rec = base + (side ? nrec - i : i - 1u);
+                put_record(A.out, arc, A.wide != 0u, rec, side ? cur : prev, side ? prev : cur, (side ? es_dphi(p, t, tp) : es_dphi(p, tp, t)) + 0.0f, r.seg, kind);
+                prev = cur; tp = t;
+            }
         }
     }
 }
