@@ -35,7 +35,8 @@
 namespace sx {
 
 constexpr int kCtTile = 32;                          // segments per tile at most (a warp: lane per segment)
-constexpr int kCtSub = 8;                            // segments per sub-tile of a tile that overflowed; the smallest tile
+constexpr int kCtSub = 8;                            // segments per sub-tile of a tile that overflowed (halved again when that overflows)
+constexpr int kCtTileMin = 4;                        // the smallest tile of a call
 constexpr int kCtSplitCap = 112;                     // splits of Alg. 2 per tile
 constexpr int kCtLeafCap = kCtTile + kCtSplitCap;    // Euler-spiral pieces per tile (leaves = curves + splits)
 constexpr int kCtPointCap = 2 * kCtTile + kCtSplitCap;   // the end points of every segment + 1 per split
@@ -191,8 +192,8 @@ k_count(const CountArgs A) {
     const int lane = threadIdx.x & 31;
     const uint32_t lt = (1u << lane) - 1u;
     const bool ok = (*A.err & kErrBadStream) == 0u;   // a malformed stream silences every segment
-    uint32_t T = A.force >= (uint32_t)kCtSub ? A.force : *reinterpret_cast<volatile uint32_t*>(A.hint);
-    T = T >= 32u ? 32u : (T >= 16u ? 16u : (uint32_t)kCtSub);
+    uint32_t T = A.force >= (uint32_t)kCtTileMin ? A.force : *reinterpret_cast<volatile uint32_t*>(A.hint);
+    T = T >= 32u ? 32u : (T >= 16u ? 16u : (T >= 8u ? 8u : (uint32_t)kCtTileMin));
     uint32_t st_direct = 0, st_sub = 0, st_walk = 0, st_leaves = 0, st_segs = 0;
 
     for (;;) {
@@ -203,6 +204,7 @@ k_count(const CountArgs A) {
         const uint32_t tile0 = tile * T, tile_n = min(T, P.n_tags - tile0), tile_end = tile0 + tile_n;
         uint32_t s0 = tile0, sn = tile_n;
         bool sub = false;   // the tile is being redone in sub-tiles
+        uint32_t sub_size = (uint32_t)kCtSub;
         if (A.force == kForceSub && tile_n > (uint32_t)kCtSub) { sub = true; sn = (uint32_t)kCtSub; st_sub++; }
 
         for (;;) {
@@ -384,6 +386,12 @@ k_count(const CountArgs A) {
                 sub = true; s0 = tile0; sn = (uint32_t)kCtSub; st_sub++;
                 continue;
             }
+            if (overflow && sn > 1u && A.force != kForceWalk) {   // a (sub-)tile that still does not fit: halve it, down to one segment
+                if (!sub) { sub = true; st_sub++; }
+                sub_size = sn >> 1;
+                sn = sub_size;
+                continue;
+            }
 
             // ================================================================ D: counts, leaf records
             bool walk = overflow;
@@ -446,7 +454,7 @@ k_count(const CountArgs A) {
             if (!sub) { st_direct++; break; }
             s0 += sn;
             if (s0 >= tile_end) break;
-            sn = min((uint32_t)kCtSub, tile_end - s0);
+            sn = min(sub_size, tile_end - s0);
         }
         st_segs += tile_n;
     }
@@ -465,10 +473,12 @@ k_count(const CountArgs A) {
             const uint32_t leaves = *reinterpret_cast<volatile uint32_t*>(A.stats + kStLeaves);
             const uint32_t segs = *reinterpret_cast<volatile uint32_t*>(A.stats + kStSegs);
             const uint32_t walked = *reinterpret_cast<volatile uint32_t*>(A.stats + kStWalk);
-            if (segs >= 256u && walked * 4u < segs) {   // (a handful of segments, or a launch that mostly walked, says nothing)
-                const float per_seg = (float)leaves / (float)(segs - walked);
+            if (segs >= 256u) {   // (a handful of segments says nothing about the scene)
+                const float per_seg = (float)leaves / (float)max(segs - walked, 1u);
                 const float room = 0.65f * (float)kCtLeafCap;
-                A.hint[1] = per_seg * 32.0f <= room ? 32u : (per_seg * 16.0f <= room ? 16u : (uint32_t)kCtSub);
+                uint32_t next = per_seg * 32.0f <= room ? 32u : (per_seg * 16.0f <= room ? 16u : (per_seg * 8.0f <= room ? 8u : (uint32_t)kCtTileMin));
+                if (walked * 4u >= segs) next = (uint32_t)kCtTileMin;   // a launch that mostly walked: its pieces were not counted
+                A.hint[1] = next;
             }
         }
     }

@@ -188,7 +188,7 @@ static sx_status run_count(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, co
                                                            tag_states, ctx_ticket(c, 0), ctx_err(c), c->d_hint);
     if (c->time_kernels) SX_CUDA(cudaEventRecord(c->ev[1], s));
     // persistent one-warp blocks: no more of them than there are tiles of the smallest size
-    uint64_t tiles = (n + sx::kCtSub - 1) / sx::kCtSub;
+    uint64_t tiles = (n + sx::kCtTileMin - 1) / sx::kCtTileMin;
     unsigned grid = (unsigned)(tiles < (uint64_t)c->count_blocks ? tiles : (uint64_t)c->count_blocks);
     sx::k_count<<<grid, 32, sizeof(sx::CtWarp), s>>>(C);
     if (c->time_kernels) SX_CUDA(cudaEventRecord(c->ev[2], s));
@@ -509,7 +509,7 @@ sx_status sx_set_option(sx_ctx* c, int32_t option, uint64_t value) {
         case SX_OPT_KEEP_SEGMENT_INFO: return SX_OK;   // (kept for compatibility: the per-segment results are always there)
         case SX_OPT_TIME_KERNELS: c->time_kernels = value != 0; c->timed = false; return SX_OK;
         case SX_OPT_TILE_SEGMENTS:
-            if (value != 0 && value != 1 && value != 2 && value != 8 && value != 16 && value != 32) return SX_E_INVALID_ARG;
+            if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8 && value != 16 && value != 32) return SX_E_INVALID_ARG;
             c->force_tiles = static_cast<uint32_t>(value);
             return SX_OK;
         default: return SX_E_INVALID_ARG;
@@ -526,7 +526,7 @@ sx_status sx_call_stats(sx_ctx* c, uint64_t* h_out4, void* cuda_stream) {
     SX_CUDA(cudaMemcpyAsync(hp, ctx_stats(c), 12, cudaMemcpyDeviceToHost, s));
     SX_CUDA(cudaMemcpyAsync(hp + 3, c->d_hint, 4, cudaMemcpyDeviceToHost, s));
     SX_CUDA(cudaStreamSynchronize(s));
-    h_out4[0] = hp[0]; h_out4[1] = hp[1]; h_out4[2] = hp[2]; h_out4[3] = c->force_tiles >= 8 ? c->force_tiles : hp[3];
+    h_out4[0] = hp[0]; h_out4[1] = hp[1]; h_out4[2] = hp[2]; h_out4[3] = c->force_tiles >= 4 ? c->force_tiles : hp[3];
     return SX_OK;
 }
 
