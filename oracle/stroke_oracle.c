@@ -40,7 +40,7 @@ typedef struct {
 
 enum { JOIN_MITER = 0, JOIN_ROUND = 1, JOIN_BEVEL = 2 };
 enum { CAP_BUTT = 0, CAP_SQUARE = 1, CAP_ROUND = 2 };
-enum { MODE_LINE = 0, MODE_ARC = 1 };
+enum { MODE_LINE = 0, MODE_ARC = 1, MODE_LINE_REFINED = 2 };   /* 2: lines with the exact density integral (L145) */
 
 /* record kinds (low 3 bits) | side bit (8 = +h side) */
 enum { K_OFFSET = 0, K_OFFSET_REV = 1, K_EVOLUTE = 2, K_CONNECTOR = 3, K_JOIN_OUTER = 4, K_JOIN_INNER = 5, K_CAP = 6, K_CLOSE = 7, K_PLUS = 8 };
@@ -168,6 +168,28 @@ float so_f_approx_inv(float u) {
     else if (a < 2.03885779f) r = (0.81f + sqrtf(0.6561f - 2.5624f * (C2 - a))) / 1.2812f;
     else r = 0.156f + sqrtf(0.024336f - 2.0f * (C3 - a));
     return u < 0 ? -r : r;
+}
+
+/* The "higher flattening quality" variant of L145 (reading R-22): the exact integral of L139 in the forward
+ * direction, and for the inverse "this approximation [as] a good initial value ...; two iterations of Newton solving are
+ * enough to refine this guess to within 32-bit floating point accuracy".  fp32 (this decides the counts and the t_i).
+ * f'(x) = sqrt|x^2 - 1| vanishes at |x| = 1, where f_approx_inv is already exact to leading order: the Newton step
+ * divides by max(f', 0.05). */
+float so_f_exact32(float x, float* deriv) {
+    float a = fabsf(x), r;
+    float d = sqrtf(fabsf((1.0f - a) * (1.0f + a)));   /* sqrt|x^2 - 1| without the cancellation of 1 - a a */
+    if (a <= 1.0f) r = 0.5f * (a * d + asinf(a));
+    else r = QUARTER_PI + 0.5f * (a * d - acoshf(a));
+    if (deriv) *deriv = d;
+    return x < 0 ? -r : r;
+}
+float so_f_inv_refined(float u) {
+    float x = so_f_approx_inv(u);
+    for (int it = 0; it < 2; it++) {
+        float d, fx = so_f_exact32(x, &d);
+        x = x - (fx - u) / fmaxf(d, 0.05f);
+    }
+    return x;
 }
 
 /* ================================================================== Appendix A: geometric Hermite interpolation
@@ -343,7 +365,7 @@ static v2d es_evolute(const piece_t* p, float t) {
 /* v -> sgn(v) |v|^1.5 and its inverse: the integral of sqrt|v| and the s ~ i^(2/3) rule of section 2.2 (L97) */
 static float pow15(float v) { float a = fabsf(v), w = a * sqrtf(a); return v < 0 ? -w : w; }
 static float pow15_inv(float w) { float c = cbrtf(fabsf(w)); c = c * c; return w < 0 ? -c : c; }
-enum { RULE_UNIFORM = 0, RULE_F_APPROX = 1, RULE_INFLECTION = 2, RULE_CUSP = 3 };
+enum { RULE_UNIFORM = 0, RULE_F_APPROX = 1, RULE_INFLECTION = 2, RULE_CUSP = 3, RULE_F_EXACT = 4 };
 static float clampf(float x, float lo, float hi) { return x < lo ? lo : (x > hi ? hi : x); }
 static float count_clamp(float n) { if (!(n >= 1.0f)) return 1.0f; return n > N_MAX ? N_MAX : n; }
 
@@ -386,10 +408,11 @@ static int offset_params(const ctx_t* c, const piece_t* p, float eta, float ta, 
                 rule = RULE_CUSP;
             }
         } else {
-            ua = so_f_approx(xa);
-            ub = so_f_approx(xb);
+            int refined = (c->mode == MODE_LINE_REFINED);
+            ua = refined ? so_f_exact32(xa, NULL) : so_f_approx(xa);
+            ub = refined ? so_f_exact32(xb, NULL) : so_f_approx(xb);
             n_f = ceilf(fabsf(ub - ua) / (4.0f * kp * ah * sqrtf(ah) * sqrtf(8.0f * c->tol_fl))); /* L83 with density sqrt|1-x^2|/(2 sqrt|h|) */
-            rule = RULE_F_APPROX;
+            rule = refined ? RULE_F_EXACT : RULE_F_APPROX;
         }
     }
     int n = (int)count_clamp(n_f);
@@ -403,6 +426,7 @@ static int offset_params(const ctx_t* c, const piece_t* p, float eta, float ta, 
         else {
             float u = ua + fr * (ub - ua), kap;
             if (rule == RULE_F_APPROX) kap = (so_f_approx_inv(u) + 1.0f) / (2.0f * eta);
+            else if (rule == RULE_F_EXACT) kap = (so_f_inv_refined(u) + 1.0f) / (2.0f * eta);
             else if (rule == RULE_INFLECTION) kap = pow15_inv(u);
             else kap = (1.0f - pow15_inv(u)) / eta;
             t = 0.5f + (kap * p->L - p->k0) / p->k1;
@@ -766,7 +790,7 @@ void so_free(so_result* r) {
 int so_expand(const uint8_t* tags, uint64_t n_tags, const float* pts, uint64_t n_points, const so_style* styles,
               uint64_t n_paths, const float* affine, float tolerance, int mode, so_result* out) {
     memset(out, 0, sizeof(*out));
-    if (!(tolerance > 0) || (mode != MODE_LINE && mode != MODE_ARC)) return -1;
+    if (!(tolerance > 0) || (mode != MODE_LINE && mode != MODE_ARC && mode != MODE_LINE_REFINED)) return -1;
     float det = affine[0] * affine[3] - affine[1] * affine[2];
     if (!isfinite(det) || det == 0.0f) return -1;
     out->seg_count = (uint32_t*)calloc(n_tags + 1, sizeof(uint32_t));
@@ -780,7 +804,7 @@ int so_expand(const uint8_t* tags, uint64_t n_tags, const float* pts, uint64_t n
     c.out = out;
     c.mode = mode;
     c.tol_es = 0.1f * tolerance; /* R-13 */
-    c.tol_fl = 0.8f * tolerance;
+    c.tol_fl = (mode == MODE_LINE_REFINED ? 0.9f : 0.8f) * tolerance;   /* R-22: the 6 % of f_approx (L145) no longer needs the margin */
     float scale = sqrtf(fabsf(det)); /* R-14 */
     uint64_t next_path = 0;
     for (uint64_t i = 0; i < n_tags; i++) {
