@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the stroke-expansion hot path on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c5|c3|c2|c1] [--mode line|arc] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c5|c3|c2|c1] [--mode line|arc|refined] [--impl ours|reference]
 
 A step is one pass of the whole hot path -- kernels (a) tag scan, (b) count pass, (c) allocation scan, (d) the four
 writers -- over one synthetic scene (default: config 4, the CAD-scale scene BASELINE.json's target is quoted on:
@@ -34,6 +34,7 @@ if ROOT not in sys.path:
 
 METRIC = "input path segments/sec expanded (device-timed)"
 UNIT = "segments/s"
+MODE_NAME = {0: "line", 1: "arc", 2: "line-refined"}
 MODE_OF = {"c3": 0, "c4": 1, "c5": 0, "c1": 0, "c2": 0}
 # whole-step dram__bytes_read.sum + dram__bytes_write.sum per step from the committed `ncu --set full` captures
 # (profiles/r2_counters.md names the command and the commit of each); None = not captured for that workload / mode
@@ -178,7 +179,7 @@ def run_reference(args):
         return
     import oracle
     oracle.build()
-    mode = MODE_OF[args.workload] if args.mode is None else int(args.mode == "arc")
+    mode = MODE_OF[args.workload] if args.mode is None else {"line": 0, "arc": 1, "refined": 2}[args.mode]
     cores = os.cpu_count() or 1
     npaths = REF_SAMPLE_PATHS[args.workload] * (4 if cores >= 8 else 1)
     sc = make_scene(args.workload, n_paths=npaths)
@@ -197,7 +198,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": args.workload, "mode": "arc" if mode else "line", "tolerance": float(sc.tolerance), "sample": sample},
+            "config": {"workload": args.workload, "mode": MODE_NAME[mode], "tolerance": float(sc.tolerance), "sample": sample},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
@@ -209,8 +210,8 @@ def unit_work(stats, kinds, mode, scale):
     n_join_outer, n_cap = int((k3 == 4).sum()), int((k3 == 6).sum())
     joins = stats["joins"] // 2
     units = {"fit_iter": stats["fit_iters"], "piece": stats["pieces"],
-             "range_arc" if mode else "range_line": stats["ranges_reg"] + stats["ranges_sup"],
-             "record_arc" if mode else "vertex_line": stats["rec_offset"],
+             "range_arc" if mode == 1 else "range_line": stats["ranges_reg"] + stats["ranges_sup"],
+             "record_arc" if mode == 1 else "vertex_line": stats["rec_offset"],
              "vertex_evolute": stats["rec_evolute"] // 2 + stats["rec_connector"] // 2,
              "join": joins, "cap": stats["caps"],
              "round_vertex": max(0, n_join_outer - joins) + max(0, n_cap - stats["caps"])}
@@ -233,11 +234,11 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(dev))
 
-    mode = MODE_OF[args.workload] if args.mode is None else int(args.mode == "arc")
+    mode = MODE_OF[args.workload] if args.mode is None else {"line": 0, "arc": 1, "refined": 2}[args.mode]
     sc = make_scene(args.workload, n_paths=args.paths)  # replicas only: every rank expands the whole scene
     n_seg, n_paths = sc.n_segments, sc.n_paths
     tags, pts, sty = B.scene_to_torch(sc, device=dev)
-    width = 8 if mode else 4
+    width = 8 if mode == 1 else 4
     sampler = ClockSampler(local)
     sampler.begin()
     issue = B.sx_measure_issue_peaks(local)
@@ -314,7 +315,7 @@ def run_ours(args):
 
     # ---- tile binning of the records just written (line mode only), device-timed
     binning = None
-    if args.binning and mode == 0:
+    if args.binning and mode != 1:
         ext = float(sc.points.max()) + 128.0
         tiles_xy = int(np.ceil(ext / 16.0))
         toff = torch.empty(tiles_xy * tiles_xy + 1, dtype=torch.int32, device=dev)
@@ -369,12 +370,12 @@ def run_ours(args):
         # the writers write the records): the roofline line is the WHOLE STEP -- algorithmic bytes over the device-timed step --
         # with the dominant kernel named by measured time and the per-kernel durations beside it
         ach = alg_bytes / t_step / 1e9
-        key = f"{args.workload}-{'arc' if mode else 'line'}"
+        key = f"{args.workload}-{MODE_NAME[mode]}"
         line = {"metric": METRIC, "value": job_throughput(n_seg, args.steps, world, t_total), "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": warm, "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": args.workload, "segments": n_seg, "paths": n_paths, "records": int(total),
-                           "mode": "arc" if mode else "line", "tolerance": float(sc.tolerance), "l2": "flushed between steps (256 MiB fill)",
+                           "mode": MODE_NAME[mode], "tolerance": float(sc.tolerance), "l2": "flushed between steps (256 MiB fill)",
                            "call": "stroke_expand_into (tag scan, count pass, allocation scan, writers; asynchronous, no host round trip)",
                            "parallelism": "replicas only" if world > 1 else "single GPU"},
                 "output_records_per_s": job_throughput(total, args.steps, world, t_total),
@@ -431,7 +432,7 @@ def main():
     ap.add_argument("--workload", default="c4", choices=sorted(MODE_OF))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--mode", default=None, choices=["line", "arc"], help="override the workload's output mode")
+    ap.add_argument("--mode", default=None, choices=["line", "arc", "refined"], help="override the workload's output mode (refined: SX_MODE_LINE_REFINED)")
     ap.add_argument("--binning", action="store_true", help="line mode: also time the tile binning of the records (SURVEY 8(f)-4)")
     ap.add_argument("--paths", type=int, default=None, help="profiling only: shrink the workload to this many paths")
     args = ap.parse_args()

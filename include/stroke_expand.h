@@ -70,7 +70,13 @@ typedef struct {
 
 enum { SX_JOIN_MITER = 0, SX_JOIN_ROUND = 1, SX_JOIN_BEVEL = 2 };
 enum { SX_CAP_BUTT = 0, SX_CAP_SQUARE = 1, SX_CAP_ROUND = 2 };
-enum { SX_MODE_LINE = 0, SX_MODE_ARC = 1 };
+/* Output modes.  SX_MODE_LINE_REFINED ("If higher flattening quality is desired at the expense
+ * of slower computation, this approximation could be used to determine a good initial value for numeric techniques; two
+ * iterations of Newton solving are enough to refine this guess to within 32-bit floating point accuracy"): lines as in
+ * SX_MODE_LINE, with the exact subdivision density integral f of L135-139 for the counts and f_approx_inv + two Newton steps
+ * for the subdivision points; the flatten tolerance rises from 0.8 to 0.9 of `tolerance` (the 6 % of f_approx no longer needs
+ * its margin; reading R-22 of DESIGN.md): 3-6 % fewer records of the same sx_line layout. */
+enum { SX_MODE_LINE = 0, SX_MODE_ARC = 1, SX_MODE_LINE_REFINED = 2 };
 
 /* ------------------------------------------------------------------ output records
  * Records are grouped by input segment, in segment order (hence by path); path_offsets[p] is the
@@ -242,8 +248,10 @@ sx_status sx_measure_issue_peaks(int32_t device, double* h_out3);
  *   SX_EVAL_ATAN2       h_in[2 i] = y, h_in[2 i + 1] = x  ->  the kernels' angle function (reading R-17 of DESIGN.md: the fp32
  *                       value nearest to atan2(y, x), by an own double-precision evaluation)
  *   SX_EVAL_NODE_ERROR  h_in[9 i ..] = u0.x u0.y u1.x u1.y |q0| |q1| chord.x chord.y dt  ->  the decision-grade error estimate
- *                       of section 7.1 that Alg. 2's accept / split test uses */
-enum { SX_EVAL_ATAN2 = 0, SX_EVAL_NODE_ERROR = 1 };
+ *                       of section 7.1 that Alg. 2's accept / split test uses
+ *   SX_EVAL_F_EXACT     h_in[i] = x  ->  the density integral f(x) of L135-139 as SX_MODE_LINE_REFINED evaluates it
+ *   SX_EVAL_F_INV_REFINED  h_in[i] = u  ->  its inverse: f_approx_inv(u) refined by two Newton steps (L145) */
+enum { SX_EVAL_ATAN2 = 0, SX_EVAL_NODE_ERROR = 1, SX_EVAL_F_EXACT = 2, SX_EVAL_F_INV_REFINED = 3 };
 sx_status sx_eval(int32_t device, int32_t what, const float* h_in, float* h_out, uint64_t n);
 
 /* Number of kernel launches the library has issued on this context so far. */

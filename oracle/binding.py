@@ -47,8 +47,8 @@ def lib():
         L.so_f_approx.argtypes = [C.c_float]
         L.so_f_approx_inv.restype = C.c_float
         L.so_f_approx_inv.argtypes = [C.c_float]
-        L.so_f_exact32.restype = C.c_float
-        L.so_f_exact32.argtypes = [C.c_float, C.POINTER(C.c_float)]
+        L.so_f_inv_newton.restype = C.c_double
+        L.so_f_inv_newton.argtypes = [C.c_float, C.c_int]
         L.so_f_inv_refined.restype = C.c_float
         L.so_f_inv_refined.argtypes = [C.c_float]
         L.so_ghi.argtypes = [C.c_float, C.c_float, C.POINTER(C.c_float), C.POINTER(C.c_float)]

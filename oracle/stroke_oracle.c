@@ -172,25 +172,36 @@ float so_f_approx_inv(float u) {
 
 /* The "higher flattening quality" variant of L145 (reading R-22): the exact integral of L139 in the forward
  * direction, and for the inverse "this approximation [as] a good initial value ...; two iterations of Newton solving are
- * enough to refine this guess to within 32-bit floating point accuracy".  fp32 (this decides the counts and the t_i).
- * f'(x) = sqrt|x^2 - 1| vanishes at |x| = 1, where f_approx_inv is already exact to leading order: the Newton step
- * divides by max(f', 0.05). */
-float so_f_exact32(float x, float* deriv) {
-    float a = fabsf(x), r;
-    float d = sqrtf(fabsf((1.0f - a) * (1.0f + a)));   /* sqrt|x^2 - 1| without the cancellation of 1 - a a */
-    if (a <= 1.0f) r = 0.5f * (a * d + asinf(a));
-    else r = QUARTER_PI + 0.5f * (a * d - acoshf(a));
-    if (deriv) *deriv = d;
-    return x < 0 ? -r : r;
+ * enough to refine this guess to within 32-bit floating point accuracy".
+ * Both in DOUBLE, rounded to fp32 once (as the angles of R-17): u = f(x) -> x is ill-conditioned next to the zeros of the
+ * density (f'(x) = sqrt|x^2 - 1| at |x| = 1: the inflection and the cusp), so an fp32 evaluation would make the subdivision
+ * points depend on the last bit of one libm's asinf.
+ * Newton from x0 = f_approx_inv(u) on f(a) = |u| for a = |x|; where the guess lies in the middle piece of L149
+ * (0.8 <= a < 1.25) the iteration runs on w(a) = sgn(e) |e|^(2/3), e = f(a) - pi/4, which is smooth and nearly linear
+ * across a = 1 (f - pi/4 ~ sqrt(8)/3 (a - 1)^1.5, L149), with w'(a) = 2/3 f'(a) / |e|^(1/3) -> 2/3 sqrt(a + 1) / (sqrt(8)/3)^(1/3). */
+static double f_and_deriv(double a, double* deriv) {
+    *deriv = sqrt(fabs((1.0 - a) * (1.0 + a)));
+    return so_f_exact(a);
 }
-float so_f_inv_refined(float u) {
-    float x = so_f_approx_inv(u);
-    for (int it = 0; it < 2; it++) {
-        float d, fx = so_f_exact32(x, &d);
-        x = x - (fx - u) / fmaxf(d, 0.05f);
+static double signed_pow23(double v) { double c = cbrt(fabs(v)); c = c * c; return v < 0 ? -c : c; }
+double so_f_inv_newton(float u, int steps) {
+    double au = fabs((double)u);
+    double a = fabs((double)so_f_approx_inv(u));
+    int middle = (a >= 0.8 && a < 1.25);
+    double wt = signed_pow23(au - M_PI / 4);
+    for (int it = 0; it < steps; it++) {
+        double d, fa = f_and_deriv(a, &d);
+        if (middle) {
+            double e = fa - M_PI / 4, ce = cbrt(fabs(e));
+            double ratio = fabs(a - 1.0) < 1e-9 ? sqrt(a + 1.0) / cbrt(sqrt(8.0) / 3.0) : d / ce;
+            a = a - (signed_pow23(e) - wt) / ((2.0 / 3.0) * ratio);
+        } else {
+            a = a - (fa - au) / d;
+        }
     }
-    return x;
+    return u < 0 ? -a : a;
 }
+float so_f_inv_refined(float u) { return (float)so_f_inv_newton(u, 2); }
 
 /* ================================================================== Appendix A: geometric Hermite interpolation
  * k = th0+th1, D = th1-th0 (L634).  k1 (L636) and chord/arc ratio c (L641-651), coefficients verbatim,
@@ -409,8 +420,8 @@ static int offset_params(const ctx_t* c, const piece_t* p, float eta, float ta, 
             }
         } else {
             int refined = (c->mode == MODE_LINE_REFINED);
-            ua = refined ? so_f_exact32(xa, NULL) : so_f_approx(xa);
-            ub = refined ? so_f_exact32(xb, NULL) : so_f_approx(xb);
+            ua = refined ? (float)so_f_exact((double)xa) : so_f_approx(xa);
+            ub = refined ? (float)so_f_exact((double)xb) : so_f_approx(xb);
             n_f = ceilf(fabsf(ub - ua) / (4.0f * kp * ah * sqrtf(ah) * sqrtf(8.0f * c->tol_fl))); /* L83 with density sqrt|1-x^2|/(2 sqrt|h|) */
             rule = refined ? RULE_F_EXACT : RULE_F_APPROX;
         }

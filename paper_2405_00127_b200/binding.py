@@ -16,8 +16,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SO_PATH = os.path.join(_HERE, "libstroke_expand.so")
 
 SX_OK, SX_E_INVALID_ARG, SX_E_BAD_STREAM, SX_E_CAPACITY, SX_E_CUDA, SX_E_STATE = 0, -1, -2, -3, -4, -5
-SX_MODE_LINE, SX_MODE_ARC = 0, 1
-RECORD_BYTES = {SX_MODE_LINE: 16, SX_MODE_ARC: 32}
+SX_MODE_LINE, SX_MODE_ARC, SX_MODE_LINE_REFINED = 0, 1, 2
+RECORD_BYTES = {SX_MODE_LINE: 16, SX_MODE_ARC: 32, SX_MODE_LINE_REFINED: 16}
 ARC_DTYPE = np.dtype([("x0", "<f4"), ("y0", "<f4"), ("x1", "<f4"), ("y1", "<f4"), ("angle", "<f4"), ("seg", "<u4"),
                       ("kind", "<u4"), ("pad", "<u4")])
 
@@ -142,7 +142,7 @@ def stroke_expand_into(ctx, tags, points, styles, affine, tolerance, mode, out_r
     needed count in .needed when the records do not fit."""
     args = _dev_streams(tags, points, styles)
     a, ap = _affine(affine)
-    width = 4 if mode == SX_MODE_LINE else 8
+    width = 8 if mode == SX_MODE_ARC else 4
     assert out_records.is_cuda and out_records.is_contiguous() and out_records.dtype == torch.float32
     cap = out_records.numel() // width
     assert path_offsets.is_cuda and path_offsets.is_contiguous() and path_offsets.element_size() == 8 and path_offsets.numel() >= args[5] + 1
@@ -167,7 +167,7 @@ def stroke_expand(ctx, tags, points, styles, affine, tolerance, mode, stream=Non
     dev = tags.device
     path_offsets = torch.empty(args[5] + 1, dtype=torch.int64, device=dev)
     holder = {}
-    width = 4 if mode == SX_MODE_LINE else 8
+    width = 8 if mode == SX_MODE_ARC else 4
 
     def _alloc(nbytes, _user):
         t = torch.empty((nbytes // (4 * width), width), dtype=torch.float32, device=dev)
@@ -193,7 +193,7 @@ def stroke_expand_host(ctx, tags, points, styles, affine, tolerance, mode, out_r
         assert not t.is_cuda and t.is_contiguous()
     assert tags.dtype == torch.uint8 and points.dtype == torch.float32 and styles.dtype == torch.uint8
     a, ap = _affine(affine)
-    width = 4 if mode == SX_MODE_LINE else 8
+    width = 8 if mode == SX_MODE_ARC else 4
     cap = out_records.numel() // width
     n_paths = styles.numel() // 16
     assert path_offsets.element_size() == 8 and path_offsets.numel() >= n_paths + 1
@@ -286,7 +286,7 @@ def sx_measure_issue_peaks(device=0):
     return dict(fp32_ffma=float(out[0]), fp32_mix=float(out[1]), mufu=float(out[2]))
 
 
-SX_EVAL_ATAN2, SX_EVAL_NODE_ERROR = 0, 1
+SX_EVAL_ATAN2, SX_EVAL_NODE_ERROR, SX_EVAL_F_EXACT, SX_EVAL_F_INV_REFINED = 0, 1, 2, 3
 
 
 def sx_eval(what, values, device=0):

@@ -19,7 +19,7 @@ struct PlanLite {
     float eta, tc;
     uint32_t seg, total;
     uint16_t n0, n1, ne;
-    uint8_t flags;   // bit 0 two ranges, 1 sup0, 2 sup1, 5 uniform evolute, 6 evolute parameters by cubing (arc mode)
+    uint8_t flags;   // bit 0 two ranges, 1 sup0, 2 sup1, 3 refined f (mode 2), 5 uniform evolute, 6 evolute parameters by cubing (arc mode)
     uint8_t rules;   // spacing rule (kRule*) of range 0 | of range 1 << 2
     float ua0, ub0, ua1, ub1, wa, wb, skp;
 };
@@ -27,7 +27,7 @@ SX_DEV PlanLite plan_pack(const SidePlan& s) {
     PlanLite q;
     q.eta = s.eta; q.tc = s.off[0].tb; q.seg = s.seg; q.total = (uint32_t)s.total;
     q.n0 = (uint16_t)s.off[0].n; q.n1 = (uint16_t)s.off[1].n; q.ne = (uint16_t)s.evo.n;
-    q.flags = (uint8_t)((s.nr == 2 ? 1u : 0u) | (s.sup[0] ? 2u : 0u) | (s.sup[1] ? 4u : 0u) | (s.evo.uniform ? 32u : 0u) | (s.evo.cube ? 64u : 0u));
+    q.flags = (uint8_t)((s.nr == 2 ? 1u : 0u) | (s.sup[0] ? 2u : 0u) | (s.sup[1] ? 4u : 0u) | (SX_OFF_REFINED(s.off[0]) ? 8u : 0u) | (s.evo.uniform ? 32u : 0u) | (s.evo.cube ? 64u : 0u));
     q.rules = (uint8_t)((uint32_t)s.off[0].rule | ((uint32_t)s.off[1].rule << 2));
     q.ua0 = s.off[0].ua; q.ub0 = s.off[0].ub; q.ua1 = s.off[1].ua; q.ub1 = s.off[1].ub;
     q.wa = s.evo.wa; q.wb = s.evo.wb; q.skp = s.evo.skp;
@@ -39,6 +39,9 @@ SX_DEV OffPlan plan_off(const PlanLite& q, bool second) {
     o.rule = (int)((q.rules >> (second ? 2 : 0)) & 3u);
     o.ta = second ? q.tc : 0.0f; o.tb = second ? 1.0f : q.tc;
     o.ua = second ? q.ua1 : q.ua0; o.ub = second ? q.ub1 : q.ub0;
+#if SX_REFINED
+    o.refined = (q.flags & 8u) != 0u;
+#endif
     return o;
 }
 SX_DEV EvoPlan plan_evo(const PlanLite& q);

@@ -176,7 +176,7 @@ SX_DEV LeafEval leaf_eval(float4 pa, float4 pb, float h, int mode, float tol_fl)
         const float eta = side ? h : -h;
         e.full[side] = !(fmaf(-ka, eta, 1.0f) > 1e-3f && fmaf(-kb, eta, 1.0f) > 1e-3f);
         e.n[side] = n_arc;
-        if (mode != kModeArc && !e.full[side]) e.n[side] = offset_count(p.k0, p.k1, p.L, eta, kModeLine, tol_fl);
+        if (mode != kModeArc && !e.full[side]) e.n[side] = offset_count(p.k0, p.k1, p.L, eta, mode, tol_fl);
         if (e.full[side]) e.n[side] = 0xffffu;   // (not simple until the full plan says so)
     }
     if (h == 0.0f) { e.n[1] = 0u; e.full[1] = false; }   // a filled path (Alg. 1): offset 0, the curve once

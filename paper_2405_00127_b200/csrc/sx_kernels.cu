@@ -17,6 +17,7 @@
 #include "sx_write.cuh"
 #include "sx_bin.cuh"
 #include "sx_peaks.cuh"
+#include "sx_refined.h"
 
 // ====================================================================== host side
 static thread_local cudaError_t g_last_cuda = cudaSuccess;
@@ -123,7 +124,7 @@ static sx_status check_inputs(const uint8_t* d_tags, uint64_t n_tags, const floa
                               uint64_t n_paths, const float* h_affine, float tolerance, int32_t mode, const uint64_t* d_path_offsets) {
     if (!h_affine || !d_path_offsets) return SX_E_INVALID_ARG;
     if (!(tolerance > 0.0f) || !(tolerance < INFINITY)) return SX_E_INVALID_ARG;
-    if (mode != SX_MODE_LINE && mode != SX_MODE_ARC) return SX_E_INVALID_ARG;
+    if (mode != SX_MODE_LINE && mode != SX_MODE_ARC && mode != SX_MODE_LINE_REFINED) return SX_E_INVALID_ARG;
     if (n_tags >= (1ull << 32) - sx::kTagTile || n_points >= (1ull << 32) || n_paths > n_tags) return SX_E_INVALID_ARG;
     if (n_tags > 0 && (!d_tags || !d_points_xy || !d_styles)) return SX_E_INVALID_ARG;
     // the kernels read tags and styles with 16-byte loads, points and offsets with 8-byte accesses
@@ -152,7 +153,7 @@ static sx_status run_count(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, co
     float det = h_affine[0] * h_affine[3] - h_affine[1] * h_affine[2];
     P.scale = sqrtf(fabsf(det));                 // R-14
     P.tol_es = 0.1f * tolerance;                 // R-13
-    P.tol_fl = 0.8f * tolerance;
+    P.tol_fl = (mode == SX_MODE_LINE_REFINED ? 0.9f : 0.8f) * tolerance;   // R-22: the 6 % of f_approx no longer needs its margin
     P.mode = mode;
     P.n_tags = static_cast<uint32_t>(n_tags);
     C.n_paths = static_cast<uint32_t>(n_paths);
@@ -190,7 +191,8 @@ static sx_status run_count(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, co
     // persistent one-warp blocks: no more of them than there are tiles of the smallest size
     uint64_t tiles = (n + sx::kCtTileMin - 1) / sx::kCtTileMin;
     unsigned grid = (unsigned)(tiles < (uint64_t)c->count_blocks ? tiles : (uint64_t)c->count_blocks);
-    sx::k_count<<<grid, 32, sizeof(sx::CtWarp), s>>>(C);
+    if (mode == SX_MODE_LINE_REFINED) sxr_launch_count(&C, grid, s);   // (sx_refined.cu: the same kernel with the refined density integral)
+    else sx::k_count<<<grid, 32, sizeof(sx::CtWarp), s>>>(C);
     if (c->time_kernels) SX_CUDA(cudaEventRecord(c->ev[2], s));
     uint32_t n_cnt_tiles = (n + sx::kCntTile - 1) / sx::kCntTile;
     sx::k_alloc_scan<<<n_cnt_tiles, sx::kScanThreads, 0, s>>>(c->seg_count, n, d_tags, c->path_idx, (uint32_t)n_paths, c->seg_off, d_path_offsets,
@@ -212,10 +214,15 @@ static sx_status run_write(sx_ctx* c, void* d_out_records, uint64_t cap_records,
     // others on the context's side streams, forked from and joined to the caller's stream with events
     SX_CUDA(cudaEventRecord(c->fork, s));
     for (int k = 0; k < kSideStreams; k++) SX_CUDA(cudaStreamWaitEvent(c->side[k], c->fork, 0));
-    sx::k_write_general<<<c->general_blocks, sx::kWrThreads, 0, s>>>(c->W);
-    sx::k_write_simple<<<c->simple_blocks, sx::kWrThreads, 0, c->side[0]>>>(c->W);
-    sx::k_write_segments<<<(n + sx::kWrThreads - 1) / sx::kWrThreads, sx::kWrThreads, 0, c->side[1]>>>(c->W);
-    sx::k_write_walk<<<c->sm_count, sx::kWrThreads, 0, c->side[2]>>>(c->W);
+    const unsigned segment_blocks = (n + sx::kWrThreads - 1) / sx::kWrThreads;
+    if (c->W.P.mode == SX_MODE_LINE_REFINED) {
+        sxr_launch_writers(&c->W, c->general_blocks, c->simple_blocks, segment_blocks, c->sm_count, s, c->side[0], c->side[1], c->side[2]);
+    } else {
+        sx::k_write_general<<<c->general_blocks, sx::kWrThreads, 0, s>>>(c->W);
+        sx::k_write_simple<<<c->simple_blocks, sx::kWrThreads, 0, c->side[0]>>>(c->W);
+        sx::k_write_segments<<<segment_blocks, sx::kWrThreads, 0, c->side[1]>>>(c->W);
+        sx::k_write_walk<<<c->sm_count, sx::kWrThreads, 0, c->side[2]>>>(c->W);
+    }
     for (int k = 0; k < kSideStreams; k++) {
         SX_CUDA(cudaEventRecord(c->join[k], c->side[k]));
         SX_CUDA(cudaStreamWaitEvent(s, c->join[k], 0));
@@ -553,16 +560,17 @@ __global__ void k_eval(int what, const float* in, float* out, uint64_t n) {
 }
 
 sx_status sx_eval(int32_t device, int32_t what, const float* h_in, float* h_out, uint64_t n) {
-    if (!h_in || !h_out || (what != SX_EVAL_ATAN2 && what != SX_EVAL_NODE_ERROR)) return SX_E_INVALID_ARG;
+    if (!h_in || !h_out || what < SX_EVAL_ATAN2 || what > SX_EVAL_F_INV_REFINED) return SX_E_INVALID_ARG;
     if (n == 0) return SX_OK;
-    const uint64_t per = what == SX_EVAL_ATAN2 ? 2 : 9;
+    const uint64_t per = what == SX_EVAL_ATAN2 ? 2 : (what == SX_EVAL_NODE_ERROR ? 9 : 1);
     SX_CUDA(cudaSetDevice(device));
     float *d_in = nullptr, *d_out = nullptr;
     SX_CUDA(cudaMalloc(&d_in, n * per * sizeof(float)));
     cudaError_t e = cudaMalloc(&d_out, n * sizeof(float));
     if (e == cudaSuccess) e = cudaMemcpy(d_in, h_in, n * per * sizeof(float), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) {
-        k_eval<<<(unsigned)((n + 255) / 256), 256>>>(what, d_in, d_out, n);
+        if (what >= SX_EVAL_F_EXACT) sxr_launch_eval(what, d_in, d_out, n);
+        else k_eval<<<(unsigned)((n + 255) / 256), 256>>>(what, d_in, d_out, n);
         e = cudaMemcpy(h_out, d_out, n * sizeof(float), cudaMemcpyDeviceToHost);
     }
     cudaFree(d_in);

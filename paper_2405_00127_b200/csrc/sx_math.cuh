@@ -12,6 +12,12 @@
 // coordinates are evaluated in segment-local coordinates with explicit fmaf and the segment base
 // point is added last (fp32 ulp at 16384 px is 9.8e-4 px).
 #pragma once
+// SX_REFINED: the translation unit sx_refined.cu compiles these headers a second time, in namespace sx_refined, with the
+// code of SX_MODE_LINE_REFINED switched on; the kernels of the other modes do not carry it (they are bound
+// by the instruction cache: DESIGN.md section 5).
+#ifndef SX_REFINED
+#define SX_REFINED 0
+#endif
 #include <stdint.h>
 #include <math.h>
 
@@ -37,7 +43,7 @@ constexpr float kKnot1 = 0.90324929f;
 constexpr float kKnot2 = 2.03885779f;
 
 enum : uint32_t { kOffset = 0, kOffsetRev = 1, kEvolute = 2, kConnector = 3, kJoinOuter = 4, kJoinInner = 5, kCap = 6, kClose = 7, kPlus = 8 };
-enum : int { kJoinMiter = 0, kJoinRound = 1, kJoinBevel = 2, kCapButt = 0, kCapSquare = 1, kCapRound = 2, kModeLine = 0, kModeArc = 1 };
+enum : int { kJoinMiter = 0, kJoinRound = 1, kJoinBevel = 2, kCapButt = 0, kCapSquare = 1, kCapRound = 2, kModeLine = 0, kModeArc = 1, kModeLineRefined = 2 };   // 2: lines with the exact density integral (L145, R-22)
 
 // ---------------------------------------------------------------- float2 helpers (plain operators: no contraction)
 struct V2 { float x, y; };

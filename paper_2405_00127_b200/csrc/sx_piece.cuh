@@ -42,6 +42,49 @@ SX_DEV float f_approx_inv(float u) {
     return u < 0.0f ? -r : r;
 }
 
+#if SX_REFINED
+// The "higher flattening quality" variant of L145 (reading R-22): the exact integral of L139 in the forward
+// direction and, as its inverse, f_approx_inv refined by "two iterations of Newton solving".  Both in DOUBLE, rounded to
+// fp32 once (as the angles of R-17): u -> x is ill-conditioned next to the zeros of the density (f' = sqrt|x^2 - 1| at
+// |x| = 1), an fp32 evaluation would make the subdivision points depend on the last bit of asinf.  Where the guess lies in
+// the middle piece of L149 the iteration runs on w(a) = sgn(e) |e|^(2/3), e = f(a) - pi/4, smooth and nearly linear
+// across a = 1, with w'(a) = 2/3 f'(a) / |e|^(1/3) -> 2/3 sqrt(a + 1) / (sqrt(8)/3)^(1/3).
+__device__ __noinline__ double f_exact_d(double a, double* deriv) {   // a >= 0
+    const double d = sqrt(fabs((1.0 - a) * (1.0 + a)));
+    *deriv = d;
+    return a <= 1.0 ? 0.5 * (a * d + asin(a)) : 0.78539816339744830962 + 0.5 * (a * d - acosh(a));
+}
+SX_DEV float f_exact(float x) {
+    double d;
+    const float r = (float)f_exact_d((double)fabsf(x), &d);
+    return x < 0.0f ? -r : r;
+}
+SX_DEV double signed_pow23(double v) { double c = cbrt(fabs(v)); c = c * c; return v < 0.0 ? -c : c; }
+__device__ __noinline__ float f_inv_refined(float u) {
+    const double au = fabs((double)u);
+    double a = fabs((double)f_approx_inv(u));
+    const bool middle = a >= 0.8 && a < 1.25;
+    const double wt = signed_pow23(au - 0.78539816339744830962);
+#pragma unroll 1
+    for (int it = 0; it < 2; it++) {
+        double d;
+        const double fa = f_exact_d(a, &d);
+        if (middle) {
+            const double e = fa - 0.78539816339744830962, ce = cbrt(fabs(e));
+            const double ratio = fabs(a - 1.0) < 1e-9 ? sqrt(a + 1.0) / 0.98057856349232452 : d / ce;   // cbrt(sqrt(8) / 3)
+            a = a - (signed_pow23(e) - wt) / ((2.0 / 3.0) * ratio);
+        } else {
+            a = a - (fa - au) / d;
+        }
+    }
+    const float r = (float)a;
+    return u < 0.0f ? -r : r;
+}
+#define SX_OFF_REFINED(o) ((o).refined)
+#else
+#define SX_OFF_REFINED(o) false
+#endif
+
 // v -> sgn(v) |v|^1.5 and its inverse: the integral of sqrt|v| and the s ~ i^(2/3) rule of section 2.2 (L97)
 SX_DEV float pow15(float v) { const float a = fabsf(v), w = a * sqrtf(a); return v < 0.0f ? -w : w; }
 SX_DEV float pow15_inv(float w) { float c = cbrtf(fabsf(w)); c = c * c; return w < 0.0f ? -c : c; }
@@ -225,13 +268,21 @@ SX_DEV V2 es_offset(const Piece& p, const Spiral& sp, float t, float eta) { retu
 SX_DEV V2 es_evolute(const Piece& p, const Spiral& sp, float t) { return normal_point(p, sp, t, es_radius(p, t)); }  // section 6
 
 // ---------------------------------------------------------------- subdivision plans
-struct OffPlan { int n; int rule; float ta, tb, ua, ub; };   // rule: how the interior parameters are spaced (kRule*)
+struct OffPlan {   // rule: how the interior parameters are spaced (kRule*)
+    int n; int rule; float ta, tb, ua, ub;
+#if SX_REFINED
+    bool refined;   // kRuleFApprox with the exact f and its Newton-refined inverse
+#endif
+};
 struct EvoPlan { int n; bool uniform, cube; float ta, tb, wa, wb, skp; };   // cube: arc mode, the parameters are uniform in cbrt(sigma)
 
 // offset range [ta,tb] of side eta (sections 4, 5): number of records and what the parameters need
 SX_DEV OffPlan offset_plan(const Piece& p, float eta, float ta, float tb, int mode, float tol_fl) {
     OffPlan o;
     o.ta = ta; o.tb = tb; o.ua = 0.0f; o.ub = 0.0f; o.rule = kRuleUniform;
+#if SX_REFINED
+    o.refined = mode == kModeLineRefined;
+#endif
     float n_f, ah = fabsf(eta);
     if (mode == kModeArc) {
         // L177 with s = L, kappa' = k1/L^2, scaled by the range fraction (R-12)
@@ -263,8 +314,10 @@ SX_DEV OffPlan offset_plan(const Piece& p, float eta, float ta, float tb, int mo
                 o.rule = kRuleCusp;
             }
         } else {
-            o.ua = f_approx(xa);
-            o.ub = f_approx(xb);
+#if SX_REFINED
+            if (o.refined) { o.ua = f_exact(xa); o.ub = f_exact(xb); } else
+#endif
+            { o.ua = f_approx(xa); o.ub = f_approx(xb); }
             n_f = ceilf(div_fast(fabsf(o.ub - o.ua), 4.0f * kp * ah * sqrt_fast(ah) * sqrt_fast(8.0f * tol_fl)));  // L83
             o.rule = kRuleFApprox;
         }
@@ -285,6 +338,9 @@ SX_DEV float offset_t(const Piece& p, const OffPlan& o, float eta, int i) {
     if (o.rule == kRuleUniform) t = o.ta + fr * (o.tb - o.ta);
     else {
         float u = o.ua + fr * (o.ub - o.ua), kap;
+#if SX_REFINED
+        if (o.rule == kRuleFApprox && o.refined) kap = (f_inv_refined(u) + 1.0f) / (2.0f * eta); else
+#endif
         if (o.rule == kRuleFApprox) kap = (f_approx_inv(u) + 1.0f) / (2.0f * eta);
         else if (o.rule == kRuleInflection) kap = pow15_inv(u);
         else kap = (1.0f - pow15_inv(u)) / eta;

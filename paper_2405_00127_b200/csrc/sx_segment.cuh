@@ -33,7 +33,7 @@ struct Writer {
     bool wide;       // arc records by 256-bit stores (the buffer is 32-byte aligned)
     SX_DEV void put(uint32_t idx, V2 a, V2 b, float angle, uint32_t kind) const {
         uint64_t r = base + idx;
-        if (mode == kModeLine) {
+        if (mode != kModeArc) {
             out[r] = make_float4(a.x, a.y, b.x, b.y);
         } else {
             store_arc(out, r, wide, make_float4(a.x, a.y, b.x, b.y), make_float4(angle, u2f(seg), u2f(kind), 0.0f));

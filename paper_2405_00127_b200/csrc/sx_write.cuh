@@ -187,6 +187,9 @@ k_write_simple(const WriteArgs A) {
             const uint32_t kind = side ? (uint32_t)(kOffset | kPlus) : (uint32_t)kOffset;
             OffPlan o;
             o.n = (int)nrec; o.rule = kRuleUniform; o.ta = 0.0f; o.tb = 1.0f; o.ua = o.ub = 0.0f;
+#if SX_REFINED
+            o.refined = false;
+#endif
             if (nrec > 1u && !arc) o = offset_plan_call(p.k0, p.k1, p.L, eta, 0.0f, 1.0f, P.mode, P.tol_fl);   // (same call, same count as in the count pass)
             float tp;
             V2 prev = end_vertex(p, kEndT0, eta, nocusp, &tp);

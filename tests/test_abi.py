@@ -52,7 +52,7 @@ def test_binding_lists_the_same_names(so_path):
 def test_record_and_style_layouts():
     from paper_2405_00127_b200 import binding, scenes
     assert scenes.STYLE_DTYPE.itemsize == 16
-    assert binding.ARC_DTYPE.itemsize == 32 and binding.RECORD_BYTES == {0: 16, 1: 32}
+    assert binding.ARC_DTYPE.itemsize == 32 and binding.RECORD_BYTES == {0: 16, 1: 32, 2: 16}
     src = open(HEADER).read()
     assert "sx_line; /* SX_MODE_LINE: 16 bytes" in src and "sx_arc; /* SX_MODE_ARC: 32 bytes" in src
 

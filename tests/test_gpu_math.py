@@ -78,3 +78,32 @@ def test_node_error_agrees_with_the_plain_formulas(B):
     print(f"node_error: relative difference median {q[0]:.1e}, 99.9 % {q[1]:.1e}")
     assert rel.max() <= 1e-4 and q[1] <= 2e-5      # (the worst cases: the two area terms nearly cancel)
     assert guard.sum() > 100
+
+
+def test_refined_density_integral_and_its_inverse(B):
+    """SX_MODE_LINE_REFINED: the kernels' f against the closed form of L139 evaluated in double
+    with numpy (not with the oracle), and f(f_inv_refined(u)) = u to fp32 accuracy -- two Newton steps from f_approx_inv --
+    over the whole range, next to the zeros of the density (|x| = 1) included; the oracle's fp32 evaluation of the same
+    formulas differs by rounding only."""
+    def f64(x):
+        a = np.abs(x)
+        r = np.where(a <= 1, 0.5 * (a * np.sqrt(np.maximum(1 - a * a, 0)) + np.arcsin(np.minimum(a, 1))),
+                     np.pi / 4 + 0.5 * (a * np.sqrt(np.maximum(a * a - 1, 0)) - np.arccosh(np.maximum(a, 1))))
+        return np.sign(x) * r
+    x = np.concatenate([np.linspace(-6, 6, 200001), 1 + np.logspace(-7, -1, 400), 1 - np.logspace(-7, -1, 400), -1 + np.logspace(-7, -1, 400),
+                        -1 - np.logspace(-7, -1, 400), np.linspace(6, 300, 5000), [0.0, 1.0, -1.0]]).astype(np.float32)
+    got = B.sx_eval(B.SX_EVAL_F_EXACT, x)
+    want = f64(x.astype(np.float64))
+    rel = np.abs(got - want) / np.maximum(1.0, np.abs(want))
+    print(f"f_exact: max relative difference to the closed form in double {rel.max():.2e}")
+    assert rel.max() <= 4e-7
+    u = want.astype(np.float32)
+    xr = B.sx_eval(B.SX_EVAL_F_INV_REFINED, u)
+    back = np.abs(f64(xr.astype(np.float64)) - u.astype(np.float64)) / np.maximum(1.0, np.abs(u))
+    print(f"f_inv_refined: max |f(f_inv(u)) - u| / max(1, |u|) {back.max():.2e}")
+    assert back.max() <= 6e-7
+    L = oracle.lib()
+    idx = np.linspace(0, len(u) - 1, 4000).astype(int)
+    worst = max(abs(float(L.so_f_inv_refined(C.c_float(u[i]))) - float(xr[i])) / max(1.0, abs(float(xr[i]))) * min(1.0, 4 * abs(abs(float(xr[i])) - 1.0) ** 0.5 + 1e-3) for i in idx)
+    print(f"f_inv_refined: max difference to the oracle's, weighted by the density {worst:.2e}")
+    assert worst <= 2e-6

@@ -62,7 +62,7 @@ def gpu_run(B, ctx, sc, mode, host=False, into=False):
         poff_t = torch.empty(sc.n_paths + 1, dtype=torch.int64, device=dev)
         cap = 16 * sc.n_segments + 64
         while True:
-            rec_t = torch.full((cap, 4 if mode == 0 else 8), float("nan"), dtype=torch.float32, device=dev)
+            rec_t = torch.full((cap, 8 if mode == 1 else 4), float("nan"), dtype=torch.float32, device=dev)
             try:
                 m = B.stroke_expand_into(ctx, tags, pts, sty, sc.affine, sc.tolerance, mode, rec_t, poff_t)
                 break
@@ -77,7 +77,7 @@ def gpu_run(B, ctx, sc, mode, host=False, into=False):
         tags, pts, sty = B.scene_to_torch(sc, pin=True)
         cap = 1 << 16
         while True:
-            out = torch.empty((cap, 4 if mode == 0 else 8), dtype=torch.float32).pin_memory()
+            out = torch.empty((cap, 8 if mode == 1 else 4), dtype=torch.float32).pin_memory()
             poff = torch.empty(sc.n_paths + 1, dtype=torch.int64).pin_memory()
             try:
                 m = B.stroke_expand_host(ctx, tags, pts, sty, sc.affine, sc.tolerance, mode, out, poff)
@@ -148,7 +148,8 @@ def oracle_run(sc, mode):
 
 
 # ---------------------------------------------------------------- element-by-element parity at oracle-sized inputs
-CASES = [("c1", None, 0), ("c2", None, 0), ("c2", None, 1), ("c3", 6000, 0), ("c4", 8000, 1), ("c5", 600, 0), ("c5", 600, 1)]
+CASES = [("c1", None, 0), ("c2", None, 0), ("c2", None, 1), ("c3", 6000, 0), ("c4", 8000, 1), ("c5", 600, 0), ("c5", 600, 1),
+         ("c1", None, 2), ("c2", None, 2), ("c3", 6000, 2), ("c5", 600, 2)]   # mode 2: SX_MODE_LINE_REFINED
 
 
 @pytest.mark.parametrize("name,npaths,mode", CASES)
@@ -187,7 +188,7 @@ def test_filled_paths_do_not_depend_on_the_tiling(B, mode):
     sc = S.with_fill(S.make("c2", n_paths=200), every=2)
     dev = "cuda:0"
     tags, pts, sty = B.scene_to_torch(sc, device=dev)
-    width = 4 if mode == 0 else 8
+    width = 8 if mode == 1 else 4
     outs = []
     for tiles in (1, 2, 8, 0):
         c = B.sx_create(0)
@@ -215,7 +216,7 @@ def test_host_buffer_entry_point_matches_device_entry_point(B, ctx, name, npaths
     assert np.array_equal(gd.angle.view(np.uint32), gh.angle.view(np.uint32))
 
 
-@pytest.mark.parametrize("name,npaths,mode", [("c1", 64, 0), ("c2", 300, 1), ("c4", 2000, 1), ("c5", 40, 0)])
+@pytest.mark.parametrize("name,npaths,mode", [("c1", 64, 0), ("c2", 300, 1), ("c4", 2000, 1), ("c5", 40, 0), ("c5", 40, 2)])
 def test_tiling_of_the_expansion_kernel_does_not_change_a_bit(B, name, npaths, mode):
     """The warps of the expansion kernel work on tiles of 32, 16 or 8 segments (adapted on the device); a tile that
     does not fit its shared-memory tables is redone in sub-tiles of 8 segments (forced with 2), and a sub-tile that
@@ -224,7 +225,7 @@ def test_tiling_of_the_expansion_kernel_does_not_change_a_bit(B, name, npaths, m
     sc = S.make(name, n_paths=npaths)
     dev = "cuda:0"
     tags, pts, sty = B.scene_to_torch(sc, device=dev)
-    width = 4 if mode == 0 else 8
+    width = 8 if mode == 1 else 4
     outs = []
     for tiles in (1, 2, 4, 8, 16, 32, 0):
         c = B.sx_create(0)
@@ -253,7 +254,8 @@ def test_tiling_of_the_expansion_kernel_does_not_change_a_bit(B, name, npaths, m
 
 
 # ---------------------------------------------------------------- the same invariant checks the oracle passes
-@pytest.mark.parametrize("name,npaths,mode", [("c1", 128, 0), ("c2", 240, 0), ("c2", 240, 1), ("c3", 300, 0), ("c4", 200, 1), ("c5", 100, 0), ("c5", 100, 1)])
+@pytest.mark.parametrize("name,npaths,mode", [("c1", 128, 0), ("c2", 240, 0), ("c2", 240, 1), ("c3", 300, 0), ("c4", 200, 1), ("c5", 100, 0), ("c5", 100, 1),
+                                              ("c1", 128, 2), ("c5", 100, 2)])
 def test_gpu_output_passes_the_invariants(B, ctx, name, npaths, mode):
     """Winding / tolerance invariants on 100 paths per config (the same check the oracle's outlines pass)."""
     from test_oracle_outline import _winding_band
@@ -262,7 +264,7 @@ def test_gpu_output_passes_the_invariants(B, ctx, name, npaths, mode):
     assert ck.watertight_violations(g.xy, g.path_off) == 0
     rng = np.random.default_rng(123)
     paths = rng.choice(npaths, size=min(npaths, 100), replace=False)
-    st = _winding_band(sc, g, paths, rng, mode, n_pts=600)
+    st = _winding_band(sc, g, paths, rng, 1 if mode == 1 else 0, n_pts=600)
     assert st["inside"] > 5000 and st["outside"] > 5000
     assert st["neg"] == 0 and st["inside_fail"] == 0 and st["outside_fail"] == 0, st
 
@@ -444,7 +446,7 @@ def _full_size(B, ctx, name, mode, every, seed):
     B.sx_set_option(ctx, B.SX_OPT_KEEP_SEGMENT_INFO, 1)
     try:
         total = B.sx_count(ctx, tags, pts, sty, sc.affine, sc.tolerance, mode, poff)
-        width = 4 if mode == 0 else 8
+        width = 8 if mode == 1 else 4
         out = torch.empty((total, width), dtype=torch.float32, device=dev)
         m = B.stroke_expand_into(ctx, tags, pts, sty, sc.affine, sc.tolerance, mode, out, poff)
         torch.cuda.synchronize()
@@ -490,6 +492,10 @@ def test_full_size_c3(B, ctx):
     _full_size(B, ctx, "c3", 0, 16, 7)
 
 
+def test_full_size_c3_refined(B, ctx):
+    _full_size(B, ctx, "c3", 2, 16, 3)
+
+
 def test_full_size_c4(B, ctx):
     _full_size(B, ctx, "c4", 1, 64, 8)
 
@@ -504,7 +510,7 @@ def test_long_chains_tight_tolerance(B, ctx):
     per iteration and than a tile, non-uniform (f_approx) subdivision, both write-kernel variants' table path."""
     sc = S.make("c1", n_paths=6)
     sc["tolerance"] = 0.002
-    for mode in (0, 1):
+    for mode in (0, 1, 2):
         g = gpu_run(B, ctx, sc, mode)
         r = oracle_run(sc, mode)
         compare(sc, mode, g, r)
