@@ -38,6 +38,9 @@ def lib():
         L.so_expand.restype = C.c_int
         L.so_expand.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64, C.c_void_p,
                                 C.c_float, C.c_int, C.POINTER(_Result)]
+        L.so_expand_dashed.restype = C.c_int
+        L.so_expand_dashed.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64, C.c_void_p,
+                                       C.c_float, C.c_int, C.c_void_p, C.c_int, C.c_float, C.POINTER(_Result)]
         L.so_free.argtypes = [C.POINTER(_Result)]
         L.so_tag_walk.restype = C.c_int
         L.so_tag_walk.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -99,8 +102,9 @@ def piece_expand(k0, k1, L, h, tol_fl, mode, x0=0.0, y0=0.0, dir0=0.0):
     return _collect(r, 1, 1)
 
 
-def expand(tags, points, styles, affine, tolerance, mode):
-    """Run the oracle on host numpy streams; returns OracleResult (copies; C buffers are freed)."""
+def expand(tags, points, styles, affine, tolerance, mode, dash=None, phase=0.0):
+    """Run the oracle on host numpy streams; returns OracleResult (copies; C buffers are freed).  dash: the call's dash
+    pattern (2, 4, 6 or 8 positive lengths in output px) for the paths whose style has bit 1 of `fill` set; phase >= 0."""
     L = lib()
     tags = np.ascontiguousarray(tags, dtype=np.uint8)
     points = np.ascontiguousarray(points, dtype=np.float32)
@@ -109,8 +113,13 @@ def expand(tags, points, styles, affine, tolerance, mode):
     assert styles.dtype.itemsize == 16 and affine.shape == (6,)
     r = _Result()
     n, p = tags.shape[0], styles.shape[0]
-    rc = L.so_expand(tags.ctypes.data, n, points.ctypes.data, points.shape[0], styles.ctypes.data, p,
-                     affine.ctypes.data, float(tolerance), int(mode), C.byref(r))
+    if dash is None:
+        rc = L.so_expand(tags.ctypes.data, n, points.ctypes.data, points.shape[0], styles.ctypes.data, p,
+                         affine.ctypes.data, float(tolerance), int(mode), C.byref(r))
+    else:
+        d = np.ascontiguousarray(dash, dtype=np.float32)
+        rc = L.so_expand_dashed(tags.ctypes.data, n, points.ctypes.data, points.shape[0], styles.ctypes.data, p,
+                                affine.ctypes.data, float(tolerance), int(mode), d.ctypes.data, int(d.shape[0]), float(phase), C.byref(r))
     if rc != 0:
         raise ValueError(f"oracle so_expand failed: {rc}")
     return _collect(r, n, p)

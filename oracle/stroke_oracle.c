@@ -34,7 +34,8 @@ typedef struct {
     float miter_limit;
     uint8_t join; /* 0 miter 1 round 2 bevel */
     uint8_t cap;  /* 0 butt 1 square 2 round */
-    uint16_t fill; /* bit 0: the path is FILLED, not stroked (Alg. 1); width, join, cap are then ignored */
+    uint16_t fill; /* bit 0: the path is FILLED, not stroked (Alg. 1); width, join, cap are then ignored;
+                      bit 1: the stroke is DASHED with the call's dash pattern (so_expand_dashed) */
     uint32_t rsv;
 } so_style;
 
@@ -287,6 +288,14 @@ typedef struct {
     float tol_es, tol_fl;
     uint32_t cur_seg;
     int fill;        /* the current path is filled: offset 0, one side (Alg. 1) */
+    /* dashing (reading R-23; see dash_piece) */
+    int nd;                  /* entries of the dash pattern (0: none) */
+    uint64_t dq[8], period, phase_q;   /* the pattern, its sum and the phase in units of 2^-16 px */
+    int dashed;              /* the current path is dashed */
+    uint64_t pos;            /* arc length from the start of the current subpath to the start of the next piece, same units */
+    uint64_t sp_total;       /* arc length of the current subpath */
+    int measuring;           /* first pass over a subpath: pieces only add their length to pos */
+    const void* style;       /* the current path's style (caps of the dashes) */
 } ctx_t;
 
 static int push_rec(ctx_t* c, v2d a, v2d b, double angle, int kind) {
@@ -579,6 +588,94 @@ static int piece_records(ctx_t* c, piece_t* p, float h) {
     return 0;
 }
 
+/* ================================================================== dashing
+ * "the core algorithm is prefix sum applied to segment length, and the Euler spiral representation is particularly well
+ * suited" (L543); "Given its parameterization by arc length ..." (L589).  The paper stops there; reading R-23 of DESIGN.md:
+ *
+ *   - The pattern is nd in {2, 4, 6, 8} positive lengths (on, off, on, off, ...) and a phase >= 0, in output px, the same for
+ *     every dashed path of the call; it restarts at every subpath.  Lengths are integers in units of 2^-16 px
+ *     (llrintf(x * 65536), at least 1 per pattern entry): sums are then exact and do not depend on the order of addition,
+ *     which is what lets a parallel prefix sum reproduce this sequential walk bit for bit.
+ *   - The arc length of a curve is that of its Euler-spiral pieces (L = chord / c, App. A), piece by piece in the order of
+ *     Alg. 2; of a line (or a degenerate curve, R-1b) the distance of its end points.
+ *   - Pattern entry j covers [a, b) of the subpath's arc length; the on-entries (j even) are the dashes.  The part of a dash
+ *     inside a piece [S, S + L) is the sub-range ta = (a - S) / L .. tb = (b - S) / L of the piece (integers converted to fp32,
+ *     one division), clipped to [0, 1]: an Euler-spiral piece again, with k0' = (tb - ta)(k0 + k1 ((ta + tb)/2 - 1/2)),
+ *     k1' = k1 (tb - ta)^2, L' = L (tb - ta), from the spiral's point and tangent at ta to those at tb.  It goes through the
+ *     SAME flattening as an undashed piece (both sides, cusps, evolutes).
+ *   - A dash begins where its entry begins (a in [S, S + L): start cap before the sub-range's records) or at arc length 0; it
+ *     ends where its entry ends (b in (S, S + L]: end cap after them) or at the subpath's total arc length.  Everything is
+ *     decided from arc-length positions alone (a piece without length emits nothing).  Caps are the path's cap style.  A
+ *     closed subpath is dashed like an open one (no closing join, no merging of its last dash with its first).
+ *   - The join after a segment is emitted iff a dash covers the junction strictly inside (a < S_next < b, 0 < S_next < total).
+ *   - Record order within a segment: per piece in increasing t, per dash in increasing arc length:
+ *     [start cap][-h side][+h side][end cap]; then the join. */
+static int emit_cap(ctx_t* c, const so_style* st, v2f Vf, v2f T, float h, v2d from, v2d to);
+static v2d round32(v2d a) { v2d r = {(double)(float)a.x, (double)(float)a.y}; return r; }
+
+static int dash_sub_piece(ctx_t* c, piece_t* p, float h, float ta, float tb, int starts, int ends, int line) {
+    const so_style* st = (const so_style*)c->style;
+    piece_t q = *p;
+    if (line) {
+        /* a straight piece: points pa + t ch, constant tangent */
+        if (ta != 0.0f) { q.pa.x = (double)(float)(p->pa.x + (double)ta * (double)p->ch.x); q.pa.y = (double)(float)(p->pa.y + (double)ta * (double)p->ch.y); }
+        if (tb != 1.0f) { q.pb.x = (double)(float)(p->pa.x + (double)tb * (double)p->ch.x); q.pb.y = (double)(float)(p->pa.y + (double)tb * (double)p->ch.y); }
+    } else if (ta != 0.0f || tb != 1.0f) {
+        float dt = tb - ta, tm = 0.5f * (ta + tb) - 0.5f;
+        q.k0 = dt * (p->k0 + p->k1 * tm);
+        q.k1 = p->k1 * dt * dt;
+        q.L = p->L * dt;
+        if (!(q.L > 1e-12f)) q.L = 1e-12f;
+        /* a cut end: the spiral's point, rounded to fp32 (an uncut end keeps the piece's own end point and tangent) */
+        if (ta != 0.0f) { v2d TA = es_tangent(p, ta); q.pa = round32(es_point(p, ta)); q.ua = v2((float)TA.x, (float)TA.y); }
+        if (tb != 1.0f) { v2d TB = es_tangent(p, tb); q.pb = round32(es_point(p, tb)); q.ub = v2((float)TB.x, (float)TB.y); }
+        q.ch = v2((float)(q.pb.x - q.pa.x), (float)(q.pb.y - q.pa.y));
+    }
+    v2f Va = v2((float)q.pa.x, (float)q.pa.y), Vb = v2((float)q.pb.x, (float)q.pb.y);
+    if (starts && emit_cap(c, st, Va, v2(-q.ua.x, -q.ua.y), h, offset_point(q.pa, q.ua, h), offset_point(q.pa, q.ua, -h))) return -1;
+    if (line) {
+        if (push_rec(c, offset_point(q.pa, q.ua, -h), offset_point(q.pb, q.ub, -h), 0, K_OFFSET)) return -1;
+        if (push_rec(c, offset_point(q.pb, q.ub, h), offset_point(q.pa, q.ua, h), 0, K_OFFSET | K_PLUS)) return -1;
+    } else if (piece_records(c, &q, h)) return -1;
+    if (ends && emit_cap(c, st, Vb, q.ub, h, offset_point(q.pb, q.ub, -h), offset_point(q.pb, q.ub, h))) return -1;
+    return 0;
+}
+
+/* one piece (an accepted Euler spiral with k0, k1, L set, or a straight segment: line != 0, L = its length) under the dash
+ * pattern; advances c->pos */
+static int dash_piece(ctx_t* c, piece_t* p, float h, int line) {
+    uint64_t Lq = (uint64_t)llrintf(p->L * 65536.0f);
+    uint64_t S = c->pos, E = S + Lq;
+    c->pos = E;
+    if (c->measuring || Lq == 0) return 0;   /* (a piece without length carries no part of a dash) */
+    if (!line) so_es_integral(p->k0, p->k1, 1.0, &p->z1x, &p->z1y);   /* Z(1): es_point of the piece itself */
+    uint64_t u = (S + c->phase_q) % c->period;   /* where in the pattern the piece starts */
+    int j = 0;
+    while (u >= c->dq[j]) { u -= c->dq[j]; j++; }
+    uint64_t s = S;
+    while (s < E) {
+        uint64_t e = s + (c->dq[j] - u);         /* end of entry j */
+        if ((j & 1) == 0) {
+            uint64_t b = e < E ? e : E;
+            int starts = (u == 0) || (s == 0);
+            int ends = (e <= E) || (E == c->sp_total);
+            float ta = s == S ? 0.0f : (float)(s - S) / (float)Lq;
+            float tb = b == E ? 1.0f : (float)(b - S) / (float)Lq;
+            if (dash_sub_piece(c, p, h, ta, tb, starts, ends, line)) return -1;
+        }
+        s = e; u = 0; j = (j + 1) % c->nd;
+    }
+    return 0;
+}
+/* does a dash cover arc position s strictly inside (a < s < b)? */
+static int dash_covers(const ctx_t* c, uint64_t s) {
+    if (s == 0 || s >= c->sp_total) return 0;
+    uint64_t u = (s + c->phase_q) % c->period;
+    int j = 0;
+    while (u >= c->dq[j]) { u -= c->dq[j]; j++; }
+    return (j & 1) == 0 && u > 0;
+}
+
 static int emit_piece(ctx_t* c, piece_t* p, float h) {
     float cc;
     so_ghi(p->th0, p->th1, &p->k1, &cc);
@@ -586,6 +683,7 @@ static int emit_piece(ctx_t* c, piece_t* p, float h) {
     if (!(cc > 0.05f)) cc = 0.05f; /* far outside the polynomial's range (|theta| near pi): keep L finite */
     p->L = p->chord / cc;
     if (!(p->L > 1e-12f)) p->L = 1e-12f; /* zero-length piece accepted at DT_MIN */
+    if (c->dashed) return dash_piece(c, p, h, 0);
     return piece_records(c, p, h);
 }
 
@@ -693,7 +791,7 @@ static int flatten_cubic(ctx_t* c, const seg_t* s, float h) {
         float th0, th1, chord;
         v2f ch = sub(next_p, last_p);
         float err = so_fit_error(last_u, next_u, last_qmag, next_qmag, ch, dt, &th0, &th1, &chord);
-        c->out->stats[ST_FIT_ITERS]++;
+        if (!c->measuring) c->out->stats[ST_FIT_ITERS]++;
         if (err <= c->tol_es || dt <= DT_MIN) {
             piece_t p;
             p.pa.x = (double)s->P0.x + (double)last_p.x; p.pa.y = (double)s->P0.y + (double)last_p.y;
@@ -798,9 +896,22 @@ void so_free(so_result* r) {
  * increasing t: [-h side, forward] [+h side, mirrored]; then the join [-h side][+h side], or, on the
  * last segment of an open subpath, [end cap][start cap] (the thread at the subpath end draws the start
  * cap, as the paper's marker thread does, L345). */
-int so_expand(const uint8_t* tags, uint64_t n_tags, const float* pts, uint64_t n_points, const so_style* styles,
-              uint64_t n_paths, const float* affine, float tolerance, int mode, so_result* out) {
+static int line_piece(ctx_t* c, const seg_t* s, float h) {   /* a straight segment as a piece of the dash walk */
+    piece_t p;
+    memset(&p, 0, sizeof(p));
+    p.pa.x = s->P0.x; p.pa.y = s->P0.y; p.pb.x = s->P3.x; p.pb.y = s->P3.y;
+    p.ua = s->ts; p.ub = s->te;
+    p.ch = sub(s->P3, s->P0);
+    p.chord = sqrtf(len2(p.ch));
+    p.L = p.chord;
+    return dash_piece(c, &p, h, 1);
+}
+
+static int expand_impl(const uint8_t* tags, uint64_t n_tags, const float* pts, uint64_t n_points, const so_style* styles,
+                       uint64_t n_paths, const float* affine, float tolerance, int mode, const float* dash, int n_dash, float phase, so_result* out) {
     memset(out, 0, sizeof(*out));
+    if (n_dash != 0 && (n_dash < 2 || n_dash > 8 || (n_dash & 1) || !dash || !(phase >= 0.0f) || !isfinite(phase))) return -1;
+    for (int k = 0; k < n_dash; k++) if (!(dash[k] > 0.0f) || !isfinite(dash[k])) return -1;
     if (!(tolerance > 0) || (mode != MODE_LINE && mode != MODE_ARC && mode != MODE_LINE_REFINED)) return -1;
     float det = affine[0] * affine[3] - affine[1] * affine[2];
     if (!isfinite(det) || det == 0.0f) return -1;
@@ -812,11 +923,19 @@ int so_expand(const uint8_t* tags, uint64_t n_tags, const float* pts, uint64_t n
     int rc = so_tag_walk(tags, n_tags, n_points, n_paths, out->pt_off, out->path_idx, out->sp_first);
     if (rc) { so_free(out); return rc; }
     ctx_t c;
+    memset(&c, 0, sizeof(c));
     c.out = out;
     c.mode = mode;
     c.tol_es = 0.1f * tolerance; /* R-13 */
     c.tol_fl = (mode == MODE_LINE_REFINED ? 0.9f : 0.8f) * tolerance;   /* R-22: the 6 % of f_approx (L145) no longer needs the margin */
     float scale = sqrtf(fabsf(det)); /* R-14 */
+    c.nd = n_dash; c.period = 0; c.dashed = 0; c.measuring = 0; c.pos = 0; c.sp_total = 0;
+    for (int k = 0; k < n_dash; k++) {
+        c.dq[k] = (uint64_t)llrintf(dash[k] * 65536.0f);
+        if (c.dq[k] == 0) c.dq[k] = 1;
+        c.period += c.dq[k];
+    }
+    c.phase_q = n_dash ? (uint64_t)llrintf(phase * 65536.0f) : 0;
     uint64_t next_path = 0;
     for (uint64_t i = 0; i < n_tags; i++) {
         uint64_t before = out->n_rec;
@@ -849,6 +968,32 @@ int so_expand(const uint8_t* tags, uint64_t n_tags, const float* pts, uint64_t n
         } else if (h > 0.0f && isfinite(h)) { /* width <= 0 or non-finite: the path emits nothing */
             seg_t s;
             load_segment(tags, pts, affine, out->pt_off, i, &s);
+            c.dashed = c.nd > 0 && (st->fill & 2);
+            c.style = st;
+            if (c.dashed && out->sp_first[i] == i) {
+                /* the subpath's arc length: the same walk, measuring only (on the GPU: the prefix sum of L543) */
+                c.measuring = 1; c.pos = 0;
+                for (uint64_t j = i;; j++) {
+                    seg_t m;
+                    load_segment(tags, pts, affine, out->pt_off, j, &m);
+                    if (m.kind == 1 || m.degenerate) { if (line_piece(&c, &m, h)) goto oom; }
+                    else if (flatten_cubic(&c, &m, h)) goto oom;
+                    if (((tags[j] >> 2) | (tags[j] >> 4)) & 1) break;
+                }
+                c.sp_total = c.pos; c.measuring = 0; c.pos = 0;
+            }
+            if (c.dashed) {
+                if (s.kind == 1 || s.degenerate) { out->stats[ST_LINE_SEGS]++; if (line_piece(&c, &s, h)) goto oom; }
+                else { out->stats[ST_CURVE_SEGS]++; if (flatten_cubic(&c, &s, h)) goto oom; }
+                uint8_t tg = tags[i];
+                if (!(((tg >> 2) | (tg >> 4)) & 1) && dash_covers(&c, c.pos)) {
+                    seg_t n;
+                    load_segment(tags, pts, affine, out->pt_off, i + 1, &n);
+                    if (emit_join(&c, st, s.P3, s.te, n.P0, n.ts, h)) goto oom;
+                }
+                out->seg_count[i] = (uint32_t)(out->n_rec - before);
+                continue;
+            }
             if (s.kind == 1 || s.degenerate) {
                 /* straight fast path (R-1b): the two offset lines are exact */
                 v2d V0 = {s.P0.x, s.P0.y}, V3 = {s.P3.x, s.P3.y};
@@ -890,6 +1035,17 @@ oom:
     return -1;
 }
 
+int so_expand(const uint8_t* tags, uint64_t n_tags, const float* pts, uint64_t n_points, const so_style* styles,
+              uint64_t n_paths, const float* affine, float tolerance, int mode, so_result* out) {
+    return expand_impl(tags, n_tags, pts, n_points, styles, n_paths, affine, tolerance, mode, NULL, 0, 0.0f, out);
+}
+/* the same with a dash pattern (n_dash in {2, 4, 6, 8} positive lengths, phase >= 0, output px) for the paths whose style
+ * has bit 1 of `fill` set: dash_piece above */
+int so_expand_dashed(const uint8_t* tags, uint64_t n_tags, const float* pts, uint64_t n_points, const so_style* styles,
+                     uint64_t n_paths, const float* affine, float tolerance, int mode, const float* dash, int n_dash, float phase, so_result* out) {
+    return expand_impl(tags, n_tags, pts, n_points, styles, n_paths, affine, tolerance, mode, dash, n_dash, phase, out);
+}
+
 /* ------------------------------------------------------------------ thin exports used by the pins */
 void so_fit_error_export(const float* u0, const float* u1, float q0mag, float q1mag, const float* ch, float dt, float* out4) {
     float th0, th1, chord;
@@ -910,6 +1066,7 @@ int so_piece_expand(float k0, float k1, float L, float x0, float y0, float dir0,
     out->path_idx = (uint32_t*)calloc(2, sizeof(uint32_t));
     out->sp_first = (uint32_t*)calloc(2, sizeof(uint32_t));
     ctx_t c;
+    memset(&c, 0, sizeof(c));
     c.out = out; c.mode = mode; c.tol_es = 0; c.tol_fl = tol_fl; c.cur_seg = 0; c.fill = (h == 0.0f);   /* h = 0: the piece of a filled path */
     piece_t p;
     memset(&p, 0, sizeof(p));

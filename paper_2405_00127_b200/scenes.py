@@ -268,6 +268,17 @@ def with_fill(scene, every=1, offset=0):
     return out
 
 
+def with_dash(scene, every=1, offset=0):
+    """Copy of the scene in which every `every`-th path (starting at `offset`) is DASHED with the call's dash pattern
+    (bit 1 of the style's `fill` field, no arithmetic here)."""
+    st = scene["styles"].copy()
+    st["fill"][offset::every] |= 2
+    out = Scene(scene)
+    out["styles"] = st
+    out["name"] = scene["name"] + "-dash"
+    return out
+
+
 def subset_paths(scene, path_ids):
     """Sub-scene holding only the given paths (paths are independent units): used to run the oracle on a
     sample of a large scene.  Each path here is one subpath."""
