@@ -64,7 +64,8 @@ typedef struct {
     uint16_t fill;     /* bit 0: FILL the path instead of stroking it (Alg. 1: "if style is fill then
                           flatten_cubic(segment, 0)"): its segments are flattened at offset 0, one record chain per
                           segment in path direction, an open subpath is closed by one line from its last point to its
-                          first (kind SX_KIND_CLOSE); width, join, cap and miter_limit are ignored                     */
+                          first (kind SX_KIND_CLOSE); width, join, cap and miter_limit are ignored.
+                          bit 1: the stroke is DASHED with the context's dash pattern (sx_set_dash)                   */
     uint32_t _rsv;
 } sx_style; /* 16 bytes */
 
@@ -227,6 +228,21 @@ enum {
                                      reference walk.  The records do not depend on it (tests/test_gpu_parity.py).      */
 };
 sx_status sx_set_option(sx_ctx* ctx, int32_t option, uint64_t value);
+
+/* Dashing on the GPU.  PAPER.md L543: "It is conceptually straightforward to implement on GPU; the core
+ * algorithm is prefix sum applied to segment length, and the Euler spiral representation is particularly well suited";
+ * L589: "... an approach based on parallel prefix sums of segment arc lengths".  The paper dashes on the CPU; the definition
+ * used here is reading R-23 of DESIGN.md (also at the top of csrc/sx_dash.cuh):
+ *   h_lengths[n]: n in {2, 4, 6, 8} positive lengths (on, off, on, off, ...), phase >= 0, in OUTPUT px (after the affine);
+ *   host pointer, copied.  n = 0 clears the pattern.  SX_E_INVALID_ARG otherwise.
+ * While a pattern is set, every stroked path whose style has bit 1 of `fill` set is dashed in the following sx_count /
+ * stroke_expand* calls on this context: the pattern restarts at every subpath; arc length is that of the Euler-spiral pieces
+ * (integers in units of 2^-16 px, summed by a parallel prefix sum); every dash is an open sub-stroke with the path's caps at
+ * both ends, whose parts inside the pieces go through the same flattening as undashed pieces; joins are emitted where a dash
+ * covers the junction; a closed subpath is dashed like an open one.  Record order within a segment: per piece, per dash
+ * [start cap][-h side][+h side][end cap], then the join.  A dashed segment of 65536 px or more is refused (SX_E_BAD_STREAM).
+ * Calls with a pattern set run the thread-per-segment kernels of csrc/sx_dash.cuh for all their paths. */
+sx_status sx_set_dash(sx_ctx* ctx, const float* h_lengths, int32_t n, float phase);
 
 /* Statistics of the last count pass on the context (synchronises `cuda_stream`): h_out4[0] tiles done in one
  * go from shared memory, [1] tiles redone in sub-tiles, [2] segments that took the thread-per-segment walk, [3] the

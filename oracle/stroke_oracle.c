@@ -945,6 +945,7 @@ static int expand_impl(const uint8_t* tags, uint64_t n_tags, const float* pts, u
         const so_style* st = &styles[path];
         float h = 0.5f * st->width * scale;
         c.fill = st->fill & 1;
+        c.dashed = 0;   /* (set below for a dashed stroke: a filled path is never dashed) */
         if (c.fill) {
             /* Alg. 1: a filled path is flattened with offset 0; an open subpath is closed by a line from its last
              * point to its first (always emitted, possibly of zero length: counts stay a function of the tags) */

@@ -24,7 +24,7 @@ ARC_DTYPE = np.dtype([("x0", "<f4"), ("y0", "<f4"), ("x1", "<f4"), ("y1", "<f4")
 SX_OPT_KEEP_SEGMENT_INFO, SX_OPT_TILE_SEGMENTS, SX_OPT_TIME_KERNELS = 1, 2, 3
 
 EXPORTS = ["sx_create", "sx_destroy", "sx_count", "sx_write", "stroke_expand", "stroke_expand_into", "stroke_expand_host",
-           "sx_bin_lines", "sx_segment_info", "sx_last_error", "sx_set_option", "sx_call_stats", "sx_kernel_times", "sx_measure_issue_peaks", "sx_eval", "sx_launch_count",
+           "sx_bin_lines", "sx_segment_info", "sx_last_error", "sx_set_option", "sx_set_dash", "sx_call_stats", "sx_kernel_times", "sx_measure_issue_peaks", "sx_eval", "sx_launch_count",
            "sx_strerror"]
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
@@ -57,6 +57,7 @@ def lib():
         L.sx_segment_info.argtypes = [vp] + [C.POINTER(vp)] * 5
         L.sx_last_error.argtypes = [vp, vp]
         L.sx_set_option.argtypes = [vp, i32, u64]
+        L.sx_set_dash.argtypes = [vp, vp, i32, f32]
         L.sx_call_stats.argtypes = [vp, C.POINTER(u64), vp]
         L.sx_eval.argtypes = [C.c_int32, C.c_int32, vp, vp, u64]
         L.sx_bin_lines.argtypes = [vp, vp, u64, C.c_uint32, C.c_uint32, vp, vp, u64, C.POINTER(u64), vp]
@@ -297,6 +298,15 @@ def sx_eval(what, values, device=0):
     out = np.zeros(n, dtype=np.float32)
     _check(lib().sx_eval(int(device), int(what), C.c_void_p(v.ctypes.data), C.c_void_p(out.ctypes.data), n), "sx_eval")
     return out
+
+
+def sx_set_dash(ctx, lengths=None, phase=0.0):
+    """Dash pattern of the context: 2, 4, 6 or 8 positive lengths in output px and a phase; None clears it."""
+    if lengths is None or len(lengths) == 0:
+        _check(lib().sx_set_dash(ctx, None, 0, C.c_float(0.0)), "sx_set_dash")
+        return
+    v = np.ascontiguousarray(lengths, dtype=np.float32)
+    _check(lib().sx_set_dash(ctx, C.c_void_p(v.ctypes.data), int(v.shape[0]), C.c_float(float(phase))), "sx_set_dash")
 
 
 def sx_launch_count(ctx):

@@ -15,7 +15,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libstroke_expand.so")
-SOURCES = [os.path.join(CSRC, "sx_kernels.cu"), os.path.join(CSRC, "sx_refined.cu")]   # (the second: the kernels of SX_MODE_LINE_REFINED)
+SOURCES = [os.path.join(CSRC, "sx_kernels.cu"), os.path.join(CSRC, "sx_refined.cu"),
+           os.path.join(CSRC, "sx_dash.cu")]   # (the second: the kernels of SX_MODE_LINE_REFINED; the third: dashing)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-fmad=false",
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]
 

@@ -18,6 +18,7 @@
 #include "sx_bin.cuh"
 #include "sx_peaks.cuh"
 #include "sx_refined.h"
+#include "sx_dash.h"
 
 // ====================================================================== host side
 static thread_local cudaError_t g_last_cuda = cudaSuccess;
@@ -58,6 +59,13 @@ struct sx_ctx {
     bool counted, total_known;
     uint64_t total;
     uint64_t launches;
+    // dashing (sx_set_dash): the pattern in units of 2^-16 px; scratch [ticket, total: 64 B][look-back words][path offsets of
+    // the length scan] and the per-segment arrays [seg_pos u64][sp_total u64][seg_len u32]
+    uint32_t n_dash;
+    unsigned long long dash_q[8], dash_period, dash_phase_q;
+    uint8_t* dash_area; uint64_t dash_area_bytes;
+    uint8_t* dash_buf; uint64_t dash_buf_segs;
+    sx_dash_launch D;
     // scratch of sx_bin_lines: [ticket, total: 64 B][look-back words][tile counters][tile cursors]
     uint8_t* bin_area; uint64_t bin_bytes;
     // staging for stroke_expand_host
@@ -138,6 +146,45 @@ static sx_status check_inputs(const uint8_t* d_tags, uint64_t n_tags, const floa
     return SX_OK;
 }
 
+// dashing: the stages before the allocation scan (the pattern was set with sx_set_dash)
+static sx_status run_dash_count(sx_ctx* c, const uint8_t* d_tags, uint32_t n, uint64_t n_paths, cudaStream_t s) {
+    const uint64_t st_bytes = states_bytes(n), head = 64;
+    const uint64_t need_area = head + st_bytes + (n_paths + 1) * 8;
+    if (need_area > c->dash_area_bytes) {
+        if (c->dash_area) SX_CUDA(cudaFree(c->dash_area));
+        c->dash_area = nullptr; c->dash_area_bytes = 0;
+        SX_CUDA(cudaMalloc(&c->dash_area, round_up(need_area + need_area / 4, 256)));
+        c->dash_area_bytes = round_up(need_area + need_area / 4, 256);
+    }
+    if (n > c->dash_buf_segs) {
+        if (c->dash_buf) SX_CUDA(cudaFree(c->dash_buf));
+        c->dash_buf = nullptr; c->dash_buf_segs = 0;
+        const uint64_t cap = round_up(n + n / 8 + 64, 64);
+        SX_CUDA(cudaMalloc(&c->dash_buf, cap * (4 + 8 + 8)));
+        c->dash_buf_segs = cap;
+    }
+    SX_CUDA(cudaMemsetAsync(c->dash_area, 0, head + st_bytes, s));
+    sx_dash_launch& D = c->D;
+    D.params = &c->C.P;
+    D.nd = c->n_dash;
+    for (int k = 0; k < 8; k++) D.dq[k] = c->dash_q[k];
+    D.period = c->dash_period; D.phase_q = c->dash_phase_q;
+    D.seg_pos = reinterpret_cast<unsigned long long*>(c->dash_buf);
+    D.sp_total = D.seg_pos + c->dash_buf_segs;
+    D.seg_len = reinterpret_cast<uint32_t*>(D.sp_total + c->dash_buf_segs);
+    D.seg_count = c->seg_count; D.seg_off = c->seg_off;
+    D.out = nullptr; D.cap_records = 0; D.wide = 0; D.err = ctx_err(c);
+    sxd_launch(0, &D, n, s);
+    uint32_t tiles = (n + sx::kCntTile - 1) / sx::kCntTile;
+    sx::k_alloc_scan<<<tiles, sx::kScanThreads, 0, s>>>(D.seg_len, n, d_tags, c->path_idx, (uint32_t)n_paths, reinterpret_cast<uint64_t*>(D.seg_pos),
+                                                       reinterpret_cast<uint64_t*>(c->dash_area + head + st_bytes), reinterpret_cast<uint64_t*>(c->dash_area + 8),
+                                                       reinterpret_cast<uint64_t*>(c->dash_area + head), reinterpret_cast<uint32_t*>(c->dash_area), ctx_err(c));
+    sxd_launch(1, &D, n, s);
+    sxd_launch(2, &D, n, s);
+    c->launches += 3;   // (+ the count launch the caller books)
+    return SX_OK;
+}
+
 // phase 1: resets the per-call device state and runs (a) the tag scan, (b) the count pass, (c) the allocation scan
 static sx_status run_count(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, const float* d_points_xy, uint64_t n_points,
                            const sx_style* d_styles, uint64_t n_paths, const float* h_affine, float tolerance, int32_t mode,
@@ -191,7 +238,11 @@ static sx_status run_count(sx_ctx* c, const uint8_t* d_tags, uint64_t n_tags, co
     // persistent one-warp blocks: no more of them than there are tiles of the smallest size
     uint64_t tiles = (n + sx::kCtTileMin - 1) / sx::kCtTileMin;
     unsigned grid = (unsigned)(tiles < (uint64_t)c->count_blocks ? tiles : (uint64_t)c->count_blocks);
-    if (mode == SX_MODE_LINE_REFINED) sxr_launch_count(&C, grid, s);   // (sx_refined.cu: the same kernel with the refined density integral)
+    if (c->n_dash) {
+        // dashing (sx_dash.cuh): arc lengths, their prefix sum, subpath totals, then the count with the pattern
+        sx_status rd = run_dash_count(c, d_tags, n, n_paths, s);
+        if (rd != SX_OK) return rd;
+    } else if (mode == SX_MODE_LINE_REFINED) sxr_launch_count(&C, grid, s);   // (sx_refined.cu: the same kernel with the refined density integral)
     else sx::k_count<<<grid, 32, sizeof(sx::CtWarp), s>>>(C);
     if (c->time_kernels) SX_CUDA(cudaEventRecord(c->ev[2], s));
     uint32_t n_cnt_tiles = (n + sx::kCntTile - 1) / sx::kCntTile;
@@ -215,6 +266,14 @@ static sx_status run_write(sx_ctx* c, void* d_out_records, uint64_t cap_records,
     SX_CUDA(cudaEventRecord(c->fork, s));
     for (int k = 0; k < kSideStreams; k++) SX_CUDA(cudaStreamWaitEvent(c->side[k], c->fork, 0));
     const unsigned segment_blocks = (n + sx::kWrThreads - 1) / sx::kWrThreads;
+    if (c->n_dash) {   // dashing: one writer, thread per segment (sx_dash.cuh)
+        c->D.out = d_out_records; c->D.cap_records = cap_records; c->D.wide = c->W.wide;
+        sxd_launch(3, &c->D, n, s);
+        c->launches += 1;
+        if (c->time_kernels) { SX_CUDA(cudaEventRecord(c->ev[4], s)); c->timed = true; }
+        SX_CUDA(cudaGetLastError());
+        return SX_OK;
+    }
     if (c->W.P.mode == SX_MODE_LINE_REFINED) {
         sxr_launch_writers(&c->W, c->general_blocks, c->simple_blocks, segment_blocks, c->sm_count, s, c->side[0], c->side[1], c->side[2]);
     } else {
@@ -305,6 +364,8 @@ sx_status sx_destroy(sx_ctx* c) {
     cudaFree(c->sync_area);
     cudaFree(c->d_hint);
     cudaFree(c->bin_area);
+    cudaFree(c->dash_area);
+    cudaFree(c->dash_buf);
     cudaFree(c->st_in);
     cudaFree(c->st_out);
     cudaFree(c->st_path);
@@ -507,6 +568,23 @@ sx_status sx_last_error(sx_ctx* c, void* cuda_stream) {
     uint32_t flags = static_cast<uint32_t>(c->h_pinned[1] & 0xffffffffu);
     if (flags & sx::kErrBadStream) return SX_E_BAD_STREAM;
     if (flags & sx::kErrCapacity) return SX_E_CAPACITY;
+    return SX_OK;
+}
+
+sx_status sx_set_dash(sx_ctx* c, const float* h_lengths, int32_t n, float phase) {
+    if (!c) return SX_E_INVALID_ARG;
+    if (n == 0) { c->n_dash = 0; return SX_OK; }
+    if (!h_lengths || n < 2 || n > 8 || (n & 1) || !(phase >= 0.0f) || !isfinite(phase)) return SX_E_INVALID_ARG;
+    for (int k = 0; k < n; k++) if (!(h_lengths[k] > 0.0f) || !isfinite(h_lengths[k])) return SX_E_INVALID_ARG;
+    c->dash_period = 0;
+    for (int k = 0; k < 8; k++) c->dash_q[k] = 0;
+    for (int k = 0; k < n; k++) {
+        c->dash_q[k] = (unsigned long long)llrintf(h_lengths[k] * 65536.0f);   // units of 2^-16 px (R-23)
+        if (c->dash_q[k] == 0) c->dash_q[k] = 1;
+        c->dash_period += c->dash_q[k];
+    }
+    c->dash_phase_q = (unsigned long long)llrintf(phase * 65536.0f);
+    c->n_dash = (uint32_t)n;
     return SX_OK;
 }
 

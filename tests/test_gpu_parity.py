@@ -118,7 +118,7 @@ def gpu_run(B, ctx, sc, mode, host=False, into=False):
     return g
 
 
-def compare(sc, mode, g, r, min_parity=COUNT_PARITY):
+def compare(sc, mode, g, r, min_parity=COUNT_PARITY, angle_tol=ANGLE_TOL):
     """Element-by-element comparison; returns the count-parity fraction."""
     assert np.array_equal(g.pt_off, r.pt_off) and np.array_equal(g.path_idx, r.path_idx) and np.array_equal(g.sp_first, r.sp_first)
     same = g.seg_count == r.seg_count
@@ -136,7 +136,7 @@ def compare(sc, mode, g, r, min_parity=COUNT_PARITY):
     d = np.abs(g.xy[ig].astype(np.float64) - r.xy[io].astype(np.float64))
     check_coords(d, r.kind[io], f"{sc.name} mode {mode}")
     if mode == 1:
-        assert np.abs(g.angle[ig] - r.angle[io]).max(initial=0.0) <= ANGLE_TOL
+        assert np.abs(g.angle[ig] - r.angle[io]).max(initial=0.0) <= angle_tol
         assert np.array_equal(g.kind[ig], r.kind[io]) and np.array_equal(g.seg[ig], r.seg[io])
     if parity == 1.0:
         assert np.array_equal(g.path_off, r.path_off)

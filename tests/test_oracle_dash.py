@@ -228,3 +228,17 @@ def test_dashed_scenes_are_watertight_and_never_wind_negatively(name, npaths, mo
         assert (w >= 0).all()
         assert (w[d > kmax * h + sc.tolerance + 0.05] == 0).all()
         assert (w > 0).any()
+
+
+def test_a_filled_path_is_never_dashed():
+    """The pattern applies to stroked paths: a filled path that carries the dash bit, after a dashed stroke in the same call,
+    gives the records of the plain fill."""
+    base = S.make("c2", n_paths=40)
+    filled = S.with_fill(base, every=2, offset=1)
+    both = S.with_dash(filled, every=1)
+    r = run(both, [9.0, 4.0], 1.0)
+    r0 = oracle.expand(filled.tags, filled.points, filled.styles, filled.affine, filled.tolerance, 0)
+    for p in range(1, 40, 2):
+        a, b, a0, b0 = int(r.path_off[p]), int(r.path_off[p + 1]), int(r0.path_off[p]), int(r0.path_off[p + 1])
+        assert np.array_equal(r.xy[a:b].view(np.uint32), r0.xy[a0:b0].view(np.uint32))
+    assert int(((r.kind & 7) == K_CAP).sum()) > 0
