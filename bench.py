@@ -120,17 +120,22 @@ def job_throughput(units_per_rank_per_step, steps, world, seconds_max):
     return world * units_per_rank_per_step * steps / seconds_max
 
 
+DASH = None   # --dash: (pattern in px, phase) applied to every path
+DASH_PATTERN = ([30.0, 12.0, 6.0, 12.0], 7.0)
+
+
 def make_scene(workload, n_paths=None):
     from paper_2405_00127_b200 import scenes as S
-    return S.make(workload, n_paths=n_paths)
+    sc = S.make(workload, n_paths=n_paths)
+    return S.with_dash(sc) if DASH else sc
 
 
 # ---------------------------------------------------------------- the oracle on the host cores
 def _oracle_chunk(job):
     import oracle
-    tags, points, styles, affine, tol, mode = job
+    tags, points, styles, affine, tol, mode, dash = job
     t0 = time.perf_counter()
-    r = oracle.expand(tags, points, styles, affine, tol, mode)
+    r = oracle.expand(tags, points, styles, affine, tol, mode, dash=dash[0] if dash else None, phase=dash[1] if dash else 0.0)
     return time.perf_counter() - t0, r.n_rec, r.stats
 
 
@@ -142,7 +147,7 @@ def oracle_jobs(sc, mode, n_chunks):
     for a, b in zip(bounds[:-1], bounds[1:]):
         if b > a:
             sub, _ = S.subset_paths(sc, np.arange(a, b))
-            jobs.append((sub.tags, sub.points, sub.styles, sub.affine, float(sub.tolerance), mode))
+            jobs.append((sub.tags, sub.points, sub.styles, sub.affine, float(sub.tolerance), mode, DASH))
     return jobs
 
 
@@ -198,7 +203,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": args.workload, "mode": MODE_NAME[mode], "tolerance": float(sc.tolerance), "sample": sample},
+            "config": {"workload": args.workload, "mode": MODE_NAME[mode], "tolerance": float(sc.tolerance), "sample": sample, **({"dash": list(DASH[0]), "dash_phase": DASH[1]} if DASH else {})},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
@@ -243,6 +248,8 @@ def run_ours(args):
     sampler.begin()
     issue = B.sx_measure_issue_peaks(local)
     ctx = B.sx_create(local)
+    if DASH:
+        B.sx_set_dash(ctx, DASH[0], DASH[1])
     stream = torch.cuda.current_stream()
     poff = torch.empty(n_paths + 1, dtype=torch.int64, device=dev)
     total = B.sx_count(ctx, tags, pts, sty, sc.affine, sc.tolerance, mode, poff)
@@ -374,7 +381,7 @@ def run_ours(args):
         line = {"metric": METRIC, "value": job_throughput(n_seg, args.steps, world, t_total), "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": warm, "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": {"workload": args.workload, "segments": n_seg, "paths": n_paths, "records": int(total),
+                "config": {"workload": args.workload, **({"dash": list(DASH[0]), "dash_phase": DASH[1]} if DASH else {}), "segments": n_seg, "paths": n_paths, "records": int(total),
                            "mode": MODE_NAME[mode], "tolerance": float(sc.tolerance), "l2": "flushed between steps (256 MiB fill)",
                            "call": "stroke_expand_into (tag scan, count pass, allocation scan, writers; asynchronous, no host round trip)",
                            "parallelism": "replicas only" if world > 1 else "single GPU"},
@@ -409,7 +416,7 @@ def run_ours(args):
             line["cpu_baseline"] = {"value": sub.n_segments / dtn, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                                     "one_core": {"value": sub.n_segments / dt1, "cores": 1}}
             import oracle
-            r = oracle.expand(sub.tags, sub.points, sub.styles, sub.affine, sub.tolerance, mode)
+            r = oracle.expand(sub.tags, sub.points, sub.styles, sub.affine, sub.tolerance, mode, dash=DASH[0] if DASH else None, phase=DASH[1] if DASH else 0.0)
             i_fp32, i_mufu, units = unit_work(r.stats, r.kind, mode, n_seg / sub.n_segments)
             ceil = {"hbm_ms": 1e3 * alg_bytes / (peak * 1e9), "fp32_ms": 1e3 * i_fp32 / issue["fp32_ffma"], "mufu_ms": 1e3 * i_mufu / issue["mufu"]}
             bound = max(ceil, key=ceil.get)
@@ -425,6 +432,7 @@ def run_ours(args):
 
 
 def main():
+    global DASH
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
@@ -433,9 +441,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--mode", default=None, choices=["line", "arc", "refined"], help="override the workload's output mode (refined: SX_MODE_LINE_REFINED)")
+    ap.add_argument("--dash", action="store_true", help="dash every path with the pattern 30-12-6-12 px, phase 7 (SURVEY 8(f)-3: GPU dashing)")
     ap.add_argument("--binning", action="store_true", help="line mode: also time the tile binning of the records (SURVEY 8(f)-4)")
     ap.add_argument("--paths", type=int, default=None, help="profiling only: shrink the workload to this many paths")
     args = ap.parse_args()
+    if args.dash:
+        DASH = DASH_PATTERN
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # started by hand: become the launcher of N replicas, one process per GPU
         cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
