@@ -44,18 +44,6 @@ SX_DEV OffPlan plan_off(const PlanLite& q, bool second) {
 #endif
     return o;
 }
-SX_DEV EvoPlan plan_evo(const PlanLite& q);
-// the fields of the SidePlan that the part table is built from
-SX_DEV SidePlan plan_unpack(const PlanLite& q) {
-    SidePlan s;
-    s.eta = q.eta; s.seg = q.seg; s.total = (int)q.total;
-    s.nr = (q.flags & 1u) ? 2 : 1;
-    s.sup[0] = (q.flags & 2u) != 0u; s.sup[1] = (q.flags & 4u) != 0u;
-    s.off[0] = plan_off(q, false); s.off[1] = plan_off(q, true);
-    s.evo = plan_evo(q);
-    s.cusp_a = s.evo.ta != 0.0f; s.cusp_b = s.evo.tb != 1.0f;
-    return s;
-}
 SX_DEV EvoPlan plan_evo(const PlanLite& q) {
     EvoPlan e;
     const bool second = (q.flags & 1u) && !(q.flags & 2u);  // two ranges and the first one regular
@@ -90,46 +78,65 @@ SX_DEV uint32_t side_part_count(const SidePlan& s) {
     return c;
 }
 
-// writes the parts of a side (output order) to dst[0..count), and their tile-relative record prefixes to pref[]
-SX_DEV void side_parts(const SidePlan& s, uint32_t side_slot, bool mirror, bool arc, uint64_t side_base, uint32_t tile_prefix,
-                       uint32_t count, Part* dst, uint32_t* pref) {
-    uint32_t idx = 0, fwd = 0;  // forward part index, records before the part in forward order
-    const uint32_t total = (uint32_t)s.total;
-    auto push = [&](uint32_t n, int32_t i0, bool dirneg, uint32_t src, uint32_t ri, bool angle, uint32_t kind, uint32_t f0, uint32_t f1) {
-        Part q;
-        uint32_t pos = idx, before = fwd;
-        if (mirror) {  // reverse the list, reverse each chain
-            pos = count - 1u - idx; before = total - fwd - n;
-            i0 = dirneg ? i0 - (int32_t)n : i0 + (int32_t)n; dirneg = !dirneg;
-            uint32_t t = f0; f0 = f1; f1 = t;
-            kind |= kPlus;
-        }
-        q.base = side_base + before; q.n = (uint16_t)n; q.i0 = (uint16_t)i0;
-        q.info = side_slot | (dirneg ? 128u : 0u) | (src << 8) | (ri << 10) | ((angle && arc) ? 2048u : 0u) | (kind << 12) | (f0 << 16) | (f1 << 19);
-        dst[pos] = q;
-        pref[pos] = tile_prefix + before;
-        idx++; fwd += n;
-    };
-#pragma unroll 1
-    for (int r = 0; r < s.nr; r++) {
-        const OffPlan o = r == 0 ? s.off[0] : s.off[1];
-        const bool sup = r == 0 ? s.sup[0] : s.sup[1];
-        const uint32_t ca = end_code(o.ta), cb = end_code(o.tb);
-        if (!sup) {
-            push((uint32_t)o.n, 0, false, 1u, (uint32_t)r, true, kOffset, ca, cb);
+// part k (OUTPUT order) of the `count` parts of a side, and the number of the side's records before it: piece_side<true>
+// (sx_segment.cuh) turned into data, one part at a time -- the general writer builds its table with one lane per PART (a
+// lane per side spent 22 % of the kernel's instructions at 4 of 32 lanes on config 5, where a third of the pieces carry an
+// evolute patch of 7 parts).  Forward order of a side with a super-critical range [ta, tb] (section 6):
+// [regular range 0] [connector x2 unless the range starts at the cusp] [evolute x2] [reversed offset, L403 / L191]
+// [connector x2 unless it ends at the cusp] [regular range 1]; the mirror image of the +h side reverses the list and each chain.
+SX_DEV Part side_part_at(const PlanLite& q, uint32_t k, uint32_t count, uint32_t side_slot, bool mirror, bool arc, uint64_t side_base, uint32_t* before_out) {
+    const uint32_t idx = mirror ? count - 1u - k : k;
+    const bool two = (q.flags & 1u) != 0u, sup0 = (q.flags & 2u) != 0u, sup1 = two && (q.flags & 4u) != 0u;
+    const uint32_t n0 = q.n0, n1 = q.n1, ne = q.ne;
+    const float tc = q.tc;   // range 0 = [0, tc], range 1 = [tc, 1]; tc = 1 when there is one range
+    uint32_t n = 0, src = 1u, ri = 0u, kind = kOffset, f0 = 0u, f1 = 0u, fwd = 0u;
+    int32_t i0 = 0;
+    bool dirneg = false, angle = true;
+    if (!(sup0 || sup1)) {   // regular ranges only
+        ri = idx;
+        n = idx ? n1 : n0;
+        f0 = end_code(idx ? tc : 0.0f); f1 = end_code(idx ? 1.0f : tc);
+        fwd = idx ? n0 : 0u;
+    } else {
+        const uint32_t sr = sup0 ? 0u : 1u, nsr = sr ? n1 : n0;   // the super-critical range and its offset count
+        const float ta = sr ? tc : 0.0f, tb = sr ? 1.0f : tc;
+        const uint32_t ca = end_code(ta), cb = end_code(tb);
+        const bool cusp_a = ta != 0.0f, cusp_b = tb != 1.0f;
+        const uint32_t ea = cusp_a ? (uint32_t)kEndCusp : (ca | kEndEvo), eb = cusp_b ? (uint32_t)kEndCusp : (cb | kEndEvo);
+        const uint32_t nca = cusp_a ? 0u : 2u, ncb = cusp_b ? 0u : 2u;
+        uint32_t i = idx;
+        if (i < sr) {   // the regular range 0 before the patch
+            n = n0; f0 = end_code(0.0f); f1 = end_code(tc);
         } else {
-            // evolute patch (section 6): connectors x2, evolute x2, reversed offset, connectors x2;
-            // the evolute meets the offset curve at the cusp.  (Loops, not copies: code size.)
-            const uint32_t ea = s.cusp_a ? (uint32_t)kEndCusp : (ca | kEndEvo), eb = s.cusp_b ? (uint32_t)kEndCusp : (cb | kEndEvo);
-#pragma unroll 1
-            for (int c = 0; c < (s.cusp_a ? 0 : 2); c++) push(1u, 0, false, 0u, 0u, false, kConnector, ca, ea);
-#pragma unroll 1
-            for (int c = 0; c < 2; c++) push((uint32_t)s.evo.n, 0, false, 2u, 0u, true, kEvolute, ea, eb);   // (arc mode: the evolute turns with the spiral)
-            push((uint32_t)o.n, o.n, true, 1u, (uint32_t)r, true, kOffsetRev, cb, ca);  // L403, L191
-#pragma unroll 1
-            for (int c = 0; c < (s.cusp_b ? 0 : 2); c++) push(1u, 0, false, 0u, 0u, false, kConnector, eb, cb);
+            i -= sr; fwd = sr ? n0 : 0u;
+            if (i < nca) { n = 1u; src = 0u; angle = false; kind = kConnector; f0 = ca; f1 = ea; fwd += i; }
+            else {
+                i -= nca; fwd += nca;
+                if (i < 2u) { n = ne; src = 2u; kind = kEvolute; f0 = ea; f1 = eb; fwd += i * ne; }   // (arc mode: the evolute turns with the spiral)
+                else {
+                    fwd += 2u * ne;
+                    if (i == 2u) { n = nsr; i0 = (int32_t)nsr; dirneg = true; ri = sr; kind = kOffsetRev; f0 = cb; f1 = ca; }
+                    else {
+                        i -= 3u; fwd += nsr;
+                        if (i < ncb) { n = 1u; src = 0u; angle = false; kind = kConnector; f0 = eb; f1 = cb; fwd += i; }
+                        else { fwd += ncb; n = n1; ri = 1u; f0 = end_code(tc); f1 = end_code(1.0f); }   // the regular range 1 after the patch
+                    }
+                }
+            }
         }
     }
+    uint32_t before = fwd;
+    if (mirror) {   // reverse the list, reverse each chain
+        before = q.total - fwd - n;
+        i0 = dirneg ? i0 - (int32_t)n : i0 + (int32_t)n; dirneg = !dirneg;
+        const uint32_t t = f0; f0 = f1; f1 = t;
+        kind |= kPlus;
+    }
+    Part r;
+    r.base = side_base + before; r.n = (uint16_t)n; r.i0 = (uint16_t)i0;
+    r.info = side_slot | (dirneg ? 128u : 0u) | (src << 8) | (ri << 10) | ((angle && arc) ? 2048u : 0u) | (kind << 12) | (f0 << 16) | (f1 << 19);
+    *before_out = before;
+    return r;
 }
 
 // an END vertex of a part: same arithmetic as normal_point at t = 0 / t = 1; the cusp point is evaluated once per

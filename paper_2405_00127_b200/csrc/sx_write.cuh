@@ -311,7 +311,29 @@ k_write_general(const WriteArgs A) {
                 if (lane >= dd) { ip += a2; ir += b2; }
             }
             const uint32_t tparts = __shfl_sync(kFull, ip, 31), trecs = __shfl_sync(kFull, ir, 31);
-            if (np_) side_parts(plan_unpack(W.plan[lane]), (uint32_t)lane, side != 0, arc, base, ir - nr_, np_, &W.part[ip - np_], &W.ppref[ip - np_]);
+            // the part table, lane per PART: the owning side is the last lane whose first part is <= j (binary search by
+            // shuffles over the non-decreasing prefix), its plan is in shared memory, the part a closed form of its index
+            {
+                const uint32_t p_first = ip - np_, r_first = ir - nr_;
+                const uint32_t base_lo = (uint32_t)base, base_hi = (uint32_t)(base >> 32);
+                for (uint32_t j0 = 0; j0 < tparts; j0 += 32u) {
+                    const uint32_t j = j0 + (uint32_t)lane;
+                    uint32_t own = 0;
+#pragma unroll
+                    for (uint32_t step = 16u; step > 0u; step >>= 1) {
+                        const uint32_t cand = own + step;
+                        const uint32_t pc = __shfl_sync(kFull, p_first, (int)(cand & 31u));
+                        if (cand < 32u && pc <= j) own = cand;
+                    }
+                    const uint32_t o_first = __shfl_sync(kFull, p_first, (int)own), o_np = __shfl_sync(kFull, np_, (int)own), o_rec = __shfl_sync(kFull, r_first, (int)own);
+                    const uint64_t o_base = (uint64_t)__shfl_sync(kFull, base_lo, (int)own) | ((uint64_t)__shfl_sync(kFull, base_hi, (int)own) << 32);
+                    if (j < tparts) {
+                        uint32_t before;
+                        W.part[j] = side_part_at(W.plan[own], j - o_first, o_np, own, (own & 1u) != 0u, arc, o_base, &before);
+                        W.ppref[j] = o_rec + before;
+                    }
+                }
+            }
             if (lane == 0) W.ppref[tparts] = trecs;
             __syncwarp();
             const uint32_t tverts = trecs - tparts;
