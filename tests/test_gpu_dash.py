@@ -101,3 +101,17 @@ def test_dashed_fill_and_mixed_styles(B, ctx):
     g, r = dashed_pair(B, ctx, sc, 1, [14.0, 6.0], 2.5)
     compare(sc, 1, g, r, angle_tol=DASH_ANGLE_TOL)
     assert ck.watertight_violations(g.xy, g.path_off) == 0
+
+
+@pytest.mark.parametrize("dash,phase", [([7.0, 3.0], 0.0), ([0.01, 0.02], 0.005), ([1000.0, 5.0], 0.0), ([1000.0, 5.0], 998.0), ([50.0, 50.0], 50.0),
+                                        ([2.0 ** -9, 2.0 ** -9], 0.0)])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_dash_edge_scenes(B, ctx, dash, phase, mode):
+    """Zero-length segments at the start, in the middle and at the end of a dashed path, a degenerate cubic, a closed
+    triangle, dashes of 1/512 px and a pattern longer than the path (tests/test_oracle_dash.py::edge_scenes): the position
+    rules decide caps and joins identically on both sides."""
+    from test_oracle_dash import edge_scenes
+    sc = edge_scenes()
+    g, r = dashed_pair(B, ctx, sc, mode, dash, phase)
+    assert compare(sc, mode, g, r, min_parity=1.0, angle_tol=DASH_ANGLE_TOL) == 1.0
+    assert ck.watertight_violations(g.xy, g.path_off) == 0

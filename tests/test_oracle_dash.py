@@ -242,3 +242,34 @@ def test_a_filled_path_is_never_dashed():
         a, b, a0, b0 = int(r.path_off[p]), int(r.path_off[p + 1]), int(r0.path_off[p]), int(r0.path_off[p + 1])
         assert np.array_equal(r.xy[a:b].view(np.uint32), r0.xy[a0:b0].view(np.uint32))
     assert int(((r.kind & 7) == K_CAP).sum()) > 0
+
+
+def edge_scenes():
+    """Hand-built paths that stress the position rules: zero-length segments at the start, in the middle and at the end of a
+    dashed path, a degenerate cubic, a closed triangle, dashes much shorter than a segment and a pattern longer than the path."""
+    z = [40.0, 40.0]
+    paths = [
+        dict(start=z, segs=[[z], [[90, 40]], [[90, 40]], [[90, 95]], [[90, 95]]], width=5.0, cap=S.CAP_ROUND, join=S.JOIN_ROUND),
+        dict(start=[10, 10], segs=[[[10, 10], [10, 10], [10, 10]], [[60, 15], [20, 70], [80, 80]]], width=3.0, cap=S.CAP_SQUARE),
+        dict(start=[100, 100], segs=[[[160, 100]], [[130, 150]], [[100, 100]]], width=4.0, closed=True, join=S.JOIN_MITER),
+        dict(start=[200, 20], segs=[[[205, 20]]], width=1.0),
+        dict(start=[300, 300], segs=[[[340, 380], [420, 260], [460, 340]]], width=30.0, cap=S.CAP_BUTT),
+    ]
+    return S.with_dash(S.from_paths(paths))
+
+
+@pytest.mark.parametrize("dash,phase", [([7.0, 3.0], 0.0), ([0.01, 0.02], 0.005), ([1000.0, 5.0], 0.0), ([1000.0, 5.0], 998.0), ([50.0, 50.0], 50.0),
+                                        ([2.0 ** -9, 2.0 ** -9], 0.0)])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_edge_scenes_stay_watertight(dash, phase, mode):
+    sc = edge_scenes()
+    if dash[0] < 1e-3 and mode == 1:
+        pytest.skip("the finest patterns: line mode is enough")
+    r = run(sc, dash, phase, mode)
+    assert np.isfinite(r.xy).all() and ck.watertight_violations(r.xy, r.path_off) == 0
+    # the number of caps is twice the number of dashes; with the pattern longer than every path: one dash or none per subpath
+    caps_per_cap = {S.CAP_BUTT: 1, S.CAP_SQUARE: 3}
+    if dash[0] >= 1000.0 and phase == 0.0:
+        for p in (1, 3, 4):
+            a, b = int(r.path_off[p]), int(r.path_off[p + 1])
+            assert int(((r.kind[a:b] & 7) == K_CAP).sum()) == 2 * caps_per_cap[int(sc.styles[p]["cap"])]
