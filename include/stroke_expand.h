@@ -206,6 +206,27 @@ sx_status sx_bin_lines(sx_ctx* ctx, const sx_line* d_lines, uint64_t n_lines, ui
                        uint32_t* d_tile_offsets, uint32_t* d_tile_lines, uint64_t cap_entries, uint64_t* h_total,
                        void* cuda_stream);
 
+/* The same binning for callers that CANNOT ALLOCATE (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): no context, and the scratch (per-tile counters and cursors, look-back words of the scan) lives in a static
+ * device array of SX_STATIC_SCRATCH_BYTES that every GPU loading the library holds until the process exits.  The call issues
+ * memsets, kernels and one 4-byte device-to-device copy on cuda_stream and nothing else: no cudaMalloc, no cudaFree, no
+ * allocating library routine, no host synchronisation.
+ *   device                      the GPU the pointers belong to (made current by the call)
+ *   d_lines, n_lines, tiles_x, tiles_y, d_tile_offsets, d_tile_lines, cap_entries: as for sx_bin_lines; the pair total is
+ *                               d_tile_offsets[tiles_x * tiles_y] (device memory: read it after the stream has run)
+ *   d_flags                     device, optional, one word written at the end of the call: 0, or SX_STATIC_FLAG_CAPACITY when
+ *                               the pairs did not fit cap_entries or 32 bits (nothing is written past the capacity)
+ * LIMIT: tiles_x * tiles_y <= SX_STATIC_MAX_TILES (a viewport of 4096 x 4096 px); larger viewports are rejected with
+ * SX_E_INVALID_ARG (use sx_bin_lines).  All calls on one GPU share the static array, which keeps the last call's contents:
+ * each call clears what it uses first, and calls that OVERLAP on a GPU (different streams or host threads) RACE on it --
+ * serialise them.  Results are those of sx_bin_lines bit for bit (the offsets; a tile's records in no defined order). */
+#define SX_STATIC_MAX_TILES 65536u
+#define SX_STATIC_SCRATCH_BYTES 524672u
+#define SX_STATIC_FLAG_CAPACITY 2u
+sx_status sx_bin_lines_static(int32_t device, const sx_line* d_lines, uint64_t n_lines, uint32_t tiles_x, uint32_t tiles_y,
+                              uint32_t* d_tile_offsets, uint32_t* d_tile_lines, uint64_t cap_entries, uint32_t* d_flags,
+                              void* cuda_stream);
+
 /* ------------------------------------------------------------------ introspection
  * Device pointers into the context's scratch of the last sx_count (valid until the next call on the
  * context): the tag-scan results and the per-segment record counts / offsets.  Any out pointer may

@@ -24,7 +24,7 @@ ARC_DTYPE = np.dtype([("x0", "<f4"), ("y0", "<f4"), ("x1", "<f4"), ("y1", "<f4")
 SX_OPT_KEEP_SEGMENT_INFO, SX_OPT_TILE_SEGMENTS, SX_OPT_TIME_KERNELS = 1, 2, 3
 
 EXPORTS = ["sx_create", "sx_destroy", "sx_count", "sx_write", "stroke_expand", "stroke_expand_into", "stroke_expand_host",
-           "sx_bin_lines", "sx_segment_info", "sx_last_error", "sx_set_option", "sx_set_dash", "sx_call_stats", "sx_kernel_times", "sx_measure_issue_peaks", "sx_eval", "sx_launch_count",
+           "sx_bin_lines", "sx_bin_lines_static", "sx_segment_info", "sx_last_error", "sx_set_option", "sx_set_dash", "sx_call_stats", "sx_kernel_times", "sx_measure_issue_peaks", "sx_eval", "sx_launch_count",
            "sx_strerror"]
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
@@ -58,6 +58,7 @@ def lib():
         L.sx_last_error.argtypes = [vp, vp]
         L.sx_set_option.argtypes = [vp, i32, u64]
         L.sx_set_dash.argtypes = [vp, vp, i32, f32]
+        L.sx_bin_lines_static.argtypes = [i32, vp, u64, C.c_uint32, C.c_uint32, vp, vp, u64, vp, vp]
         L.sx_call_stats.argtypes = [vp, C.POINTER(u64), vp]
         L.sx_eval.argtypes = [C.c_int32, C.c_int32, vp, vp, u64]
         L.sx_bin_lines.argtypes = [vp, vp, u64, C.c_uint32, C.c_uint32, vp, vp, u64, C.POINTER(u64), vp]
@@ -231,6 +232,28 @@ def sx_bin_lines(ctx, lines, tiles_x, tiles_y, tile_offsets, tile_lines=None, wa
         raise e
     _check(st, "sx_bin_lines")
     return int(total.value) if want_total else None
+
+
+SX_STATIC_MAX_TILES, SX_STATIC_FLAG_CAPACITY = 65536, 2
+
+
+def sx_bin_lines_static(lines, tiles_x, tiles_y, tile_offsets, tile_lines=None, flags=None, stream=None):
+    """sx_bin_lines without a context and without any allocation (static device scratch; tiles_x * tiles_y <= 65536; calls that
+    overlap on one GPU race).  Asynchronous: the pair total is tile_offsets[tiles_x * tiles_y]; flags: optional int32 CUDA tensor
+    [1], written 0 or SX_STATIC_FLAG_CAPACITY.  The device is the tensors' device."""
+    assert lines.is_cuda and lines.is_contiguous() and lines.dtype == torch.float32 and lines.dim() == 2 and lines.shape[1] == 4
+    assert tile_offsets.is_cuda and tile_offsets.is_contiguous() and tile_offsets.element_size() == 4
+    assert tile_offsets.numel() >= int(tiles_x) * int(tiles_y) + 1
+    cap = 0
+    if tile_lines is not None:
+        assert tile_lines.is_cuda and tile_lines.is_contiguous() and tile_lines.element_size() == 4
+        cap = tile_lines.numel()
+    if flags is not None:
+        assert flags.is_cuda and flags.element_size() == 4 and flags.numel() >= 1
+    st = lib().sx_bin_lines_static(int(lines.device.index or 0), C.c_void_p(lines.data_ptr()), lines.shape[0], int(tiles_x), int(tiles_y),
+                                   C.c_void_p(tile_offsets.data_ptr()), C.c_void_p(tile_lines.data_ptr() if cap else 0), cap,
+                                   C.c_void_p(flags.data_ptr() if flags is not None else 0), _stream_ptr(stream))
+    _check(st, "sx_bin_lines_static")
 
 
 def _view(ptr, n, dtype, device):

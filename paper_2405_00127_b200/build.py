@@ -16,7 +16,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libstroke_expand.so")
 SOURCES = [os.path.join(CSRC, "sx_kernels.cu"), os.path.join(CSRC, "sx_refined.cu"),
-           os.path.join(CSRC, "sx_dash.cu")]   # (the second: the kernels of SX_MODE_LINE_REFINED; the third: dashing)
+           os.path.join(CSRC, "sx_dash.cu"),
+           os.path.join(CSRC, "sx_static.cu")]   # (the second: the kernels of SX_MODE_LINE_REFINED; the third: dashing; the fourth: sx_bin_lines_static)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-fmad=false",
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]
 
