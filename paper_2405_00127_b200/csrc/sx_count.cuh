@@ -22,9 +22,10 @@
 // regular ranges (one thread can write them) are stored from the FRONT of the leaf buffer, all others from the BACK
 // (one 64-bit atomic reserves both for a tile): the two kinds have their own writer.
 //
-// A tile whose nodes, points or leaves do not fit the tables is redone in SUB-TILES of 8 segments.  A sub-tile that
-// still does not fit, that meets a zero derivative at an interior subdivision point (the perturbation rule of L251
-// then depends on the visiting order), or whose leaves find no room in the leaf buffer, takes the thread-per-segment
+// A tile whose nodes, points or leaves do not fit the tables is redone in SUB-TILES of 8 segments, a sub-tile that still
+// does not fit is halved (8 -> 4 -> 2 -> 1).  What does not fit even alone, what meets a zero derivative at an interior
+// subdivision point (the perturbation rule of L251 then depends on the visiting order), and what finds no room for its
+// leaves in the leaf buffer takes the thread-per-segment
 // walk of sx_segment.cuh: its curve segments go to the WALK LIST, which the walk writer serves.  Same records, slower.
 // The tile size of a call comes from the context's hint word, which the last warp of every launch adapts to the
 // scene (pieces per segment seen) for the calls that follow.

@@ -114,7 +114,7 @@ k_write_segments(const WriteArgs A) {
     segment_tail_given<true>(P, tag, s, st, h, W, T1, &w, first);
 }
 
-// ---------------------------------------------------------------- simple leaves: thread per (leaf, side)
+// ---------------------------------------------------------------- simple leaves: thread per leaf
 // control points of a curve segment (quadratic or cubic) without its tangents: what load_segment_at computes, branch-free
 // (the same expressions, hence the same bits); l* / e*: the legs pick_tangent chooses the start / end tangent from
 struct Ctrl { V2 P0, P3, c1, c2, c3, l1, l2, l3, e1, e2, e3; };
