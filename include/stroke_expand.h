@@ -242,9 +242,9 @@ sx_status sx_last_error(sx_ctx* ctx, void* cuda_stream);
 enum {
     SX_OPT_KEEP_SEGMENT_INFO = 1, /* accepted and ignored: the per-segment counts / offsets are always kept              */
     SX_OPT_TIME_KERNELS = 3,      /* value != 0: the library records CUDA events around its kernels (sx_kernel_times)          */
-    SX_OPT_TILE_SEGMENTS = 2      /* test knob for the count pass, whose warps work on tiles of 32, 16, 8 or 4 segments
+    SX_OPT_TILE_SEGMENTS = 2      /* test knob for the count pass, whose warps work on tiles of 32, 16, 12, 8 or 4 segments
                                      (adapted on the device to what fits a warp's shared-memory tables): 0 adaptive
-                                     (default); 4 / 8 / 16 / 32 fixed; 2 = every tile is redone in sub-tiles of 8 segments
+                                     (default); any value from 4 to 32 fixed; 2 = every tile is redone in sub-tiles of 8 segments
                                      (the path of a tile that overflowed); 1 = every tile takes the thread-per-segment
                                      reference walk.  The records do not depend on it (tests/test_gpu_parity.py).      */
 };

@@ -48,7 +48,7 @@ constexpr int kDirectMax = 6;                        // records of a side that o
 constexpr int kCtWarpsPerSM = 16;
 constexpr uint32_t kFull = 0xffffffffu;
 
-enum : uint32_t { kForceWalk = 1u, kForceSub = 2u };   // CountArgs::force (test knob); 8, 16, 32 fix the tile size
+enum : uint32_t { kForceWalk = 1u, kForceSub = 2u };   // CountArgs::force (test knob); 4 .. 32 fix the tile size
 enum : int { kStDirect = 0, kStSub = 1, kStWalk = 2, kStLeaves = 3, kStSegs = 4, kStDone = 5, kStWords = 8 };
 
 // one Euler-spiral piece as the count pass hands it to the writers
@@ -194,7 +194,7 @@ k_count(const CountArgs A) {
     const uint32_t lt = (1u << lane) - 1u;
     const bool ok = (*A.err & kErrBadStream) == 0u;   // a malformed stream silences every segment
     uint32_t T = A.force >= (uint32_t)kCtTileMin ? A.force : *reinterpret_cast<volatile uint32_t*>(A.hint);
-    T = T >= 32u ? 32u : (T >= 16u ? 16u : (T >= 8u ? 8u : (uint32_t)kCtTileMin));
+    T = T >= 32u ? 32u : (T >= (uint32_t)kCtTileMin ? T : (uint32_t)kCtTileMin);   // any size from kCtTileMin to a warp's 32 lanes
     uint32_t st_direct = 0, st_sub = 0, st_walk = 0, st_leaves = 0, st_segs = 0;
 
     for (;;) {
@@ -476,8 +476,8 @@ k_count(const CountArgs A) {
             const uint32_t walked = *reinterpret_cast<volatile uint32_t*>(A.stats + kStWalk);
             if (segs >= 256u) {   // (a handful of segments says nothing about the scene)
                 const float per_seg = (float)leaves / (float)max(segs - walked, 1u);
-                const float room = 0.65f * (float)kCtLeafCap;
-                uint32_t next = per_seg * 32.0f <= room ? 32u : (per_seg * 16.0f <= room ? 16u : (per_seg * 8.0f <= room ? 8u : (uint32_t)kCtTileMin));
+                const float room = 0.65f * (float)kCtLeafCap, room12 = 0.72f * (float)kCtLeafCap;   // (12: config 5, 8.5 pieces per segment, count pass - 17 % against 8)
+                uint32_t next = per_seg * 32.0f <= room ? 32u : (per_seg * 16.0f <= room ? 16u : (per_seg * 12.0f <= room12 ? 12u : (per_seg * 8.0f <= room ? 8u : (uint32_t)kCtTileMin)));
                 if (walked * 4u >= segs) next = (uint32_t)kCtTileMin;   // a launch that mostly walked: its pieces were not counted
                 A.hint[1] = next;
             }

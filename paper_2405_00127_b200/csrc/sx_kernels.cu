@@ -43,7 +43,7 @@ struct sx_ctx {
     double leaves_per_seg;  // the most a call on this context has needed so far (learned whenever a call reads its total)
     uint8_t* sync_area;   // [flags, tickets, statistics, counters: 128 B][d_total 128 B][look-back words of the allocation scan][tag tile states]
     uint64_t sync_bytes;
-    uint32_t* d_hint;     // [0] tile size of the call in flight, [1] the one the last count pass proposed (adapted on the device, kept across calls)
+    uint32_t* d_hint;     // [0] tile size of the call in flight, [1] the one the last count pass proposed, [2] [3] its feedback state (adapted on the device, kept across calls)
     uint64_t* h_pinned;   // pinned: [0] total, [1] flags, [2..3] stats, [4] leaf counter
     int sm_count;
     int count_blocks, simple_blocks, general_blocks;   // persistent grids: resident blocks on the device
@@ -330,8 +330,8 @@ sx_status sx_create(sx_ctx** out, int32_t device) {
     cudaError_t e = cudaMallocHost(reinterpret_cast<void**>(&c->h_pinned), 64);
     if (e != cudaSuccess) { g_last_cuda = e; free(c); return SX_E_CUDA; }
     e = cudaMalloc(&c->d_hint, 64);
-    uint32_t first[2] = {(uint32_t)sx::kCtTile, (uint32_t)sx::kCtTile};
-    if (e == cudaSuccess) e = cudaMemcpy(c->d_hint, first, 8, cudaMemcpyHostToDevice);
+    uint32_t first[16] = {(uint32_t)sx::kCtTile, (uint32_t)sx::kCtTile};   // [2] the share of the tables (float bits, 0: unset), [3] pieces per segment last seen
+    if (e == cudaSuccess) e = cudaMemcpy(c->d_hint, first, 64, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(sx::k_count, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(sx::CtWarp));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(sx::k_count, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     int per_sm = 0;
@@ -594,7 +594,7 @@ sx_status sx_set_option(sx_ctx* c, int32_t option, uint64_t value) {
         case SX_OPT_KEEP_SEGMENT_INFO: return SX_OK;   // (kept for compatibility: the per-segment results are always there)
         case SX_OPT_TIME_KERNELS: c->time_kernels = value != 0; c->timed = false; return SX_OK;
         case SX_OPT_TILE_SEGMENTS:
-            if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8 && value != 16 && value != 32) return SX_E_INVALID_ARG;
+            if (value != 0 && value != 1 && value != 2 && (value < 4 || value > 32)) return SX_E_INVALID_ARG;
             c->force_tiles = static_cast<uint32_t>(value);
             return SX_OK;
         default: return SX_E_INVALID_ARG;

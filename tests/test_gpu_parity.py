@@ -227,7 +227,7 @@ def test_tiling_of_the_expansion_kernel_does_not_change_a_bit(B, name, npaths, m
     tags, pts, sty = B.scene_to_torch(sc, device=dev)
     width = 8 if mode == 1 else 4
     outs = []
-    for tiles in (1, 2, 4, 8, 16, 32, 0):
+    for tiles in (1, 2, 4, 8, 12, 16, 27, 32, 0):
         c = B.sx_create(0)
         try:
             B.sx_set_option(c, B.SX_OPT_TILE_SEGMENTS, tiles)
