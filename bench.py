@@ -38,7 +38,7 @@ MODE_NAME = {0: "line", 1: "arc", 2: "line-refined"}
 MODE_OF = {"c3": 0, "c4": 1, "c5": 0, "c1": 0, "c2": 0}
 # whole-step dram__bytes_read.sum + dram__bytes_write.sum per step from the committed `ncu --set full` captures
 # (profiles/r2_counters.md names the command and the commit of each); None = not captured for that workload / mode
-NCU_TRAFFIC = {"c4-arc": 523.8e6, "c5-line": 23100e6, "c5-arc": 24412e6, "c3-line": 74.3e6}
+NCU_TRAFFIC = {"c4-arc": 525.9e6, "c5-line": 23232e6, "c5-arc": 24513e6, "c3-line": 74.3e6}
 NCU_TRAFFIC_SOURCE = "profiles/r2_counters.md"
 REF_SAMPLE_PATHS = {"c4": 20000, "c5": 1000, "c3": 20000, "c1": 256, "c2": 2000}
 # issue slots (FMA = 1) and special-function operations per unit of the method's own work
