@@ -22,6 +22,8 @@
 
 // ====================================================================== host side
 static thread_local cudaError_t g_last_cuda = cudaSuccess;
+// (for the library's other translation units: sx_strerror(SX_E_CUDA) reports the last CUDA error of the calling thread)
+void sx_internal_note_cuda_error(int e) { g_last_cuda = static_cast<cudaError_t>(e); }
 
 #define SX_CUDA(call)                                      \
     do {                                                   \

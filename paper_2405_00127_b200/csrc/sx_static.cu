@@ -20,6 +20,8 @@
 #include "../../include/stroke_expand.h"
 #include <mutex>
 
+void sx_internal_note_cuda_error(int e);   // sx_kernels.cu: what sx_strerror(SX_E_CUDA) reports
+
 namespace {
 
 constexpr uint32_t kStaticMaxTiles = SX_STATIC_MAX_TILES;
@@ -38,7 +40,6 @@ constexpr int kMaxDevices = 64;
 struct DeviceSetup { unsigned char* scratch; int sm_count; bool ready; };
 DeviceSetup g_setup[kMaxDevices];
 std::mutex g_setup_mutex;
-thread_local cudaError_t g_static_cuda = cudaSuccess;
 
 // once per device, that device current: the DEVICE address of the array (its name is only a stand-in on the host)
 sx_status setup_device(int device, DeviceSetup* out) {
@@ -47,10 +48,10 @@ sx_status setup_device(int device, DeviceSetup* out) {
     if (!d.ready) {
         unsigned char* ptr = nullptr;
         cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_static_scratch);
-        if (e != cudaSuccess || ptr == nullptr) { g_static_cuda = e; return SX_E_CUDA; }
+        if (e != cudaSuccess || ptr == nullptr) { sx_internal_note_cuda_error((int)e); return SX_E_CUDA; }
         int sms = 0;
         e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
-        if (e != cudaSuccess) { g_static_cuda = e; return SX_E_CUDA; }
+        if (e != cudaSuccess) { sx_internal_note_cuda_error((int)e); return SX_E_CUDA; }
         d.scratch = ptr;
         d.sm_count = sms > 0 ? sms : 148;
         d.ready = true;
@@ -64,7 +65,7 @@ sx_status setup_device(int device, DeviceSetup* out) {
 #define SXS_CUDA(call)                                                      \
     do {                                                                    \
         cudaError_t e_ = (call);                                            \
-        if (e_ != cudaSuccess) { g_static_cuda = e_; return SX_E_CUDA; }    \
+        if (e_ != cudaSuccess) { sx_internal_note_cuda_error((int)e_); return SX_E_CUDA; }    \
     } while (0)
 
 sx_status sx_bin_lines_static(int32_t device, const sx_line* d_lines, uint64_t n_lines, uint32_t tiles_x, uint32_t tiles_y,
